@@ -1,0 +1,167 @@
+/* su3stream.h -- C ABI of libsu3stream: lattice-wide, site-wise SU(3)xSU(3)
+ * streaming products on NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute follows arXiv:1710.09409 (P:N = PAPER.md line N):
+ *   - a lattice field = one object per (outer) site, `Lattice<obj>`        P:76-89,  Listing 1
+ *   - obj = complex 3x3 matrix (`Su3f`), the streaming test `z = x*y`      P:113-126, section 4, Listing 3
+ *   - composite expressions evaluated in ONE pass over the sites           P:91-109, Listing 2
+ *   - scalar ("naive", AoS) layout
+ *   - vector layout: the lattice is split into N_sub virtual nodes, the
+ *     split lives at the level of the basic complex type
+ *   - extract / merge: lane l of each of the 9 element vectors <-> one
+ *     scalar 3x3 matrix (this defines su3_convert)                         P:174-181, Listing 4
+ *   - a same-run streaming ceiling next to every bandwidth number          P:199-201 (STREAM triad lines)
+ * Where the paper is silent the readings S1..S19 of DESIGN.md apply.
+ *
+ * Conventions (all calls)
+ *   - extern "C", plain pointers and sizes; no exceptions cross the ABI.
+ *   - DEVICE memory is the caller's (e.g. a torch tensor): su3_field_wrap records
+ *     the pointer and never allocates, frees or touches it.  A su3_field handle is
+ *     host memory owned by the library until su3_field_free.
+ *   - Every call returns su3_status.  On failure nothing is launched, outputs are
+ *     untouched, and su3_last_error() (thread-local) describes the failure.
+ *   - Arithmetic calls enqueue on `cuda_stream` (a cudaStream_t passed as void*;
+ *     NULL = legacy default stream) and return without synchronising.
+ *   - `z` may be the SAME field as any input.  Partially overlapping fields are
+ *     undefined.
+ *   - Handles are immutable after wrap; calls are thread-safe (su3_tune_set is a
+ *     process-wide knob and is the one exception: do not race it with launches).
+ *   - There is no CPU fallback anywhere: without a CUDA device the arithmetic
+ *     calls return SU3_ERR_CUDA.
+ *
+ * Data layout (reals are IEEE fp32 or fp64; a complex number is (re, im) adjacent)
+ *   matrix element (i,j) is e = 3*i + j (row-major, S1); matrix index of (site, mu)
+ *   is m = site*n_lorentz + mu (S6); site = x0 + L0*(x1 + L1*(x2 + L2*x3)) (S2).
+ *   SU3_SCALAR : real offset = (m*9 + e)*2 + reim
+ *   SU3_VECTOR : real offset = (((o*n_lorentz + mu)*9 + e)*W + l)*2 + reim, with
+ *                r[d] = L[d]/simd[d], oc[d] = x[d] mod r[d], ic[d] = x[d] div r[d],
+ *                o = lexicographic index of oc over r, l = lexicographic index of ic
+ *                over simd, both d=0 fastest (the virtual-node map, S3).
+ *   Default split of W over the dimensions (simd all 0, S4): factors of two handed
+ *   out starting at d=3 and moving down, wrapping: 2->{1,1,1,2} 4->{1,1,2,2}
+ *   8->{1,2,2,2} 16->{2,2,2,2} 32->{2,2,2,4}.
+ */
+#ifndef SU3STREAM_H
+#define SU3STREAM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SU3_OK = 0,
+  SU3_ERR_NULL = 1,     /* a required pointer argument is NULL                       */
+  SU3_ERR_INVALID = 2,  /* bad enum, L[d]<=0, n_lorentz not in {1,4}, W not a power
+                           of two in 1..32, W!=1 with SU3_SCALAR, prod(simd)!=W,
+                           L[d] % simd[d] != 0                                      */
+  SU3_ERR_MISMATCH = 3, /* operands disagree in L, n_lorentz, prec (and, for the
+                           arithmetic calls, layout / W / simd)                     */
+  SU3_ERR_ALIGN = 4,    /* device pointer not 16-byte aligned                        */
+  SU3_ERR_SIZE = 5,     /* buffer smaller than su3_field_bytes                       */
+  SU3_ERR_CUDA = 6      /* CUDA runtime error (string in su3_last_error)             */
+} su3_status;
+
+typedef enum { SU3_F32 = 4, SU3_F64 = 8 } su3_prec;          /* bytes per real */
+typedef enum { SU3_SCALAR = 0, SU3_VECTOR = 1 } su3_layout;
+
+/* Plain data, caller-owned, copied on use. */
+typedef struct {
+  int32_t L[4];      /* lattice extents                                              */
+  int32_t n_lorentz; /* 1 (colour-matrix field) or 4 (gauge-field shape)             */
+  int32_t prec;      /* su3_prec                                                     */
+  int32_t layout;    /* su3_layout                                                   */
+  int32_t W;         /* sites interleaved lane-wise; must be 1 for SU3_SCALAR        */
+  int32_t simd[4];   /* virtual-node grid, product = W; all 0 => default split (S4)  */
+} su3_desc;
+
+typedef struct su3_field su3_field; /* opaque: validated descriptor + device pointer */
+
+/* Launch knobs of the streaming pipeline (process-wide; 0 = library default).
+ * They never change results, only speed; bench.py and the tests use them to pin
+ * the launch configuration that is being measured. */
+typedef struct {
+  int32_t tile_mats;    /* matrices per pipeline tile: 32, 64, 128 or 256               */
+  int32_t stages;       /* shared-memory ring depth, 2..16                             */
+  int32_t ctas_per_sm;  /* persistent CTAs per SM, 1..8                                 */
+  int32_t l2_hint;      /* 0 auto (by footprint), 1 none, 2 evict_first loads+stores   */
+  int32_t path;         /* 0 auto, 1 TMA-bulk staged pipeline, 2 direct per-lane LDG   */
+  int32_t reserved[3];
+} su3_tune;
+
+/* Never NULL; thread-local; valid until the next failing call on this thread. */
+const char *su3_last_error(void);
+
+/* Library version string, e.g. "su3stream 0.1 (sm_100a)". */
+const char *su3_version(void);
+
+/* Bytes a field of this descriptor occupies: volume * n_lorentz * 18 * prec.
+ * Validates the descriptor (SU3_ERR_INVALID).  Host-only, needs no GPU. */
+su3_status su3_field_bytes(const su3_desc *desc, size_t *nbytes);
+
+/* Normalise a descriptor: validates it and fills simd[] with the split in use. */
+su3_status su3_desc_normalize(const su3_desc *desc, su3_desc *out);
+
+/* Wrap caller-owned DEVICE memory.  dev_ptr must be 16-byte aligned (SU3_ERR_ALIGN)
+ * and nbytes >= su3_field_bytes (SU3_ERR_SIZE).  Host-only bookkeeping. */
+su3_status su3_field_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out);
+su3_status su3_field_free(su3_field *f); /* frees the handle only, never the device memory */
+su3_status su3_field_desc(const su3_field *f, su3_desc *out); /* normalised descriptor     */
+su3_status su3_field_ptr(const su3_field *f, void **dev_ptr, size_t *nbytes);
+
+/* Host-side index map (for tests and for filling a field by hand): offset IN REALS of
+ * (site, mu, row i, col j, reim) for this descriptor.  SU3_ERR_INVALID if out of range. */
+su3_status su3_index(const su3_desc *desc, int64_t site, int mu, int i, int j, int reim, int64_t *off);
+
+/* z = x*y, site by site: z_ij = sum_k x_ik y_kj (Listing 3).  All three fields
+ * must have identical descriptors (SU3_ERR_MISMATCH).  A1 (scalar) / A2 (vector). */
+su3_status su3_mul(su3_field *z, const su3_field *x, const su3_field *y, void *cuda_stream);
+
+/* z = (x*y)*w in one pass, x*y kept in registers (composite expressions are
+ * evaluated inside the one site loop; left-associative as C++ parses x*y*w).  A3. */
+su3_status su3_mul3(su3_field *z, const su3_field *x, const su3_field *y, const su3_field *w, void *cuda_stream);
+
+/* z = x*y + v in one pass (the `v1+v2+v1*v2` pattern of P:104-106 on matrices).  A4. */
+su3_status su3_mul_add(su3_field *z, const su3_field *x, const su3_field *y, const su3_field *v, void *cuda_stream);
+
+/* z = x + y, element-wise (P:104 `v3=v1+v2`).  Also the 2-read-1-write streaming
+ * reference (the analogue of the paper's STREAM line). */
+su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *cuda_stream);
+
+/* Layout conversion scalar <-> vector: a pure, bit-exact permutation of complex numbers,
+ * vec[o][mu][e][l] = sca[site(o,l)][mu][e] (extract/merge).  Exactly one of
+ * dst/src must be SU3_SCALAR and the other SU3_VECTOR; L, n_lorentz, prec must agree
+ * (SU3_ERR_MISMATCH).  dst and src must not alias.  A5. */
+su3_status su3_convert(su3_field *dst, const su3_field *src, void *cuda_stream);
+
+/* dst = src, own 128-bit copy kernel: the same-run bandwidth ceiling.  Fields
+ * must have identical descriptors.  A6. */
+su3_status su3_copy(su3_field *dst, const su3_field *src, void *cuda_stream);
+
+/* End-to-end z = x*y with HOST buffers: x_host, y_host (inputs) and z_host (output) are host
+ * arrays of su3_field_bytes bytes in the layout of the (identical) descriptors of the three
+ * DEVICE staging fields zd, xd, yd.  Enqueues, on cuda_stream, chunked host->device copies
+ * of x and y, the product kernel per chunk, and the device->host copy of z, overlapped on
+ * internal copy streams, then makes cuda_stream wait for all of it.  Does not synchronise
+ * the host; pinned host memory is needed for the copies to be asynchronous.  `chunks` <= 0
+ * picks a default. */
+su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host,
+                        su3_field *zd, su3_field *xd, su3_field *yd, int chunks, void *cuda_stream);
+
+/* Launch knobs (see su3_tune).  su3_tune_set(NULL) restores the defaults. */
+su3_status su3_tune_set(const su3_tune *t);
+su3_status su3_tune_get(su3_tune *out);
+
+/* Number of kernels this library has launched in this process (monotonic). */
+int64_t su3_launch_count(void);
+
+/* Device facts the harness prints next to its numbers: SM count, L2 bytes, memory clock
+ * (kHz), bus width (bits), of the current CUDA device.  SU3_ERR_CUDA without a device. */
+su3_status su3_device_info(int32_t *sm_count, int64_t *l2_bytes, int32_t *mem_clock_khz, int32_t *bus_width_bits);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SU3STREAM_H */

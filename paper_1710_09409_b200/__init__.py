@@ -1,0 +1,211 @@
+"""Thin Python binding of libsu3stream (include/su3stream.h): argument marshalling only.
+
+Every step of the hot path (z = x*y, the fused expressions, the layout permutation, the
+copy ceiling; arXiv:1710.09409 section 4/5) runs
+in the library's CUDA kernels.  PyTorch supplies device memory and streams, nothing else.
+There is no CPU fallback: if the shared library cannot be built or loaded, importing this
+package raises.
+"""
+import ctypes
+
+from ._build import build as _build_lib
+
+SU3_OK, SU3_ERR_NULL, SU3_ERR_INVALID, SU3_ERR_MISMATCH, SU3_ERR_ALIGN, SU3_ERR_SIZE, SU3_ERR_CUDA = range(7)
+SU3_F32, SU3_F64 = 4, 8
+SU3_SCALAR, SU3_VECTOR = 0, 1
+
+EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
+           "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
+           "su3_mul_add", "su3_add", "su3_convert", "su3_copy", "su3_mul_host", "su3_tune_set",
+           "su3_tune_get", "su3_launch_count", "su3_device_info"]
+
+
+class su3_desc(ctypes.Structure):
+    _fields_ = [("L", ctypes.c_int32 * 4), ("n_lorentz", ctypes.c_int32), ("prec", ctypes.c_int32),
+                ("layout", ctypes.c_int32), ("W", ctypes.c_int32), ("simd", ctypes.c_int32 * 4)]
+
+
+class su3_tune(ctypes.Structure):
+    _fields_ = [("tile_mats", ctypes.c_int32), ("stages", ctypes.c_int32), ("ctas_per_sm", ctypes.c_int32),
+                ("l2_hint", ctypes.c_int32), ("path", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
+
+
+class Su3Error(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("su3_status %d: %s" % (status, message))
+        self.status = status
+
+
+def _load():
+    lib = ctypes.CDLL(_build_lib())
+    vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+    D, T = ctypes.POINTER(su3_desc), ctypes.POINTER(su3_tune)
+    sig = {
+        "su3_last_error": (ctypes.c_char_p, []),
+        "su3_version": (ctypes.c_char_p, []),
+        "su3_field_bytes": (i32, [D, ctypes.POINTER(sz)]),
+        "su3_desc_normalize": (i32, [D, D]),
+        "su3_field_wrap": (i32, [D, vp, sz, ctypes.POINTER(vp)]),
+        "su3_field_free": (i32, [vp]),
+        "su3_field_desc": (i32, [vp, D]),
+        "su3_field_ptr": (i32, [vp, ctypes.POINTER(vp), ctypes.POINTER(sz)]),
+        "su3_index": (i32, [D, i64, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(i64)]),
+        "su3_mul": (i32, [vp, vp, vp, vp]),
+        "su3_mul3": (i32, [vp, vp, vp, vp, vp]),
+        "su3_mul_add": (i32, [vp, vp, vp, vp, vp]),
+        "su3_add": (i32, [vp, vp, vp, vp]),
+        "su3_convert": (i32, [vp, vp, vp]),
+        "su3_copy": (i32, [vp, vp, vp]),
+        "su3_mul_host": (i32, [vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]),
+        "su3_tune_set": (i32, [T]),
+        "su3_tune_get": (i32, [T]),
+        "su3_launch_count": (i64, []),
+        "su3_device_info": (i32, [ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), ctypes.POINTER(i32)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+lib = _load()  # fails loudly if the CUDA library is missing
+
+
+def _ck(status):
+    if status != SU3_OK:
+        raise Su3Error(status, lib.su3_last_error().decode())
+
+
+def su3_last_error():
+    return lib.su3_last_error().decode()
+
+
+def su3_version():
+    return lib.su3_version().decode()
+
+
+def make_desc(L, n_lorentz=1, prec=SU3_F64, layout=SU3_SCALAR, W=1, simd=None):
+    d = su3_desc()
+    L = (int(L),) * 4 if isinstance(L, int) else tuple(int(v) for v in L)
+    d.L[:] = L
+    d.n_lorentz, d.prec, d.layout, d.W = int(n_lorentz), int(prec), int(layout), int(W)
+    d.simd[:] = tuple(int(v) for v in simd) if simd is not None else (0, 0, 0, 0)
+    return d
+
+
+def su3_field_bytes(desc):
+    n = ctypes.c_size_t()
+    _ck(lib.su3_field_bytes(ctypes.byref(desc), ctypes.byref(n)))
+    return n.value
+
+
+def su3_desc_normalize(desc):
+    out = su3_desc()
+    _ck(lib.su3_desc_normalize(ctypes.byref(desc), ctypes.byref(out)))
+    return out
+
+
+def su3_index(desc, site, mu, i, j, reim):
+    off = ctypes.c_int64()
+    _ck(lib.su3_index(ctypes.byref(desc), int(site), int(mu), int(i), int(j), int(reim), ctypes.byref(off)))
+    return off.value
+
+
+class Field:
+    """A su3_field handle plus the torch tensor that owns its device memory."""
+
+    def __init__(self, desc, tensor):
+        self.tensor = tensor  # keeps the memory alive as long as the handle
+        h = ctypes.c_void_p()
+        _ck(lib.su3_field_wrap(ctypes.byref(desc), ctypes.c_void_p(tensor.data_ptr()),
+                               tensor.numel() * tensor.element_size(), ctypes.byref(h)))
+        self.handle = h
+        self.desc = su3_field_desc(self)
+        self.nbytes = su3_field_bytes(self.desc)
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h:
+            lib.su3_field_free(h)
+
+
+def su3_field_wrap(desc, tensor):
+    return Field(desc, tensor)
+
+
+def su3_field_desc(field):
+    out = su3_desc()
+    _ck(lib.su3_field_desc(field.handle, ctypes.byref(out)))
+    return out
+
+
+def su3_field_ptr(field):
+    p, n = ctypes.c_void_p(), ctypes.c_size_t()
+    _ck(lib.su3_field_ptr(field.handle, ctypes.byref(p), ctypes.byref(n)))
+    return p.value, n.value
+
+
+def alloc_field(desc, device="cuda"):
+    """north_star "allocate a field": su3_field_bytes -> torch.empty -> su3_field_wrap."""
+    import torch
+    return Field(desc, torch.empty(su3_field_bytes(desc), dtype=torch.uint8, device=device))
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(int(stream))
+
+
+def su3_mul(z, x, y, stream=None):
+    _ck(lib.su3_mul(z.handle, x.handle, y.handle, _stream(stream)))
+
+
+def su3_mul3(z, x, y, w, stream=None):
+    _ck(lib.su3_mul3(z.handle, x.handle, y.handle, w.handle, _stream(stream)))
+
+
+def su3_mul_add(z, x, y, v, stream=None):
+    _ck(lib.su3_mul_add(z.handle, x.handle, y.handle, v.handle, _stream(stream)))
+
+
+def su3_add(z, x, y, stream=None):
+    _ck(lib.su3_add(z.handle, x.handle, y.handle, _stream(stream)))
+
+
+def su3_convert(dst, src, stream=None):
+    _ck(lib.su3_convert(dst.handle, src.handle, _stream(stream)))
+
+
+def su3_copy(dst, src, stream=None):
+    _ck(lib.su3_copy(dst.handle, src.handle, _stream(stream)))
+
+
+def su3_mul_host(z_host, x_host, y_host, zd, xd, yd, chunks=0, stream=None):
+    """z_host, x_host, y_host: host tensors/arrays exposing .data_ptr() or .ctypes.data."""
+    def hp(a):
+        return ctypes.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+    _ck(lib.su3_mul_host(hp(z_host), hp(x_host), hp(y_host), zd.handle, xd.handle, yd.handle, int(chunks),
+                         _stream(stream)))
+
+
+def su3_tune_set(tile_mats=0, stages=0, ctas_per_sm=0, l2_hint=0, path=0):
+    t = su3_tune(int(tile_mats), int(stages), int(ctas_per_sm), int(l2_hint), int(path))
+    _ck(lib.su3_tune_set(ctypes.byref(t)))
+
+
+def su3_tune_get():
+    t = su3_tune()
+    _ck(lib.su3_tune_get(ctypes.byref(t)))
+    return dict(tile_mats=t.tile_mats, stages=t.stages, ctas_per_sm=t.ctas_per_sm, l2_hint=t.l2_hint, path=t.path)
+
+
+def su3_launch_count():
+    return int(lib.su3_launch_count())
+
+
+def su3_device_info():
+    sm, l2, mk, bw = ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32()
+    _ck(lib.su3_device_info(ctypes.byref(sm), ctypes.byref(l2), ctypes.byref(mk), ctypes.byref(bw)))
+    return dict(sm_count=sm.value, l2_bytes=l2.value, mem_clock_khz=mk.value, bus_width_bits=bw.value)

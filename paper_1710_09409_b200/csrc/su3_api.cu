@@ -1,0 +1,513 @@
+// su3_api.cu -- the C ABI of libsu3stream (include/su3stream.h): descriptor validation,
+// field handles, kernel selection and launch.  Host logic only; the arithmetic lives in
+// su3_kernels.cuh.  No CPU fallback: without a CUDA device every arithmetic call fails
+// with SU3_ERR_CUDA.
+#include "../../include/su3stream.h"
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "su3_kernels.cuh"
+
+struct su3_field {
+  su3_desc d;  // normalised
+  void *ptr;
+  size_t nbytes;
+  int64_t volume;
+  int64_t nmat;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<int64_t> g_launches{0};
+std::mutex g_tune_mu;
+su3_tune g_tune = {0, 0, 0, 0, 0, {0, 0, 0}};
+
+su3_status fail(su3_status st, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+void default_simd(int W, int32_t simd[4]) {  // reading S4
+  for (int d = 0; d < 4; d++) simd[d] = 1;
+  for (int d = 3; W > 1; W >>= 1, d = (d + 3) & 3) simd[d] *= 2;
+}
+
+su3_status normalize(const su3_desc *in, su3_desc *out) {
+  if (!in || !out) return fail(SU3_ERR_NULL, "descriptor pointer is NULL");
+  su3_desc d = *in;
+  for (int k = 0; k < 4; k++)
+    if (d.L[k] <= 0) return fail(SU3_ERR_INVALID, "L[%d] = %d must be positive", k, d.L[k]);
+  if (d.n_lorentz != 1 && d.n_lorentz != 4) return fail(SU3_ERR_INVALID, "n_lorentz = %d not in {1,4}", d.n_lorentz);
+  if (d.prec != SU3_F32 && d.prec != SU3_F64) return fail(SU3_ERR_INVALID, "prec = %d not in {4,8}", d.prec);
+  if (d.layout != SU3_SCALAR && d.layout != SU3_VECTOR) return fail(SU3_ERR_INVALID, "layout = %d not in {0,1}", d.layout);
+  if (d.W < 1 || d.W > 32 || (d.W & (d.W - 1))) return fail(SU3_ERR_INVALID, "W = %d is not a power of two in 1..32", d.W);
+  if (d.layout == SU3_SCALAR && d.W != 1) return fail(SU3_ERR_INVALID, "W = %d must be 1 for the scalar layout", d.W);
+  bool any = false;
+  for (int k = 0; k < 4; k++) any = any || d.simd[k] != 0;
+  if (any) {
+    long prod = 1;
+    for (int k = 0; k < 4; k++) {
+      if (d.simd[k] <= 0) return fail(SU3_ERR_INVALID, "simd[%d] = %d must be positive", k, d.simd[k]);
+      prod *= d.simd[k];
+    }
+    if (prod != d.W) return fail(SU3_ERR_INVALID, "prod(simd) = %ld differs from W = %d", prod, d.W);
+  } else {
+    default_simd(d.W, d.simd);
+  }
+  for (int k = 0; k < 4; k++)
+    if (d.L[k] % d.simd[k]) return fail(SU3_ERR_INVALID, "L[%d] = %d not divisible by simd[%d] = %d", k, d.L[k], k, d.simd[k]);
+  *out = d;
+  return SU3_OK;
+}
+
+int64_t volume_of(const su3_desc &d) { return (int64_t)d.L[0] * d.L[1] * d.L[2] * d.L[3]; }
+
+bool same_lattice(const su3_desc &a, const su3_desc &b) {
+  return !memcmp(a.L, b.L, sizeof a.L) && a.n_lorentz == b.n_lorentz && a.prec == b.prec;
+}
+bool same_desc(const su3_desc &a, const su3_desc &b) {
+  return same_lattice(a, b) && a.layout == b.layout && a.W == b.W && !memcmp(a.simd, b.simd, sizeof a.simd);
+}
+
+// ---------------------------------------------------------------- device facts (cached per process)
+struct DevInfo {
+  bool ok = false;
+  int sms = 0, smem_optin = 0, mem_khz = 0, bus_bits = 0;
+  long long l2 = 0;
+  char err[256] = "";
+};
+const DevInfo &devinfo() {
+  static DevInfo di;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    cudaDeviceProp pr;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&pr, dev);
+    if (e != cudaSuccess) {
+      snprintf(di.err, sizeof di.err, "no usable CUDA device: %s", cudaGetErrorString(e));
+      (void)cudaGetLastError();
+      return;
+    }
+    di.sms = pr.multiProcessorCount;
+    di.smem_optin = (int)pr.sharedMemPerBlockOptin;
+    di.l2 = pr.l2CacheSize;
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMemoryClockRate, dev) == cudaSuccess) di.mem_khz = v;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrGlobalMemoryBusWidth, dev) == cudaSuccess) di.bus_bits = v;
+    di.ok = true;
+  });
+  return di;
+}
+
+// ---------------------------------------------------------------- kernel tables
+typedef void (*stream_kernel_t)(const su3::StreamParams);
+constexpr int NCW = 8;  // consumer warps per CTA of the pipeline kernel (tile <= 256 matrices)
+
+template <typename R, int OP> stream_kernel_t pipe_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_pipe_kernel<R, 1, OP, NCW>;
+    case 2: return su3::su3_pipe_kernel<R, 2, OP, NCW>;
+    case 4: return su3::su3_pipe_kernel<R, 4, OP, NCW>;
+    case 8: return su3::su3_pipe_kernel<R, 8, OP, NCW>;
+    case 16: return su3::su3_pipe_kernel<R, 16, OP, NCW>;
+    case 32: return su3::su3_pipe_kernel<R, 32, OP, NCW>;
+  }
+  return nullptr;
+}
+template <typename R, int OP> stream_kernel_t direct_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_direct_kernel<R, 1, OP>;
+    case 2: return su3::su3_direct_kernel<R, 2, OP>;
+    case 4: return su3::su3_direct_kernel<R, 4, OP>;
+    case 8: return su3::su3_direct_kernel<R, 8, OP>;
+    case 16: return su3::su3_direct_kernel<R, 16, OP>;
+    case 32: return su3::su3_direct_kernel<R, 32, OP>;
+  }
+  return nullptr;
+}
+template <typename R> stream_kernel_t pick(int op, int W, bool direct) {
+  switch (op) {
+    case su3::OP_MUL: return direct ? direct_for_w<R, su3::OP_MUL>(W) : pipe_for_w<R, su3::OP_MUL>(W);
+    case su3::OP_MUL3: return direct ? direct_for_w<R, su3::OP_MUL3>(W) : pipe_for_w<R, su3::OP_MUL3>(W);
+    case su3::OP_MUL_ADD: return direct ? direct_for_w<R, su3::OP_MUL_ADD>(W) : pipe_for_w<R, su3::OP_MUL_ADD>(W);
+  }
+  return nullptr;
+}
+
+su3_status cuda_fail(const char *what, cudaError_t e) {
+  return fail(SU3_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+// Launch one arithmetic expression over `nmat` matrices starting at the given pointers.
+su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const void *y, const void *u, int64_t nmat,
+                         size_t footprint_bytes, cudaStream_t stream) {
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (nmat == 0) return SU3_OK;
+  su3_tune tn;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    tn = g_tune;
+  }
+  const int nin = (op == su3::OP_MUL) ? 2 : 3;
+  const int cb = 2 * prec;
+  const bool direct = tn.path == 2;
+  stream_kernel_t k = (prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct);
+  if (!k) return fail(SU3_ERR_INVALID, "no kernel for op %d prec %d W %d", op, prec, W);
+
+  su3::StreamParams p;
+  p.z = z; p.x = x; p.y = y; p.u = u; p.nmat = nmat;
+  int hint = tn.l2_hint;
+  if (hint == 0) hint = (footprint_bytes > (size_t)di.l2) ? 1 : 1;  // auto: no hint (measured: DESIGN.md section 6)
+  p.hint = (hint == 2) ? 1 : 0;
+
+  if (direct) {
+    p.tile_mats = 0; p.stages = 0;
+    const int64_t blocks_needed = (nmat + 255) / 256;
+    const int64_t cap = (int64_t)di.sms * 8 * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 1);
+    const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
+    k<<<grid, 256, 0, stream>>>(p);
+  } else {
+    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
+    const int64_t max_grid = (int64_t)di.sms * ctas;
+    int tm = tn.tile_mats;
+    if (tm == 0) {  // auto: largest tile that still gives every persistent CTA a few tiles
+      tm = 128;
+      while (tm > 32 && (nmat + tm - 1) / tm < 4 * max_grid) tm >>= 1;
+    }
+    if (tm != 32 && tm != 64 && tm != 128 && tm != 256) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128,256}", tm);
+    const size_t stage_bytes = (size_t)nin * tm * 9 * cb;
+    // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
+    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    int stages = tn.stages;
+    if (stages == 0) {
+      stages = (int)((budget - 256) / stage_bytes);
+      if (stages > 8) stages = 8;
+    }
+    if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);
+    const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t);
+    if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "pipeline needs %zu B of shared memory, device allows %d", smem, di.smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
+    p.tile_mats = tm; p.stages = stages;
+    const int64_t ntiles = (nmat + tm - 1) / tm;
+    const unsigned grid = (unsigned)(ntiles < max_grid ? ntiles : max_grid);
+    k<<<grid, (NCW + 1) * 32, smem, stream>>>(p);
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("kernel launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
+su3_status check_arith(const su3_field *z, const su3_field *x, const su3_field *y, const su3_field *u, bool has_u) {
+  if (!z || !x || !y || (has_u && !u)) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_desc(z->d, x->d) || !same_desc(z->d, y->d) || (has_u && !same_desc(z->d, u->d)))
+    return fail(SU3_ERR_MISMATCH, "operand descriptors differ (L, n_lorentz, prec, layout, W, simd must all agree)");
+  return SU3_OK;
+}
+
+su3_status arith(int op, su3_field *z, const su3_field *x, const su3_field *y, const su3_field *u, void *stream) {
+  su3_status st = check_arith(z, x, y, u, op != su3::OP_MUL);
+  if (st != SU3_OK) return st;
+  const size_t fp = z->nbytes * (op == su3::OP_MUL ? 3 : 4);
+  return launch_stream(op, z->d.prec, z->d.W, z->ptr, x->ptr, y->ptr, u ? u->ptr : nullptr, z->nmat, fp,
+                       (cudaStream_t)stream);
+}
+
+unsigned flat_grid(size_t n_items, size_t per_block, int blocks_per_sm) {
+  const DevInfo &di = devinfo();
+  size_t need = (n_items + per_block - 1) / per_block;
+  size_t cap = (size_t)di.sms * blocks_per_sm;
+  if (need < 1) need = 1;
+  return (unsigned)(need < cap ? need : cap);
+}
+
+// ---------------------------------------------------------------- su3_mul_host resources
+struct HostPipe {
+  std::mutex mu;
+  cudaStream_t h2d = nullptr, d2h = nullptr;
+  std::vector<cudaEvent_t> ev;
+  cudaError_t ensure(size_t nev) {
+    cudaError_t e = cudaSuccess;
+    if (!h2d && (e = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if (!d2h && (e = cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    while (ev.size() < nev) {
+      cudaEvent_t v;
+      if ((e = cudaEventCreateWithFlags(&v, cudaEventDisableTiming)) != cudaSuccess) return e;
+      ev.push_back(v);
+    }
+    return e;
+  }
+};
+HostPipe g_hp;
+
+}  // namespace
+
+extern "C" {
+
+const char *su3_last_error(void) { return g_err; }
+const char *su3_version(void) { return "su3stream 0.1 (sm_100a)"; }
+
+su3_status su3_desc_normalize(const su3_desc *desc, su3_desc *out) { return normalize(desc, out); }
+
+su3_status su3_field_bytes(const su3_desc *desc, size_t *nbytes) {
+  if (!nbytes) return fail(SU3_ERR_NULL, "nbytes is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  *nbytes = (size_t)volume_of(d) * d.n_lorentz * 18 * d.prec;
+  return SU3_OK;
+}
+
+su3_status su3_field_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
+  if (!out) return fail(SU3_ERR_NULL, "out is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  if (!dev_ptr) return fail(SU3_ERR_NULL, "device pointer is NULL");
+  if ((uintptr_t)dev_ptr & 15) return fail(SU3_ERR_ALIGN, "device pointer %p is not 16-byte aligned", dev_ptr);
+  const size_t need = (size_t)volume_of(d) * d.n_lorentz * 18 * d.prec;
+  if (nbytes < need) return fail(SU3_ERR_SIZE, "buffer of %zu bytes is smaller than the %zu the field needs", nbytes, need);
+  su3_field *f = new (std::nothrow) su3_field;
+  if (!f) return fail(SU3_ERR_SIZE, "out of host memory");
+  f->d = d; f->ptr = dev_ptr; f->nbytes = need; f->volume = volume_of(d); f->nmat = f->volume * d.n_lorentz;
+  *out = f;
+  return SU3_OK;
+}
+
+su3_status su3_field_free(su3_field *f) {
+  if (!f) return fail(SU3_ERR_NULL, "field handle is NULL");
+  delete f;
+  return SU3_OK;
+}
+
+su3_status su3_field_desc(const su3_field *f, su3_desc *out) {
+  if (!f || !out) return fail(SU3_ERR_NULL, "NULL argument");
+  *out = f->d;
+  return SU3_OK;
+}
+
+su3_status su3_field_ptr(const su3_field *f, void **dev_ptr, size_t *nbytes) {
+  if (!f || !dev_ptr || !nbytes) return fail(SU3_ERR_NULL, "NULL argument");
+  *dev_ptr = f->ptr; *nbytes = f->nbytes;
+  return SU3_OK;
+}
+
+su3_status su3_index(const su3_desc *desc, int64_t site, int mu, int i, int j, int reim, int64_t *off) {
+  if (!off) return fail(SU3_ERR_NULL, "off is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  if (site < 0 || site >= volume_of(d) || mu < 0 || mu >= d.n_lorentz || i < 0 || i > 2 || j < 0 || j > 2 || reim < 0 || reim > 1)
+    return fail(SU3_ERR_INVALID, "index (site %lld, mu %d, i %d, j %d, reim %d) out of range", (long long)site, mu, i, j, reim);
+  const int e = 3 * i + j;
+  if (d.layout == SU3_SCALAR) {
+    *off = ((site * d.n_lorentz + mu) * 9 + e) * 2 + reim;
+    return SU3_OK;
+  }
+  int64_t o = 0, ostride = 1, l = 0, lstride = 1, s = site;
+  for (int k = 0; k < 4; k++) {
+    const int64_t xk = s % d.L[k];
+    s /= d.L[k];
+    const int64_t r = d.L[k] / d.simd[k];
+    o += (xk % r) * ostride; ostride *= r;
+    l += (xk / r) * lstride; lstride *= d.simd[k];
+  }
+  *off = (((o * d.n_lorentz + mu) * 9 + e) * d.W + l) * 2 + reim;
+  return SU3_OK;
+}
+
+su3_status su3_mul(su3_field *z, const su3_field *x, const su3_field *y, void *s) {
+  return arith(su3::OP_MUL, z, x, y, nullptr, s);
+}
+su3_status su3_mul3(su3_field *z, const su3_field *x, const su3_field *y, const su3_field *w, void *s) {
+  return arith(su3::OP_MUL3, z, x, y, w, s);
+}
+su3_status su3_mul_add(su3_field *z, const su3_field *x, const su3_field *y, const su3_field *v, void *s) {
+  return arith(su3::OP_MUL_ADD, z, x, y, v, s);
+}
+
+su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *stream) {
+  su3_status st = check_arith(z, x, y, nullptr, false);
+  if (st != SU3_OK) return st;
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  const size_t n16 = z->nbytes / 16;
+  const int nrem = (int)((z->nbytes % 16) / z->d.prec);
+  const unsigned grid = flat_grid(n16, 512, 8);
+  if (z->d.prec == SU3_F64)
+    su3::su3_add_kernel<double><<<grid, 256, 0, (cudaStream_t)stream>>>((double *)z->ptr, (const double *)x->ptr, (const double *)y->ptr, n16, nrem);
+  else
+    su3::su3_add_kernel<float><<<grid, 256, 0, (cudaStream_t)stream>>>((float *)z->ptr, (const float *)x->ptr, (const float *)y->ptr, n16, nrem);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_add launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
+su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
+  if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_desc(dst->d, src->d)) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  const size_t n16 = dst->nbytes / 16;
+  const int tail8 = (dst->nbytes % 16) ? 1 : 0;
+  const unsigned grid = flat_grid(n16, 1024, 8);
+  su3::su3_copy_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((uint4 *)dst->ptr, (const uint4 *)src->ptr, n16, tail8);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_copy launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
+su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
+  if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_lattice(dst->d, src->d)) return fail(SU3_ERR_MISMATCH, "su3_convert: L, n_lorentz and prec must agree");
+  if (dst->d.layout == src->d.layout)
+    return fail(SU3_ERR_MISMATCH, "su3_convert: exactly one of dst/src must be SU3_SCALAR and the other SU3_VECTOR");
+  if (dst->ptr == src->ptr) return fail(SU3_ERR_MISMATCH, "su3_convert: dst and src must not alias");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  const su3_desc &v = (dst->d.layout == SU3_VECTOR) ? dst->d : src->d;
+  su3::ConvertParams p;
+  memset(&p, 0, sizeof p);
+  p.dst = dst->ptr; p.src = src->ptr;
+  p.nl = v.n_lorentz;
+  p.nrec = dst->volume / v.W * v.n_lorentz;
+  p.to_vector = dst->d.layout == SU3_VECTOR;
+  long long stride = 1;
+  for (int k = 0; k < 4; k++) {
+    p.r[k] = v.L[k] / v.simd[k];
+    p.sstride[k] = stride;
+    stride *= v.L[k];
+  }
+  for (int l = 0; l < v.W; l++) {  // lane l = lexicographic index of ic over simd, d=0 fastest
+    long long off = 0;
+    int rem = l;
+    for (int k = 0; k < 4; k++) {
+      const int ic = rem % v.simd[k];
+      rem /= v.simd[k];
+      off += (long long)ic * p.r[k] * p.sstride[k];
+    }
+    p.lane_off[l] = off * v.n_lorentz * 9;
+  }
+  if (p.nrec == 0) return SU3_OK;
+  constexpr int TR = 64;
+  const long long blocks = (p.nrec + TR - 1) / TR;
+  if (blocks > 0x7fffffffLL) return fail(SU3_ERR_SIZE, "su3_convert: lattice too large for one launch");
+  cudaStream_t s = (cudaStream_t)stream;
+  const unsigned grid = (unsigned)blocks;
+#define SU3_CONVERT_CASE(WW)                                                                     \
+  case WW:                                                                                       \
+    if (v.prec == SU3_F64) su3::su3_convert_kernel<double2, WW, TR><<<grid, 256, 0, s>>>(p);     \
+    else su3::su3_convert_kernel<float2, WW, TR><<<grid, 256, 0, s>>>(p);                        \
+    break;
+  switch (v.W) {
+    SU3_CONVERT_CASE(1) SU3_CONVERT_CASE(2) SU3_CONVERT_CASE(4) SU3_CONVERT_CASE(8) SU3_CONVERT_CASE(16) SU3_CONVERT_CASE(32)
+    default: return fail(SU3_ERR_INVALID, "su3_convert: W = %d", v.W);
+  }
+#undef SU3_CONVERT_CASE
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
+su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su3_field *zd, su3_field *xd,
+                        su3_field *yd, int chunks, void *cuda_stream) {
+  if (!z_host || !x_host || !y_host) return fail(SU3_ERR_NULL, "host pointer is NULL");
+  su3_status st = check_arith(zd, xd, yd, nullptr, false);
+  if (st != SU3_OK) return st;
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  cudaStream_t user = (cudaStream_t)cuda_stream;
+  const int W = zd->d.W, prec = zd->d.prec;
+  const int64_t nmat = zd->nmat;
+  const size_t mat_bytes = (size_t)18 * prec;
+  // chunk boundaries: multiples of 2*W matrices keep every chunk 16-byte aligned and lane-complete
+  const int64_t gran = 2 * (int64_t)W;
+  if (chunks <= 0) chunks = 8;
+  int64_t per = (nmat + chunks - 1) / chunks;
+  per = (per + gran - 1) / gran * gran;
+  if (per < gran) per = gran;
+  const int64_t nchunks = nmat ? (nmat + per - 1) / per : 0;
+  std::lock_guard<std::mutex> lk(g_hp.mu);
+  cudaError_t e = g_hp.ensure((size_t)(2 * nchunks + 2));
+  if (e != cudaSuccess) return cuda_fail("su3_mul_host stream/event setup", e);
+  cudaEvent_t ev_start = g_hp.ev[0], ev_done = g_hp.ev[1];
+#define SU3_CK(call)                                         \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(#call, e_);      \
+  } while (0)
+  SU3_CK(cudaEventRecord(ev_start, user));
+  SU3_CK(cudaStreamWaitEvent(g_hp.h2d, ev_start, 0));
+  SU3_CK(cudaStreamWaitEvent(g_hp.d2h, ev_start, 0));
+  for (int64_t c = 0; c < nchunks; c++) {
+    const int64_t m0 = c * per;
+    const int64_t nm = (nmat - m0 < per) ? nmat - m0 : per;
+    const size_t off = (size_t)m0 * mat_bytes, len = (size_t)nm * mat_bytes;
+    cudaEvent_t ev_in = g_hp.ev[2 + 2 * c], ev_k = g_hp.ev[3 + 2 * c];
+    SU3_CK(cudaMemcpyAsync((char *)xd->ptr + off, (const char *)x_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
+    SU3_CK(cudaMemcpyAsync((char *)yd->ptr + off, (const char *)y_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
+    SU3_CK(cudaEventRecord(ev_in, g_hp.h2d));
+    SU3_CK(cudaStreamWaitEvent(user, ev_in, 0));
+    st = launch_stream(su3::OP_MUL, prec, W, (char *)zd->ptr + off, (const char *)xd->ptr + off,
+                       (const char *)yd->ptr + off, nullptr, nm, 3 * zd->nbytes, user);
+    if (st != SU3_OK) return st;
+    SU3_CK(cudaEventRecord(ev_k, user));
+    SU3_CK(cudaStreamWaitEvent(g_hp.d2h, ev_k, 0));
+    SU3_CK(cudaMemcpyAsync((char *)z_host + off, (const char *)zd->ptr + off, len, cudaMemcpyDeviceToHost, g_hp.d2h));
+  }
+  SU3_CK(cudaEventRecord(ev_done, g_hp.d2h));
+  SU3_CK(cudaStreamWaitEvent(user, ev_done, 0));
+#undef SU3_CK
+  return SU3_OK;
+}
+
+su3_status su3_tune_set(const su3_tune *t) {
+  su3_tune v = {0, 0, 0, 0, 0, {0, 0, 0}};
+  if (t) v = *t;
+  if (v.tile_mats != 0 && v.tile_mats != 32 && v.tile_mats != 64 && v.tile_mats != 128 && v.tile_mats != 256)
+    return fail(SU3_ERR_INVALID, "tile_mats = %d not in {0,32,64,128,256}", v.tile_mats);
+  if (v.stages != 0 && (v.stages < 2 || v.stages > 16)) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16", v.stages);
+  if (v.ctas_per_sm < 0 || v.ctas_per_sm > 8) return fail(SU3_ERR_INVALID, "ctas_per_sm = %d outside 0..8", v.ctas_per_sm);
+  if (v.l2_hint < 0 || v.l2_hint > 2) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..2", v.l2_hint);
+  if (v.path < 0 || v.path > 2) return fail(SU3_ERR_INVALID, "path = %d outside 0..2", v.path);
+  std::lock_guard<std::mutex> lk(g_tune_mu);
+  g_tune = v;
+  return SU3_OK;
+}
+
+su3_status su3_tune_get(su3_tune *out) {
+  if (!out) return fail(SU3_ERR_NULL, "out is NULL");
+  std::lock_guard<std::mutex> lk(g_tune_mu);
+  *out = g_tune;
+  return SU3_OK;
+}
+
+int64_t su3_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+su3_status su3_device_info(int32_t *sm_count, int64_t *l2_bytes, int32_t *mem_clock_khz, int32_t *bus_width_bits) {
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (sm_count) *sm_count = di.sms;
+  if (l2_bytes) *l2_bytes = di.l2;
+  if (mem_clock_khz) *mem_clock_khz = di.mem_khz;
+  if (bus_width_bits) *bus_width_bits = di.bus_bits;
+  return SU3_OK;
+}
+
+}  // extern "C"

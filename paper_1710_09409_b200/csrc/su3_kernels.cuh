@@ -1,0 +1,471 @@
+// su3_kernels.cuh -- sm_100a device code of libsu3stream.
+//
+// Hot path of arXiv:1710.09409 section 4/5 (Listing 3):
+// the lattice-wide, site-wise complex 3x3 product z = x*y and the fused one-pass
+// expressions z = x*y*w, z = x*y + v, in the scalar (AoS) and the
+// lane-interleaved vector layout, plus the layout permutation (extract/merge) and the
+// streaming ceilings.  No code is shared with oracle/ (the CPU checker).
+//
+// Design: every field is a flat byte stream of records.  A record
+// of the vector layout with W lanes is 9 element-vectors of W complex numbers; the
+// scalar layout is the W = 1 case.  The arithmetic kernels are HBM-bound (0.46-1.4
+// flop/byte), so the kernel is a persistent, warp-specialised streaming pipeline:
+//
+//   producer warp (1 elected lane)          consumer warps (1 thread = 1 matrix)
+//   -------------------------------         ------------------------------------
+//   wait  empty[s]                          wait  full[s]
+//   cp.async.bulk  x,y(,u) tile -> smem     LDS   own matrix of x, y(, u)   (conflict-free)
+//   (TMA 1-D bulk copy, mbarrier tx)        FMA   27 (54) complex multiply-adds in registers
+//                                           STS   z into the x slot, fence.proxy.async
+//                                           bar   consumers only
+//                                           cp.async.bulk  smem -> z tile   (1 thread)
+//                                           arrive empty[s-1] once its store has read smem
+//
+// A tile is a CONTIGUOUS byte range of every operand (T matrices = T*144 B fp64 / T*72 B
+// fp32), so the 144/72-byte AoS records reach HBM as full-line bulk transactions whatever
+// the layout; the layout only changes the shared-memory index of a thread's matrix.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace su3 {
+
+enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2 };
+
+// ---------------------------------------------------------------- complex helpers
+template <typename R> struct Cplx;
+template <> struct Cplx<float> { typedef float2 type; };
+template <> struct Cplx<double> { typedef double2 type; };
+
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+
+// c = a.b, c_ij = sum_k a_ik b_kj (S7), k ascending, as a fixed chain of
+// round-to-nearest FMAs.  Written with intrinsics so that every kernel that inlines it
+// (scalar or vector layout, staged or direct path) produces bit-identical results.
+template <typename C2>
+__device__ __forceinline__ void mat33_mul(const C2 (&a)[9], const C2 (&b)[9], C2 (&c)[9]) {
+#pragma unroll
+  for (int i = 0; i < 3; i++) {
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      auto re = mul_rn(a[3 * i].x, b[j].x);
+      auto im = mul_rn(a[3 * i].x, b[j].y);
+      re = fma_rn(-a[3 * i].y, b[j].y, re);
+      im = fma_rn(a[3 * i].y, b[j].x, im);
+#pragma unroll
+      for (int k = 1; k < 3; k++) {
+        re = fma_rn(a[3 * i + k].x, b[3 * k + j].x, re);
+        im = fma_rn(a[3 * i + k].x, b[3 * k + j].y, im);
+        re = fma_rn(-a[3 * i + k].y, b[3 * k + j].y, re);
+        im = fma_rn(a[3 * i + k].y, b[3 * k + j].x, im);
+      }
+      c[3 * i + j].x = re;
+      c[3 * i + j].y = im;
+    }
+  }
+}
+
+// ---------------------------------------------------------------- PTX wrappers (sm_90+/sm_100a)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+// TMA 1-D bulk copy global -> shared, completion on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar,
+                                              uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+      : "memory");
+}
+// TMA 1-D bulk copy shared -> global, bulk async-group completion.
+__device__ __forceinline__ void bulk_s2g(void *dst_gmem, const void *src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_hint(void *dst_gmem, const void *src_smem, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst_gmem),
+               "r"(smem_u32(src_smem)), "r"(bytes), "l"(pol)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N> __device__ __forceinline__ void bulk_wait_all() {
+  asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// ---------------------------------------------------------------- the streaming pipeline (A1-A4)
+struct StreamParams {
+  void *z;
+  const void *x;
+  const void *y;
+  const void *u;   // third operand: w (OP_MUL3) or v (OP_MUL_ADD); unused for OP_MUL
+  long long nmat;  // matrices in the range handled by this launch (multiple of W)
+  int tile_mats;   // matrices per tile: multiple of 32 (hence of W), <= NCW*32
+  int stages;      // ring depth >= 2
+  int hint;        // 1: L2 evict_first on loads and stores
+};
+
+template <int OP> struct NumInputs { static const int value = (OP == OP_MUL) ? 2 : 3; };
+
+// One thread's matrix: element e of lane l of record q sits at complex index (q*9 + e)*W + l
+// of the slot.  Thread t owns (q = t / W, l = t % W).  Bank check: with
+// 16-byte (fp64) or 8-byte (fp32) complex numbers every quarter-/half-warp request covers
+// all 32 banks exactly once for every W in {1,2,4,8,16,32}.
+template <typename R, int W, int OP, int NCW>
+__global__ void __launch_bounds__((NCW + 1) * 32) su3_pipe_kernel(const StreamParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int NIN = NumInputs<OP>::value;
+  constexpr int CB = (int)sizeof(C2);
+  extern __shared__ __align__(128) unsigned char smem[];
+
+  const int TM = p.tile_mats;
+  const int S = p.stages;
+  const uint32_t slot_bytes = (uint32_t)TM * 9u * CB;
+  const uint32_t stage_bytes = NIN * slot_bytes;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)S * stage_bytes);
+  uint64_t *empty = full + S;
+
+  const int tid = threadIdx.x;
+  const long long ntiles = (p.nmat + TM - 1) / TM;
+
+  if (tid == 0) {
+    for (int s = 0; s < S; s++) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], 1);
+    }
+    fence_mbar_init();
+    fence_proxy_async();
+  }
+  __syncthreads();
+
+  if (tid >= NCW * 32) {
+    // ------------------------------------------------ producer: one elected lane issues the TMA bulk loads
+    if (tid == NCW * 32) {
+      const unsigned char *src[3] = {(const unsigned char *)p.x, (const unsigned char *)p.y,
+                                     (const unsigned char *)p.u};
+      uint64_t pol = 0;
+      if (p.hint) pol = policy_evict_first();
+      int s = 0;
+      uint32_t ph = 0;
+      for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(&empty[s], ph ^ 1u);
+        const long long m0 = tile * TM;
+        const long long left = p.nmat - m0;
+        const int nm = left < TM ? (int)left : TM;
+        const uint32_t bytes = (uint32_t)nm * 9u * CB;
+        const uint32_t b16 = bytes & ~15u;  // bulk copies move multiples of 16 bytes
+        unsigned char *st = smem + (size_t)s * stage_bytes;
+        const size_t goff = (size_t)m0 * 9u * CB;
+        if (bytes != b16) {  // fp32 with an odd matrix count: 8 trailing bytes per operand
+#pragma unroll
+          for (int o = 0; o < NIN; o++)
+            *reinterpret_cast<uint64_t *>(st + o * slot_bytes + b16) =
+                *reinterpret_cast<const uint64_t *>(src[o] + goff + b16);
+        }
+        mbar_arrive_expect_tx(&full[s], NIN * b16);
+#pragma unroll
+        for (int o = 0; o < NIN; o++) {
+          if (p.hint)
+            bulk_g2s_hint(st + o * slot_bytes, src[o] + goff, b16, &full[s], pol);
+          else
+            bulk_g2s(st + o * slot_bytes, src[o] + goff, b16, &full[s]);
+        }
+        if (++s == S) {
+          s = 0;
+          ph ^= 1u;
+        }
+      }
+    }
+    return;
+  }
+
+  // -------------------------------------------------- consumers: one thread per matrix of the tile
+  const int t = tid;
+  const int base = (t / W) * 9 * W + (t % W);
+  uint64_t pol = 0;
+  if (p.hint && t == 0) pol = policy_evict_first();
+  int s = 0, prev_s = -1;
+  uint32_t ph = 0;
+  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const long long m0 = tile * TM;
+    const long long left = p.nmat - m0;
+    const int nm = left < TM ? (int)left : TM;
+    unsigned char *st = smem + (size_t)s * stage_bytes;
+    mbar_wait(&full[s], ph);
+    if (t < nm) {
+      C2 *sx = reinterpret_cast<C2 *>(st) + base;
+      const C2 *sy = reinterpret_cast<const C2 *>(st + slot_bytes) + base;
+      C2 a[9], b[9], c[9];
+#pragma unroll
+      for (int e = 0; e < 9; e++) a[e] = sx[e * W];
+#pragma unroll
+      for (int e = 0; e < 9; e++) b[e] = sy[e * W];
+      mat33_mul(a, b, c);
+      if (OP == OP_MUL3) {
+        const C2 *su = reinterpret_cast<const C2 *>(st + 2 * slot_bytes) + base;
+#pragma unroll
+        for (int e = 0; e < 9; e++) b[e] = su[e * W];
+        mat33_mul(c, b, a);
+#pragma unroll
+        for (int e = 0; e < 9; e++) c[e] = a[e];
+      } else if (OP == OP_MUL_ADD) {
+        const C2 *su = reinterpret_cast<const C2 *>(st + 2 * slot_bytes) + base;
+#pragma unroll
+        for (int e = 0; e < 9; e++) {
+          C2 v = su[e * W];
+          c[e].x = add_rn(c[e].x, v.x);
+          c[e].y = add_rn(c[e].y, v.y);
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < 9; e++) sx[e * W] = c[e];
+    }
+    fence_proxy_async();  // generic-proxy smem writes -> visible to the bulk (async-proxy) store
+    named_bar_sync(1, NCW * 32);
+    if (t == 0) {
+      const uint32_t bytes = (uint32_t)nm * 9u * CB;
+      const uint32_t b16 = bytes & ~15u;
+      unsigned char *zdst = (unsigned char *)p.z + (size_t)m0 * 9u * CB;
+      if (p.hint)
+        bulk_s2g_hint(zdst, st, b16, pol);
+      else
+        bulk_s2g(zdst, st, b16);
+      bulk_commit();
+      if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(st + b16);
+      // the previous tile's store has finished READING its stage: hand that stage back
+      bulk_wait_read<1>();
+      if (prev_s >= 0) mbar_arrive(&empty[prev_s]);
+    }
+    prev_s = s;
+    if (++s == S) {
+      s = 0;
+      ph ^= 1u;
+    }
+  }
+  if (t == 0) bulk_wait_all<0>();  // smem must outlive the last store; writes complete before exit
+}
+
+// ---------------------------------------------------------------- direct path (path = 2)
+// One thread per matrix, operands read straight from global memory with one complex number
+// per load.  For W*sizeof(complex) >= 32 bytes every warp request is made of whole sectors
+// (vector layout: each group of W threads reads one W*c-byte element vector).  For W = 1
+// this is the paper's naive AoS kernel ("lack of memory coalescence"),
+// kept as the measured counter-example.
+template <typename R, int W, int OP>
+__global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
+  typedef typename Cplx<R>::type C2;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < p.nmat; t += stride) {
+    const long long base = (t / W) * 9 * W + (t % W);
+    const C2 *gx = reinterpret_cast<const C2 *>(p.x) + base;
+    const C2 *gy = reinterpret_cast<const C2 *>(p.y) + base;
+    C2 *gz = reinterpret_cast<C2 *>(p.z) + base;
+    C2 a[9], b[9], c[9];
+#pragma unroll
+    for (int e = 0; e < 9; e++) a[e] = gx[e * W];
+#pragma unroll
+    for (int e = 0; e < 9; e++) b[e] = gy[e * W];
+    if (OP == OP_MUL) {
+      mat33_mul(a, b, c);
+    } else if (OP == OP_MUL3) {
+      const C2 *gu = reinterpret_cast<const C2 *>(p.u) + base;
+      C2 w[9];
+#pragma unroll
+      for (int e = 0; e < 9; e++) w[e] = gu[e * W];
+      mat33_mul(a, b, c);
+      mat33_mul(c, w, a);
+#pragma unroll
+      for (int e = 0; e < 9; e++) c[e] = a[e];
+    } else {
+      const C2 *gu = reinterpret_cast<const C2 *>(p.u) + base;
+      C2 w[9];
+#pragma unroll
+      for (int e = 0; e < 9; e++) w[e] = gu[e * W];
+      mat33_mul(a, b, c);
+#pragma unroll
+      for (int e = 0; e < 9; e++) {
+        c[e].x = add_rn(c[e].x, w[e].x);
+        c[e].y = add_rn(c[e].y, w[e].y);
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < 9; e++) gz[e * W] = c[e];
+  }
+}
+
+// ---------------------------------------------------------------- streaming ceilings (A6) and z = x + y
+// dst = src over n16 16-byte words (+ an optional 8-byte tail), 4 independent 128-bit loads
+// in flight per thread.
+__global__ void __launch_bounds__(256) su3_copy_kernel(uint4 *__restrict__ dst, const uint4 *__restrict__ src,
+                                                       size_t n16, int tail8) {
+  const size_t bd = blockDim.x;
+  const size_t stride = (size_t)gridDim.x * bd * 4;
+  size_t i = (size_t)blockIdx.x * bd * 4 + threadIdx.x;
+  for (; i + 3 * bd < n16; i += stride) {
+    uint4 v0 = src[i], v1 = src[i + bd], v2 = src[i + 2 * bd], v3 = src[i + 3 * bd];
+    dst[i] = v0;
+    dst[i + bd] = v1;
+    dst[i + 2 * bd] = v2;
+    dst[i + 3 * bd] = v3;
+  }
+  for (; i < n16; i += bd) dst[i] = src[i];
+  if (tail8 && blockIdx.x == 0 && threadIdx.x == 0)
+    reinterpret_cast<uint2 *>(dst + n16)[0] = reinterpret_cast<const uint2 *>(src + n16)[0];
+}
+
+template <typename R> struct Vec16;
+template <> struct Vec16<float> {
+  typedef float4 type;
+  static __device__ __forceinline__ float4 add(float4 a, float4 b) {
+    return make_float4(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y), __fadd_rn(a.z, b.z), __fadd_rn(a.w, b.w));
+  }
+};
+template <> struct Vec16<double> {
+  typedef double2 type;
+  static __device__ __forceinline__ double2 add(double2 a, double2 b) {
+    return make_double2(__dadd_rn(a.x, b.x), __dadd_rn(a.y, b.y));
+  }
+};
+
+// z = x + y over n16 16-byte words (+ nrem trailing reals); layout-agnostic (element-wise).
+template <typename R>
+__global__ void __launch_bounds__(256) su3_add_kernel(R *z, const R *x, const R *y, size_t n16, int nrem) {
+  typedef typename Vec16<R>::type V;
+  V *z16 = reinterpret_cast<V *>(z);
+  const V *x16 = reinterpret_cast<const V *>(x);
+  const V *y16 = reinterpret_cast<const V *>(y);
+  const size_t bd = blockDim.x;
+  const size_t stride = (size_t)gridDim.x * bd * 2;
+  size_t i = (size_t)blockIdx.x * bd * 2 + threadIdx.x;
+  for (; i + bd < n16; i += stride) {
+    V a0 = x16[i], a1 = x16[i + bd], b0 = y16[i], b1 = y16[i + bd];
+    z16[i] = Vec16<R>::add(a0, b0);
+    z16[i + bd] = Vec16<R>::add(a1, b1);
+  }
+  for (; i < n16; i += bd) z16[i] = Vec16<R>::add(x16[i], y16[i]);
+  if (blockIdx.x == 0 && (int)threadIdx.x < nrem) {
+    const size_t k = n16 * (16 / sizeof(R)) + threadIdx.x;
+    z[k] = add_rn(x[k], y[k]);
+  }
+}
+
+// ---------------------------------------------------------------- layout conversion (A5)
+// vec[o][mu][e][l] = sca[site(o,l)][mu][e]  (extract/merge; virtual-node map S3).
+// A block handles TR consecutive vector records (rec = o*nl + mu): the vector side is one
+// contiguous, fully coalesced range; the scalar side is W streams of contiguous records.
+struct ConvertParams {
+  void *dst;
+  const void *src;
+  long long nrec;       // vector records = (volume / W) * nl
+  int nl;
+  int r[4];             // sub-lattice extents L[d] / simd[d]
+  long long sstride[4]; // scalar-site stride of dimension d: 1, L0, L0*L1, L0*L1*L2
+  long long lane_off[32]; // (site offset of lane l) * nl * 9, in complex numbers
+  int to_vector;        // 1: dst is the vector layout; 0: dst is the scalar layout
+};
+
+template <typename C2, int W, int TR>
+__global__ void __launch_bounds__(256) su3_convert_kernel(const ConvertParams p) {
+  __shared__ long long sbase[TR];  // scalar-side complex index of (rec, lane 0, e = 0)
+  const long long rec0 = (long long)blockIdx.x * TR;
+  const long long left = p.nrec - rec0;
+  const int nr = left < TR ? (int)left : TR;
+  if ((int)threadIdx.x < nr) {
+    const long long rec = rec0 + threadIdx.x;
+    long long o = rec / p.nl;
+    const int mu = (int)(rec - o * p.nl);
+    long long site = 0;
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+      const long long q = o / p.r[d];
+      site += (o - q * p.r[d]) * p.sstride[d];
+      o = q;
+    }
+    sbase[threadIdx.x] = (site * p.nl + mu) * 9;
+  }
+  __syncthreads();
+  const C2 *src = reinterpret_cast<const C2 *>(p.src);
+  C2 *dst = reinterpret_cast<C2 *>(p.dst);
+  const long long vbase = rec0 * 9 * W;
+  const int n = nr * 9 * W;
+  constexpr int U = 4;
+  for (int i0 = threadIdx.x; i0 < n; i0 += 256 * U) {
+    long long vi[U], si[U];
+    C2 val[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+      const int idx = i0 + u * 256;
+      const int l = idx % W;
+      const int q = idx / W;  // = rl*9 + e
+      const int rl = q / 9;
+      const int e = q - rl * 9;
+      vi[u] = vbase + idx;
+      si[u] = (idx < n) ? sbase[rl] + p.lane_off[l] + e : 0;
+    }
+#pragma unroll
+    for (int u = 0; u < U; u++)
+      if (i0 + u * 256 < n) val[u] = p.to_vector ? src[si[u]] : src[vi[u]];
+#pragma unroll
+    for (int u = 0; u < U; u++)
+      if (i0 + u * 256 < n) {
+        if (p.to_vector)
+          dst[vi[u]] = val[u];
+        else
+          dst[si[u]] = val[u];
+      }
+  }
+}
+
+}  // namespace su3

@@ -1,0 +1,128 @@
+"""The C-ABI boundary without a GPU: the library loads, exports every symbol that
+include/su3stream.h declares, validates descriptors as the header states, and its host-side
+index map reproduces the hand-computed spot values of tests/golden (reading S3/S4).
+No compute call is made here (-m "not gpu")."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1710_09409_b200 as su3
+from helpers import load_vector_map_spots
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_exports_match_header():
+    text = open(os.path.join(ROOT, "include", "su3stream.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = set(re.findall(r"\b(su3_[a-z0-9_]+)\s*\(", text))
+    assert declared == set(su3.EXPORTS)
+    for name in declared:
+        assert hasattr(su3.lib, name), name
+    assert su3.su3_version().startswith("su3stream")
+
+
+def test_field_bytes_for_the_configs():
+    assert su3.su3_field_bytes(su3.make_desc(8)) == 4096 * 144
+    assert su3.su3_field_bytes(su3.make_desc(16, layout=su3.SU3_VECTOR, W=4)) == 65536 * 144
+    assert su3.su3_field_bytes(su3.make_desc(32, n_lorentz=4)) == 4 * 32 ** 4 * 144
+    assert su3.su3_field_bytes(su3.make_desc(48, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=8)) == 48 ** 4 * 72
+    assert su3.su3_field_bytes(su3.make_desc(64)) == 64 ** 4 * 144  # > 2^31: 64-bit sizes
+
+
+@pytest.mark.parametrize("kw", [
+    dict(L=(8, 8, 0, 8)), dict(L=8, n_lorentz=2), dict(L=8, prec=2), dict(L=8, layout=3),
+    dict(L=8, layout=1, W=3), dict(L=8, layout=1, W=64), dict(L=8, layout=0, W=4),
+    dict(L=8, layout=1, W=4, simd=(1, 1, 1, 2)), dict(L=(8, 8, 8, 9), layout=1, W=2),
+    dict(L=8, layout=1, W=4, simd=(1, 1, -2, -2)),
+])
+def test_invalid_descriptors(kw):
+    with pytest.raises(su3.Su3Error) as ei:
+        su3.su3_field_bytes(su3.make_desc(**kw))
+    assert ei.value.status == su3.SU3_ERR_INVALID
+    assert su3.su3_last_error()
+
+
+def test_default_split_and_normalize():
+    _, splits = load_vector_map_spots()
+    for W, simd in splits.items():
+        d = su3.su3_desc_normalize(su3.make_desc(8, layout=su3.SU3_VECTOR if W > 1 else su3.SU3_SCALAR, W=W))
+        assert tuple(d.simd) == simd
+    d = su3.su3_desc_normalize(su3.make_desc(8, layout=su3.SU3_VECTOR, W=4, simd=(2, 2, 1, 1)))
+    assert tuple(d.simd) == (2, 2, 1, 1)
+
+
+def test_index_spot_values():
+    spots, _ = load_vector_map_spots()
+    for s in spots:
+        d = su3.make_desc(s["L"], layout=su3.SU3_VECTOR, W=s["W"])
+        for (i, j, c) in [(0, 0, 0), (1, 2, 1), (2, 2, 1)]:
+            want = (((s["outer"]) * 9 + 3 * i + j) * s["W"] + s["lane"]) * 2 + c
+            assert su3.su3_index(d, s["site"], 0, i, j, c) == want
+    d = su3.make_desc(4, n_lorentz=4)
+    assert su3.su3_index(d, 7, 3, 2, 1, 1) == ((7 * 4 + 3) * 9 + 7) * 2 + 1
+    with pytest.raises(su3.Su3Error):
+        su3.su3_index(d, 256, 0, 0, 0, 0)
+    with pytest.raises(su3.Su3Error):
+        su3.su3_index(d, 0, 4, 0, 0, 0)
+
+
+def test_index_is_a_bijection_small():
+    for kw in [dict(L=4, layout=1, W=8), dict(L=(4, 2, 6, 4), n_lorentz=4, layout=1, W=4), dict(L=2, n_lorentz=4)]:
+        d = su3.su3_desc_normalize(su3.make_desc(**kw))
+        V = d.L[0] * d.L[1] * d.L[2] * d.L[3]
+        seen = set()
+        for site in range(V):
+            for mu in range(d.n_lorentz):
+                for e in (0, 4, 8):
+                    seen.add(su3.su3_index(d, site, mu, e // 3, e % 3, 0))
+        assert len(seen) == V * d.n_lorentz * 3
+        assert max(seen) < V * d.n_lorentz * 18
+
+
+def test_wrap_errors_without_touching_memory():
+    d = su3.make_desc(2)
+    h = ctypes.c_void_p()
+    need = su3.su3_field_bytes(d)
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0), need, ctypes.byref(h)) == su3.SU3_ERR_NULL
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1008), need, ctypes.byref(h)) == su3.SU3_ERR_ALIGN
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), need - 1, ctypes.byref(h)) == su3.SU3_ERR_SIZE
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), need, None) == su3.SU3_ERR_NULL
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), need, ctypes.byref(h)) == su3.SU3_OK
+    out = su3.su3_desc()
+    assert su3.lib.su3_field_desc(h, ctypes.byref(out)) == su3.SU3_OK and tuple(out.simd) == (1, 1, 1, 1)
+    # mismatching operands are rejected before anything is launched (fake pointers are never touched)
+    d2 = su3.make_desc(2, prec=su3.SU3_F32)
+    h2 = ctypes.c_void_p()
+    assert su3.lib.su3_field_wrap(ctypes.byref(d2), ctypes.c_void_p(0x2000), need, ctypes.byref(h2)) == su3.SU3_OK
+    assert su3.lib.su3_mul(h, h, h2, None) == su3.SU3_ERR_MISMATCH
+    assert su3.lib.su3_mul(h, None, h, None) == su3.SU3_ERR_NULL
+    assert su3.lib.su3_convert(h, h, None) == su3.SU3_ERR_MISMATCH
+    assert su3.lib.su3_copy(h, h2, None) == su3.SU3_ERR_MISMATCH
+    assert su3.lib.su3_field_free(h) == su3.SU3_OK and su3.lib.su3_field_free(h2) == su3.SU3_OK
+    assert su3.lib.su3_field_free(None) == su3.SU3_ERR_NULL
+
+
+def test_tune_validation_roundtrip():
+    su3.su3_tune_set(tile_mats=64, stages=3, ctas_per_sm=2, l2_hint=1, path=1)
+    assert su3.su3_tune_get() == dict(tile_mats=64, stages=3, ctas_per_sm=2, l2_hint=1, path=1)
+    with pytest.raises(su3.Su3Error):
+        su3.su3_tune_set(tile_mats=100)
+    with pytest.raises(su3.Su3Error):
+        su3.su3_tune_set(stages=1)
+    su3.su3_tune_set()
+    assert su3.su3_tune_get()["tile_mats"] == 0
+
+
+def test_no_cpu_fallback_without_a_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    d = su3.make_desc(2)
+    h = ctypes.c_void_p()
+    su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), su3.su3_field_bytes(d), ctypes.byref(h))
+    assert su3.lib.su3_mul(h, h, h, None) == su3.SU3_ERR_CUDA  # fails loudly, computes nothing
+    assert "CUDA" in su3.su3_last_error()
+    su3.lib.su3_field_free(h)

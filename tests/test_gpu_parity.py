@@ -1,0 +1,222 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances are north_star's: per-matrix max-norm relative error
+(reading S15) <= 1e-12 in fp64 and <= 2e-5 in fp32; integer cases, convert and copy are
+bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1710_09409_b200 as su3
+import su3gen
+from gpu_util import const_field, download, geom_of, host_field, scalar_desc, upload
+from helpers import TOL, load_integer_case, rel_err
+
+pytestmark = pytest.mark.gpu
+IC = load_integer_case()
+F64, F32, SC, VE = su3.SU3_F64, su3.SU3_F32, su3.SU3_SCALAR, su3.SU3_VECTOR
+
+
+@pytest.fixture(autouse=True)
+def _default_tuning():
+    su3.su3_tune_set()
+    yield
+    su3.su3_tune_set()
+
+
+def run_op(op, desc, hosts):
+    fs = [upload(desc, h) for h in hosts]
+    z = su3.alloc_field(desc)
+    z.tensor.fill_(0xFF)
+    {"mul": su3.su3_mul, "mul3": su3.su3_mul3, "mul_add": su3.su3_mul_add, "add": su3.su3_add}[op](z, *fs)
+    return download(z)
+
+
+def oracle_op(op, desc, hosts):
+    g = geom_of(desc)
+    return {"mul": oracle.mul, "mul3": oracle.mul3, "mul_add": oracle.mul_add}[op](g, *hosts)
+
+
+def check(op, desc, hosts, tol=None):
+    z = run_op(op, desc, hosts)
+    zref = oracle_op(op, desc, hosts)
+    W = su3.su3_desc_normalize(desc).W
+    err, _ = rel_err(z, zref, W)
+    assert np.isfinite(z).all()
+    assert err <= (TOL[desc.prec] if tol is None else tol), (op, err)
+    return z, zref
+
+
+ALL_W = [(SC, 1), (VE, 1), (VE, 2), (VE, 4), (VE, 8), (VE, 16), (VE, 32)]
+
+
+# ------------------------------------------------------------------ exact integer case (bit-equal)
+@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("layout,W", ALL_W)
+def test_integer_case_bit_exact(prec, layout, W, path):
+    su3.su3_tune_set(path=path)
+    desc = su3.make_desc((4, 4, 4, 8), prec=prec, layout=layout, W=W)
+    k = np.arange(1, 8).reshape(-1, 1, 1)  # site-dependent integer multiples: tests indexing too
+    A, B, C = const_field(desc, IC["A"] * k), const_field(desc, IC["B"]), const_field(desc, IC["C"])
+    for op, hosts in [("mul", [A, B]), ("mul", [B, A]), ("mul3", [A, B, C]), ("mul_add", [A, B, C])]:
+        z = run_op(op, desc, hosts)
+        assert np.array_equal(z.astype(np.float64), oracle_op(op, desc, hosts)), (op, prec, W)
+    # and against the stored hand-computed product directly (site 0 holds 1*A)
+    z = run_op("mul", scalar_desc(desc), [const_field(scalar_desc(desc), IC["A"]), const_field(scalar_desc(desc), IC["B"])])
+    assert np.array_equal(z[:18].astype(np.float64).view(np.complex128).reshape(3, 3), IC["AB"])
+
+
+def test_identity_and_zero():
+    desc = su3.make_desc(4)
+    x = host_field(desc, 7, su3gen.FIELD_X)
+    one, zero = const_field(desc, np.eye(3)), const_field(desc, np.zeros((3, 3)))
+    v = host_field(desc, 7, su3gen.FIELD_V, kind="gauss")
+    assert np.array_equal(run_op("mul", desc, [x, one]), x)
+    assert np.array_equal(run_op("mul", desc, [one, x]), x)
+    assert not run_op("mul", desc, [x, zero]).any()
+    assert np.array_equal(run_op("mul_add", desc, [zero, x, v]), v)
+    assert np.array_equal(run_op("mul3", desc, [one, x, one]), x)
+
+
+# ------------------------------------------------------------------ BASELINE.json configs 1 and 2
+def test_config1_8x4_fp64_scalar():
+    desc = su3.make_desc(8)
+    seed = su3gen.config_seed(1)
+    x, y = host_field(desc, seed, su3gen.FIELD_X), host_field(desc, seed, su3gen.FIELD_Y)
+    z, _ = check("mul", desc, [x, y])
+    # closure of SU(3): the GPU product is unitary with det 1
+    zz = z.view(np.complex128).reshape(-1, 3, 3)
+    assert np.abs(zz @ zz.conj().transpose(0, 2, 1) - np.eye(3)).max() <= 1e-13
+    assert np.abs(np.linalg.det(zz) - 1).max() <= 1e-13
+
+
+def test_config2_16x4_both_layouts_and_roundtrip():
+    ds, dv = su3.make_desc(16), su3.make_desc(16, layout=VE, W=4)
+    seed = su3gen.config_seed(2)
+    xs, ys = host_field(ds, seed, su3gen.FIELD_X), host_field(ds, seed, su3gen.FIELD_Y)
+    xv, yv = host_field(dv, seed, su3gen.FIELD_X), host_field(dv, seed, su3gen.FIELD_Y)
+    zs, _ = check("mul", ds, [xs, ys])
+    zv, _ = check("mul", dv, [xv, yv])
+    # scalar and vector kernels share the FMA chain: bit-equal after the layout permutation
+    assert np.array_equal(oracle.convert(geom_of(dv), geom_of(ds), zs), zv)
+    # GPU convert == oracle permutation, both ways, and the round trip is the identity (bit-exact)
+    fs, fv, fs2 = upload(ds, xs), su3.alloc_field(dv), su3.alloc_field(ds)
+    su3.su3_convert(fv, fs)
+    su3.su3_convert(fs2, fv)
+    assert np.array_equal(download(fv), xv)
+    assert np.array_equal(download(fs2), xs)
+
+
+# ------------------------------------------------------------------ every W, ragged sizes, Lorentz index
+@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("layout,W", ALL_W)
+def test_all_ops_every_W(prec, layout, W, path):
+    su3.su3_tune_set(path=path)
+    desc = su3.make_desc((4, 6, 4, 8), prec=prec, layout=layout, W=W)  # 768 sites: 6 tiles of 128
+    x, y, w = (host_field(desc, 11, f) for f in (su3gen.FIELD_X, su3gen.FIELD_Y, su3gen.FIELD_W))
+    v = host_field(desc, 11, su3gen.FIELD_V, kind="gauss")
+    check("mul", desc, [x, y])
+    check("mul3", desc, [x, y, w])
+    check("mul_add", desc, [x, y, v])
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", [
+    ((3, 3, 3, 3), 1, SC, 1),    # 81 matrices: odd count -> fp32 field ends on an 8-byte tail
+    ((1, 1, 1, 1), 1, SC, 1),    # a single matrix
+    ((5, 3, 1, 7), 1, SC, 1),    # 105: one ragged tile
+    ((3, 5, 2, 6), 4, VE, 4),    # simd {1,1,2,2}; 720 matrices
+    ((6, 2, 10, 2), 4, VE, 8),   # r = {6,1,5,1}
+    ((10, 6, 6, 2), 1, VE, 2),
+    ((2, 2, 2, 2), 4, VE, 16),
+    ((12, 12, 12, 12), 1, VE, 8),  # L = 12 of the volume sweep, r = {12,6,6,6}
+])
+def test_ragged_and_lorentz(prec, L, nl, layout, W):
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    x, y, w = (host_field(desc, 13, f) for f in (su3gen.FIELD_X, su3gen.FIELD_Y, su3gen.FIELD_W))
+    for tile in (0, 32, 256):
+        su3.su3_tune_set(tile_mats=tile)
+        check("mul", desc, [x, y])
+    su3.su3_tune_set()
+    check("mul3", desc, [x, y, w])
+    # convert against the oracle permutation, both directions
+    ds = scalar_desc(desc)
+    if layout == VE:
+        xs = host_field(ds, 13, su3gen.FIELD_X)
+        fs, fv, fs2 = upload(ds, xs), su3.alloc_field(desc), su3.alloc_field(ds)
+        su3.su3_convert(fv, fs)
+        su3.su3_convert(fs2, fv)
+        assert np.array_equal(download(fv), x)
+        assert np.array_equal(download(fs2), xs)
+    # copy is bit-exact, add matches numpy exactly (one rounding per element)
+    fx, fc = upload(desc, x), su3.alloc_field(desc)
+    fc.tensor.fill_(0)
+    su3.su3_copy(fc, fx)
+    assert np.array_equal(download(fc), x)
+    assert np.array_equal(run_op("add", desc, [x, y]), x + y)
+
+
+def test_custom_simd_split():
+    desc = su3.make_desc((8, 4, 4, 4), layout=VE, W=8, simd=(4, 2, 1, 1), prec=F32)
+    x, y = host_field(desc, 17, su3gen.FIELD_X), host_field(desc, 17, su3gen.FIELD_Y)
+    check("mul", desc, [x, y])
+    ds = scalar_desc(desc)
+    fs, fv = upload(ds, host_field(ds, 17, su3gen.FIELD_X)), su3.alloc_field(desc)
+    su3.su3_convert(fv, fs)
+    assert np.array_equal(download(fv), x)
+
+
+# ------------------------------------------------------------------ launch configurations, aliasing
+@pytest.mark.parametrize("tile,stages,ctas,hint", [(32, 2, 1, 1), (64, 3, 2, 2), (128, 2, 4, 1), (128, 6, 1, 2),
+                                                   (256, 3, 1, 1), (256, 2, 2, 2), (128, 16, 1, 1)])
+def test_launch_configurations_are_equivalent(tile, stages, ctas, hint):
+    desc = su3.make_desc((16, 16, 8, 9), prec=F32)  # 18432 matrices; many tiles per CTA at ctas=1
+    x, y = host_field(desc, 19, su3gen.FIELD_X), host_field(desc, 19, su3gen.FIELD_Y)
+    ref = run_op("mul", desc, [x, y])
+    su3.su3_tune_set(tile_mats=tile, stages=stages, ctas_per_sm=ctas, l2_hint=hint)
+    assert np.array_equal(run_op("mul", desc, [x, y]), ref)
+    check("mul", desc, [x, y])
+
+
+def test_output_may_alias_an_input():
+    for desc in (su3.make_desc((8, 8, 8, 6)), su3.make_desc((8, 8, 8, 6), prec=F32, layout=VE, W=8)):
+        x, y = host_field(desc, 23, su3gen.FIELD_X), host_field(desc, 23, su3gen.FIELD_Y)
+        ref = run_op("mul", desc, [x, y])
+        fx, fy = upload(desc, x), upload(desc, y)
+        su3.su3_mul(fx, fx, fy)
+        assert np.array_equal(download(fx), ref)
+        fx, fy = upload(desc, x), upload(desc, y)
+        su3.su3_mul(fy, fx, fy)
+        assert np.array_equal(download(fy), ref)
+
+
+def test_side_stream_and_launch_count():
+    desc = su3.make_desc(8)
+    x, y = host_field(desc, 29, su3gen.FIELD_X), host_field(desc, 29, su3gen.FIELD_Y)
+    fx, fy, fz = upload(desc, x), upload(desc, y), su3.alloc_field(desc)
+    torch.cuda.synchronize()
+    n0 = su3.su3_launch_count()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        su3.su3_mul(fz, fx, fy)
+    s.synchronize()
+    assert su3.su3_launch_count() == n0 + 1
+    err, _ = rel_err(download(fz), oracle.mul(geom_of(desc), x, y), 1)
+    assert err <= 1e-12
+
+
+def test_mul_host_end_to_end():
+    for desc in (su3.make_desc((8, 8, 8, 10)), su3.make_desc((3, 3, 3, 3), prec=F32),
+                 su3.make_desc((8, 8, 8, 8), prec=F32, layout=VE, W=8)):
+        x, y = host_field(desc, 31, su3gen.FIELD_X), host_field(desc, 31, su3gen.FIELD_Y)
+        hx, hy = torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()
+        hz = torch.empty_like(hx).pin_memory()
+        zd, xd, yd = (su3.alloc_field(desc) for _ in range(3))
+        for chunks in (0, 1, 5):
+            hz.zero_()
+            su3.su3_mul_host(hz, hx, hy, zd, xd, yd, chunks=chunks)
+            torch.cuda.synchronize()
+            err, _ = rel_err(hz.numpy(), oracle.mul(geom_of(desc), x, y), su3.su3_desc_normalize(desc).W)
+            assert err <= TOL[desc.prec]
