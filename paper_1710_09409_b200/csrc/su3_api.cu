@@ -179,17 +179,22 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     k<<<grid, 256, 0, stream>>>(p);
   } else {
-    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
-    const int64_t max_grid = (int64_t)di.sms * ctas;
+    int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
     int tm = tn.tile_mats;
     if (tm == 0) {  // auto: largest tile that still gives every persistent CTA a few tiles
       tm = 128;
-      while (tm > 32 && (nmat + tm - 1) / tm < 4 * max_grid) tm >>= 1;
+      while (tm > 32 && (nmat + tm - 1) / tm < 4 * (int64_t)di.sms * ctas) tm >>= 1;
     }
     if (tm != 32 && tm != 64 && tm != 128 && tm != 256) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128,256}", tm);
     const size_t stage_bytes = (size_t)nin * tm * 9 * cb;
     // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
-    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    // auto CTAs/SM: a big tile may leave room for fewer resident CTAs than the default
+    while (tn.ctas_per_sm == 0 && ctas > 1 && (budget - 256) / stage_bytes < 2) {
+      ctas--;
+      budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    }
+    const int64_t max_grid = (int64_t)di.sms * ctas;
     int stages = tn.stages;
     if (stages == 0) {
       stages = (int)((budget - 256) / stage_bytes);

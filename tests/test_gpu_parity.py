@@ -170,7 +170,7 @@ def test_custom_simd_split():
 
 # ------------------------------------------------------------------ launch configurations, aliasing
 @pytest.mark.parametrize("tile,stages,ctas,hint", [(32, 2, 1, 1), (64, 3, 2, 2), (128, 2, 4, 1), (128, 6, 1, 2),
-                                                   (256, 3, 1, 1), (256, 2, 2, 2), (128, 16, 1, 1)])
+                                                   (256, 3, 1, 1), (256, 2, 2, 2), (64, 16, 1, 1)])
 def test_launch_configurations_are_equivalent(tile, stages, ctas, hint):
     desc = su3.make_desc((16, 16, 8, 9), prec=F32)  # 18432 matrices; many tiles per CTA at ctas=1
     x, y = host_field(desc, 19, su3gen.FIELD_X), host_field(desc, 19, su3gen.FIELD_Y)
