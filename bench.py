@@ -1,0 +1,464 @@
+#!/usr/bin/env python
+"""bench.py -- the SU(3)xSU(3) streaming benchmark (BASELINE.json metric) on N B200s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--L 64] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A STEP is one pass of the whole hot path over one batch of
+seeded synthetic SU(3) fields on an L^4 lattice (default L = 64, fp64: the HBM-bound top of the
+volume sweep, BASELINE.json configs[4]; Listing 3):
+
+    A5  convert  x, y, w : scalar -> vector (W=4)          3 launches, 2 field streams each
+    A1  mul      zs = xs*ys          (scalar layout)       3 streams, 198 flop/matrix
+    A2  mul      zv = xv*yv          (vector layout W=4)   3 streams
+    A3  mul3     z3 = xv*yv*wv       (vector layout)       4 streams, 396 flop/matrix
+    A4  mul_add  z4 = xs*ys + vs     (scalar layout)       4 streams, 216 flop/matrix
+    A5  convert  zb = scalar(zv)                           2 streams
+    A6  copy     zc = zs             (the ceiling kernel)  2 streams
+
+`value` = algorithmic bytes of the step (S9: 24 field streams) / device time, inputs resident in HBM.
+`e2e`   = the same step with HOST buffers: x, y, w, v come from pinned host memory (x, y and the A1
+          result through the C-ABI call su3_mul_host) and the four results go back to the host,
+          all inside the timed region.
+One JSON line on stdout (rank 0); progress goes to stderr.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "su3xsu3_stream_GBps"
+UNIT = "GB/s"
+FLOPS = {"mul": 198, "mul3": 396, "mul_add": 216, "convert": 0, "copy": 0, "add": 18}
+STREAMS = {"mul": 3, "mul3": 4, "mul_add": 4, "convert": 2, "copy": 2, "add": 3}
+W64, W32 = 4, 8  # vector lengths of the configs: fp64 W=4, fp32 W=8 (64-byte element vectors)
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--L", type=int, default=64, help="local lattice extent per GPU (L^4 sites)")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the volume sweep (configs[4]) after the timed steps")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-L", type=int, default=32, help="lattice extent of the oracle's bounded sample")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------- the oracle legs
+def oracle_step(L, reps, threads=None):
+    """Time the oracle, as it stands, on `reps` passes of one step (rows A1-A6; A6 is a memcpy) of an L^4
+    fp64 lattice.  Returns (seconds per pass [reps], bytes a pass moves by S9's accounting, threads used)."""
+    import oracle
+    import su3gen
+    if threads:
+        oracle.set_num_threads(threads)
+    seed = su3gen.config_seed(5)
+    gs, gv = oracle.Geom(L), oracle.Geom(L, layout=oracle.su3_oracle.VECTOR, W=W64)
+    n = gs.nmat
+    xs, ys, ws = (su3gen.su3_field(seed, f, n).view(np.float64).reshape(-1) for f in (0, 1, 2))
+    vs = su3gen.gaussian_field(seed, 3, n).view(np.float64).reshape(-1)
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        xv, yv, wv = (oracle.convert(gv, gs, a) for a in (xs, ys, ws))
+        zs = oracle.mul(gs, xs, ys)
+        zv = oracle.mul(gv, xv, yv)
+        z3 = oracle.mul3(gv, xv, yv, wv)
+        z4 = oracle.mul_add(gs, xs, ys, vs)
+        zb = oracle.convert(gs, gv, zv)
+        zc = zs.copy()
+        times.append(time.perf_counter() - t0)
+    assert np.array_equal(zb, zs) and zc.size == zs.size and z3.size == z4.size
+    return times, 24 * n * 144, oracle.num_threads()
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle on the host cores, same metric/config; every step is one pass over a
+    bounded sample (a smaller lattice of the same sweep) so that W+K passes end within a few minutes."""
+    if rank != 0:
+        return
+    L = min(args.cpu_L, args.L)
+    if args.warmup + args.steps > 30:
+        L = min(L, 24)
+    times, nbytes, threads = oracle_step(L, args.warmup + args.steps)
+    timed = times[args.warmup:]
+    sec = sum(timed) / len(timed)
+    val = nbytes / sec / 1e9
+    sample = "every step = rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep; workload %d^4)" % (L, args.L)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg5 volume sweep top: %d^4 fp64, rows A1-A6" % args.L, "sample_L": L},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }), flush=True)
+
+
+# ---------------------------------------------------------------------------- clocks during the timed region
+CLOCK_Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+           "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+           "clocks_event_reasons.sw_power_cap")
+
+
+class ClockSampler:
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + CLOCK_Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); smax.append(float(c[2])); power.append(float(c[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(smax), "power_w_max": max(power),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+
+    import paper_1710_09409_b200 as su3   # raises if libsu3stream.so cannot be built/loaded: no fallback
+    import su3gen
+    from paper_1710_09409_b200 import shard
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    L = args.L
+    info = su3.su3_device_info()
+    F64, F32, SC, VE = su3.SU3_F64, su3.SU3_F32, su3.SU3_SCALAR, su3.SU3_VECTOR
+    ds, dv = su3.make_desc(L), su3.make_desc(L, layout=VE, W=W64)
+    nmat = L ** 4
+    B = su3.su3_field_bytes(ds)
+    # weak scaling: the global lattice is (L, L, L, L*world), rank r owns the x3 slab r (section 8(e))
+    gL = shard.weak_global_extents((L,) * 4, world)
+    m0, m1 = shard.matrix_range(gL, 1, rank, world)
+    assert m1 - m0 == nmat
+    seed = su3gen.config_seed(5)
+
+    # ---- seeded inputs, generated once on the host in fp64 (S10-S14) straight into pinned memory
+    t0 = time.time()
+    host = {}
+    for name, fid in (("x", su3gen.FIELD_X), ("y", su3gen.FIELD_Y), ("w", su3gen.FIELD_W), ("v", su3gen.FIELD_V)):
+        h = torch.empty(nmat * 9, dtype=torch.complex128, pin_memory=True)
+        a = h.numpy().reshape(nmat, 3, 3)
+        (su3gen.gaussian_field if name == "v" else su3gen.su3_field)(seed, fid, nmat, m0=m0, out=a)
+        host[name] = h
+    hz = [torch.empty(B, dtype=torch.uint8, pin_memory=True) for _ in range(2)]
+    log("[rank %d] generated 4 x %d^4 fields (%.2f GB each) in %.1f s" % (rank, L, B / 1e9, time.time() - t0))
+
+    def hbytes(t):
+        return torch.view_as_real(t).view(-1).view(torch.uint8) if t.dtype == torch.complex128 else t
+
+    f = {}
+    for n_ in ("xs", "ys", "ws", "vs", "zs", "z4", "zb", "zc"):
+        f[n_] = su3.alloc_field(ds, device=dev)
+    for n_ in ("xv", "yv", "wv", "zv", "z3"):
+        f[n_] = su3.alloc_field(dv, device=dev)
+    for n_ in ("x", "y", "w", "v"):
+        f[n_ + "s"].tensor.copy_(hbytes(host[n_]), non_blocking=True)
+    torch.cuda.synchronize()
+
+    rows = [  # (row, op, launch, field streams)
+        ("A5 convert xs->xv", "convert", lambda: su3.su3_convert(f["xv"], f["xs"])),
+        ("A5 convert ys->yv", "convert", lambda: su3.su3_convert(f["yv"], f["ys"])),
+        ("A5 convert ws->wv", "convert", lambda: su3.su3_convert(f["wv"], f["ws"])),
+        ("A1 mul scalar", "mul", lambda: su3.su3_mul(f["zs"], f["xs"], f["ys"])),
+        ("A2 mul vector W=%d" % W64, "mul", lambda: su3.su3_mul(f["zv"], f["xv"], f["yv"])),
+        ("A3 mul3 vector W=%d" % W64, "mul3", lambda: su3.su3_mul3(f["z3"], f["xv"], f["yv"], f["wv"])),
+        ("A4 mul_add scalar", "mul_add", lambda: su3.su3_mul_add(f["z4"], f["xs"], f["ys"], f["vs"])),
+        ("A5 convert zv->zb", "convert", lambda: su3.su3_convert(f["zb"], f["zv"])),
+        ("A6 copy zs->zc", "copy", lambda: su3.su3_copy(f["zc"], f["zs"])),
+    ]
+    step_bytes = sum(STREAMS[op] for _, op, _ in rows) * B
+    step_flops = sum(FLOPS[op] for _, op, _ in rows) * nmat
+
+    def step(events=None):
+        for i, (_, _, launch) in enumerate(rows):
+            if events is not None:
+                events[i].record()
+            launch()
+        if events is not None:
+            events[len(rows)].record()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps, per-launch events inside
+    clocks = ClockSampler(local_rank)   # sampled from here on: warm-up and timed steps are both under load
+    t_warm = time.perf_counter()
+    nwarm = 0
+    while nwarm < max(args.warmup, 3) or time.perf_counter() - t_warm < 0.6:
+        step()
+        torch.cuda.synchronize()
+        nwarm += 1
+    barrier()
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(len(rows) + 1)] for _ in range(K)]
+    n0 = su3.su3_launch_count()
+    barrier()
+    t_wall = time.perf_counter()
+    for k in range(K):
+        step(evs[k])
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t_wall = time.perf_counter() - t_wall
+    launches = su3.su3_launch_count() - n0
+    clk = clocks.stop()
+    total_ms = evs[0][0].elapsed_time(evs[K - 1][len(rows)])
+    row_ms = [float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)])) for i in range(len(rows))]
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = world * step_bytes / (ms_per_step * 1e-3) / 1e9
+
+    # ---- correctness tripwires on the full-size outputs (the parity tests proper are tests/ -m gpu)
+    torch.cuda.synchronize()
+    checks = {
+        "vector_result_equals_scalar_result_bitwise": bool(torch.equal(f["zb"].tensor, f["zs"].tensor)),
+        "copy_bitwise": bool(torch.equal(f["zc"].tensor, f["zs"].tensor)),
+    }
+    return dict(torch=torch, su3=su3, dist=dist, dev=dev, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
+                nmat=nmat, step_bytes=step_bytes, step_flops=step_flops, ms_per_step=ms_per_step, value=value,
+                launches=launches, clk=clk, checks=checks, info=info, t_wall=t_wall, barrier=barrier, step=step,
+                hbytes=hbytes)
+
+
+def time_calls(torch, fn, target_ms=2.0, batches=5, warm=3):
+    """SURVEY 8(d) protocol: warm-up calls, then `batches` batches of Nloop back-to-back calls between two
+    CUDA events on the current stream; returns (min, median) ms per call."""
+    for _ in range(warm):
+        fn()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); fn(); b.record(); b.synchronize()
+    est = max(a.elapsed_time(b), 1e-3)
+    nloop = int(min(1000, max(10, target_ms / est)))
+    per = []
+    for _ in range(batches):
+        a.record()
+        for _ in range(nloop):
+            fn()
+        b.record(); b.synchronize()
+        per.append(a.elapsed_time(b) / nloop)
+    return float(min(per)), float(np.median(per))
+
+
+def run_e2e(args, r, world):
+    """The same step with HOST buffers: x, y in and the A1 result out through su3_mul_host (chunked, copy/compute
+    overlapped inside the library); w, v in and the A2 (converted back), A3, A4 results out as plain async
+    copies on the same stream.  Everything between the two events is inside the timed region."""
+    torch, su3, f, host, hz, hbytes = r["torch"], r["su3"], r["f"], r["host"], r["hz"], r["hbytes"]
+    B = r["B"]
+    hx, hy, hw, hv = (hbytes(host[k]) for k in ("x", "y", "w", "v"))
+
+    def e2e_step():
+        su3.su3_mul_host(hz[0], hx, hy, f["zs"], f["xs"], f["ys"], chunks=8)       # A1 (+ x, y now resident)
+        f["ws"].tensor.copy_(hw, non_blocking=True)
+        f["vs"].tensor.copy_(hv, non_blocking=True)
+        su3.su3_convert(f["xv"], f["xs"]); su3.su3_convert(f["yv"], f["ys"]); su3.su3_convert(f["wv"], f["ws"])
+        su3.su3_mul(f["zv"], f["xv"], f["yv"])                                        # A2
+        su3.su3_convert(f["zb"], f["zv"])
+        hz[1].copy_(f["zb"].tensor, non_blocking=True)
+        su3.su3_mul3(f["z3"], f["xv"], f["yv"], f["wv"])                              # A3
+        hz[1].copy_(f["z3"].tensor, non_blocking=True)
+        su3.su3_mul_add(f["z4"], f["xs"], f["ys"], f["vs"])                           # A4
+        hz[1].copy_(f["z4"].tensor, non_blocking=True)
+        su3.su3_copy(f["zc"], f["zs"])                                                # A6
+
+    n = max(2, min(args.steps, 5))
+    e2e_step()
+    r["barrier"]()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(n):
+        e2e_step()
+    b.record()
+    b.synchronize()
+    ms = a.elapsed_time(b) / n
+    if r["dist"] is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=r["dev"])
+        r["dist"].all_reduce(t, op=r["dist"].ReduceOp.MAX)
+        ms = float(t.item())
+    ok = bool(torch.equal(hz[0], f["zs"].tensor.cpu()))
+    return {"value": world * r["step_bytes"] / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
+            "d2h_bytes_per_step": 4 * B, "ms_per_step": ms, "steps": n,
+            "api": "su3_mul_host (A1) + pinned async copies around su3_convert/su3_mul/su3_mul3/su3_mul_add/su3_copy",
+            "host_result_matches_device": ok}
+
+
+def run_ceilings_and_sweep(args, r):
+    """Same-run ceilings (A6: own copy kernel, cudaMemcpyAsync D2D, the 2-read-1-write add) at the workload
+    size, then the volume sweep of BASELINE.json configs[4]: z = x*y for L = 8..64, fp64/fp32, scalar/vector,
+    warm protocol (Listing 3: same operands every call).  Operands are prefixes of the resident fields."""
+    torch, su3, f, B = r["torch"], r["su3"], r["f"], r["B"]
+    l2 = r["info"]["l2_bytes"]
+    out = {}
+    mn, md = time_calls(torch, lambda: su3.su3_copy(f["zc"], f["zs"]))
+    out["su3_copy"] = 2 * B / (mn * 1e-3) / 1e9
+    mn, md = time_calls(torch, lambda: f["zc"].tensor.copy_(f["zs"].tensor))
+    out["memcpy_d2d"] = 2 * B / (mn * 1e-3) / 1e9
+    mn, md = time_calls(torch, lambda: su3.su3_add(f["zc"], f["xs"], f["ys"]))
+    out["su3_add_2r1w"] = 3 * B / (mn * 1e-3) / 1e9
+    ceiling = max(out["su3_copy"], out["memcpy_d2d"])
+    out["bar_denominator"] = ceiling
+    if args.no_sweep:
+        return out, []
+    # fp32 copies of x, y in both layouts (input preparation only: rounding fp64 -> fp32, S16)
+    x32 = f["xs"].tensor.view(torch.float64).to(torch.float32)
+    y32 = f["ys"].tensor.view(torch.float64).to(torch.float32)
+    d32s = su3.make_desc(args.L, prec=su3.SU3_F32)
+    d32v = su3.make_desc(args.L, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=W32)
+    fx32s, fy32s = su3.su3_field_wrap(d32s, x32.view(torch.uint8)), su3.su3_field_wrap(d32s, y32.view(torch.uint8))
+    fx32v, fy32v = su3.alloc_field(d32v), su3.alloc_field(d32v)
+    su3.su3_convert(fx32v, fx32s); su3.su3_convert(fy32v, fy32s)
+    src = {(8, 0): (f["xs"], f["ys"], f["zc"]), (8, 1): (f["xv"], f["yv"], f["zc"]),
+           (4, 0): (fx32s, fy32s, f["zc"]), (4, 1): (fx32v, fy32v, f["zc"])}
+    sweep = []
+    for Ls in (8, 12, 16, 24, 32, 48, 64):
+        if Ls > args.L:
+            continue
+        for prec in (8, 4):
+            for layout in (0, 1):
+                W = 1 if layout == 0 else (W64 if prec == 8 else W32)
+                d = su3.make_desc(Ls, prec=prec, layout=layout, W=W)
+                nb = su3.su3_field_bytes(d)
+                xs_, ys_, zs_ = src[(prec, layout)]
+                fx = su3.su3_field_wrap(d, xs_.tensor[:nb]); fy = su3.su3_field_wrap(d, ys_.tensor[:nb])
+                fz = su3.su3_field_wrap(d, zs_.tensor[:nb])
+                mn, md = time_calls(torch, lambda: su3.su3_mul(fz, fx, fy))
+                gbs = 3 * nb / (mn * 1e-3) / 1e9
+                regime = "L2-resident" if 3 * nb < 0.75 * l2 else ("HBM-bound" if 3 * nb > 2 * l2 else "straddles L2")
+                sweep.append({"L": Ls, "prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector",
+                              "W": W, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3,
+                              "GBps": gbs, "GFLOPps": FLOPS["mul"] * Ls ** 4 / (mn * 1e-3) / 1e9, "regime": regime,
+                              "frac_of_copy": gbs / ceiling if regime == "HBM-bound" else None})
+    return out, sweep
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world != args.gpus:
+        log("note: --gpus %d but WORLD_SIZE=%d; using WORLD_SIZE (launch N>1 with torch.distributed.run)" % (args.gpus, world))
+    r = run_ours(args, rank, world, local_rank)
+    torch = r["torch"]
+    e2e = None if args.no_e2e else run_e2e(args, r, world)
+    ceilings, sweep = ({}, [])
+    if rank == 0:
+        ceilings, sweep = run_ceilings_and_sweep(args, r)
+    peak, peak_src = measured_peak()
+    B, nmat = r["B"], r["nmat"]
+    ops = []
+    for (name, op, _), ms in zip(r["rows"], r["row_ms"]):
+        gbs = STREAMS[op] * B / (ms * 1e-3) / 1e9
+        ops.append({"row": name, "ms": ms, "GBps": gbs, "GFLOPps": FLOPS[op] * nmat / (ms * 1e-3) / 1e9,
+                    "frac_of_measured_peak": gbs / peak,
+                    "frac_of_copy": gbs / ceilings["bar_denominator"] if ceilings else None})
+    a1 = ops[3]
+    roofline = {"bound": "hbm", "kernel": "su3_pipe_kernel<double,W=1,OP_MUL> (row A1, z=x*y fp64 scalar)",
+                "achieved": a1["GBps"], "peak": peak, "unit": "GB/s", "frac": a1["GBps"] / peak, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": 3 * B, "avg_launch_ms": a1["ms"], "traffic": None,
+                "traffic_note": "see profiles/ for the ncu --set full dram__bytes of this kernel"}
+    cpu = None
+    if rank == 0 and not args.no_cpu:
+        Lc = min(args.cpu_L, args.L)
+        times, nbytes, threads = oracle_step(Lc, 3)
+        cpu = {"value": nbytes / min(times) / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": "rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep), best of 3 passes" % Lc}
+    if r["dist"] is not None:
+        r["dist"].barrier()
+        r["dist"].destroy_process_group()
+    if rank != 0:
+        return
+    line = {
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[4] top point: %d^4 lattice per GPU (%d matrices, %.3f GB per field), "
+                               "fp64 complex, scalar + vector(W=%d) layouts, rows A1-A6 per step" % (args.L, nmat, B / 1e9, W64),
+                   "L": args.L, "step_bytes": r["step_bytes"], "step_flops": r["step_flops"],
+                   "l2_policy": "inputs larger than L2 (every launch streams >= %.1f GB; L2 = %.0f MB)" % (2 * B / 1e9, r["info"]["l2_bytes"] / 1e6),
+                   "parallelism": "independent x3 slabs, no collective" if world > 1 else "single GPU"},
+        "GFLOPps": world * r["step_flops"] / (r["ms_per_step"] * 1e-3) / 1e9,
+        "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+        "ops": ops, "ceilings_GBps": ceilings, "sweep": sweep, "checks": r["checks"],
+        "wall_s_timed_region": r["t_wall"],
+    }
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()
