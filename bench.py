@@ -292,23 +292,37 @@ def run_ours(args, rank, world, local_rank):
                 hbytes=hbytes)
 
 
-def time_calls(torch, fn, target_ms=2.0, batches=5, warm=3):
+def time_calls(torch, fn, target_ms=2.0, batches=5, warm=3, graph_below_us=0.0):
     """SURVEY 8(d) protocol: warm-up calls, then `batches` batches of Nloop back-to-back calls between two
-    CUDA events on the current stream; returns (min, median) ms per call."""
+    CUDA events on the current stream; returns (min, median) ms per call and how the calls were issued.
+    Calls shorter than `graph_below_us` are launch-bound from Python: their Nloop calls are captured once
+    into a CUDA graph and the graph is replayed (the library's calls are capturable: no sync, no allocation)."""
     for _ in range(warm):
         fn()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(); fn(); b.record(); b.synchronize()
-    est = max(a.elapsed_time(b), 1e-3)
+    a.record(); fn(); fn(); b.record(); b.synchronize()
+    est = max(a.elapsed_time(b) / 2, 1e-3)
     nloop = int(min(1000, max(10, target_ms / est)))
+    how = "stream"
+    run = None
+    if est * 1e3 < graph_below_us:
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for _ in range(nloop):
+                fn()
+        run, how = g.replay, "cuda_graph(%d calls)" % nloop
+        run()
     per = []
     for _ in range(batches):
         a.record()
-        for _ in range(nloop):
-            fn()
+        if run is not None:
+            run()
+        else:
+            for _ in range(nloop):
+                fn()
         b.record(); b.synchronize()
         per.append(a.elapsed_time(b) / nloop)
-    return float(min(per)), float(np.median(per))
+    return float(min(per)), float(np.median(per)), how
 
 
 def run_e2e(args, r, world):
@@ -361,11 +375,11 @@ def run_ceilings_and_sweep(args, r):
     torch, su3, f, B = r["torch"], r["su3"], r["f"], r["B"]
     l2 = r["info"]["l2_bytes"]
     out = {}
-    mn, md = time_calls(torch, lambda: su3.su3_copy(f["zc"], f["zs"]))
+    mn, md, _ = time_calls(torch, lambda: su3.su3_copy(f["zc"], f["zs"]))
     out["su3_copy"] = 2 * B / (mn * 1e-3) / 1e9
-    mn, md = time_calls(torch, lambda: f["zc"].tensor.copy_(f["zs"].tensor))
+    mn, md, _ = time_calls(torch, lambda: f["zc"].tensor.copy_(f["zs"].tensor))
     out["memcpy_d2d"] = 2 * B / (mn * 1e-3) / 1e9
-    mn, md = time_calls(torch, lambda: su3.su3_add(f["zc"], f["xs"], f["ys"]))
+    mn, md, _ = time_calls(torch, lambda: su3.su3_add(f["zc"], f["xs"], f["ys"]))
     out["su3_add_2r1w"] = 3 * B / (mn * 1e-3) / 1e9
     ceiling = max(out["su3_copy"], out["memcpy_d2d"])
     out["bar_denominator"] = ceiling
@@ -393,12 +407,29 @@ def run_ceilings_and_sweep(args, r):
                 xs_, ys_, zs_ = src[(prec, layout)]
                 fx = su3.su3_field_wrap(d, xs_.tensor[:nb]); fy = su3.su3_field_wrap(d, ys_.tensor[:nb])
                 fz = su3.su3_field_wrap(d, zs_.tensor[:nb])
-                mn, md = time_calls(torch, lambda: su3.su3_mul(fz, fx, fy))
+                mn, md, how = time_calls(torch, lambda: su3.su3_mul(fz, fx, fy), graph_below_us=60.0)
                 gbs = 3 * nb / (mn * 1e-3) / 1e9
                 regime = "L2-resident" if 3 * nb < 0.75 * l2 else ("HBM-bound" if 3 * nb > 2 * l2 else "straddles L2")
+                cold = None
+                if regime != "HBM-bound":
+                    # "cold" protocol (S18): rotate through operand triples so that a call never finds its lines
+                    # in L2; triple k = the k-th nb-sized slice of the resident 64^4-sized fields
+                    nb_al = (nb + 255) // 256 * 256
+                    ntrip = int(min(zs_.tensor.numel() // nb_al, xs_.tensor.numel() // nb_al, 2 * l2 // (3 * nb) + 2))
+                    if ntrip * 3 * nb > 2 * l2:
+                        trip = [tuple(su3.su3_field_wrap(d, t.tensor[k * nb_al:k * nb_al + nb]) for t in (zs_, xs_, ys_))
+                                for k in range(ntrip)]
+                        ctr = [0]
+
+                        def rot():
+                            z_, x_, y_ = trip[ctr[0] % ntrip]
+                            ctr[0] += 1
+                            su3.su3_mul(z_, x_, y_)
+                        cmn, _, _ = time_calls(torch, rot, target_ms=4.0, warm=ntrip, graph_below_us=60.0)
+                        cold = 3 * nb / (cmn * 1e-3) / 1e9
                 sweep.append({"L": Ls, "prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector",
-                              "W": W, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3,
-                              "GBps": gbs, "GFLOPps": FLOPS["mul"] * Ls ** 4 / (mn * 1e-3) / 1e9, "regime": regime,
+                              "W": W, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3, "issued": how,
+                              "GBps": gbs, "GFLOPps": FLOPS["mul"] * Ls ** 4 / (mn * 1e-3) / 1e9, "regime": regime, "cold_GBps": cold,
                               "frac_of_copy": gbs / ceiling if regime == "HBM-bound" else None})
     return out, sweep
 

@@ -83,7 +83,7 @@ typedef struct su3_field su3_field; /* opaque: validated descriptor + device poi
  * They never change results, only speed; bench.py and the tests use them to pin
  * the launch configuration that is being measured. */
 typedef struct {
-  int32_t tile_mats;    /* matrices per pipeline tile: 32, 64, 128 or 256               */
+  int32_t tile_mats;    /* matrices per pipeline tile: 32, 64 or 128 (su3_copy: x matrix bytes) */
   int32_t stages;       /* shared-memory ring depth, 2..16                             */
   int32_t ctas_per_sm;  /* persistent CTAs per SM, 1..8                                 */
   int32_t l2_hint;      /* 0 auto (by footprint), 1 none, 2 evict_first loads+stores   */

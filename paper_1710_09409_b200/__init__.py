@@ -125,7 +125,7 @@ class Field:
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None
-        if h:
+        if h and lib is not None:  # lib is None while the interpreter shuts down
             lib.su3_field_free(h)
 
 

@@ -112,7 +112,7 @@ const DevInfo &devinfo() {
 
 // ---------------------------------------------------------------- kernel tables
 typedef void (*stream_kernel_t)(const su3::StreamParams);
-constexpr int NCW = 8;  // consumer warps per CTA of the pipeline kernel (tile <= 256 matrices)
+constexpr int NCW = 4;  // consumer warps per CTA of the pipeline kernel (tile <= 128 matrices)
 
 template <typename R, int OP> stream_kernel_t pipe_for_w(int W) {
   switch (W) {
@@ -141,8 +141,21 @@ template <typename R> stream_kernel_t pick(int op, int W, bool direct) {
     case su3::OP_MUL: return direct ? direct_for_w<R, su3::OP_MUL>(W) : pipe_for_w<R, su3::OP_MUL>(W);
     case su3::OP_MUL3: return direct ? direct_for_w<R, su3::OP_MUL3>(W) : pipe_for_w<R, su3::OP_MUL3>(W);
     case su3::OP_MUL_ADD: return direct ? direct_for_w<R, su3::OP_MUL_ADD>(W) : pipe_for_w<R, su3::OP_MUL_ADD>(W);
+    case su3::OP_ADD: return direct ? nullptr : pipe_for_w<R, su3::OP_ADD>(1);  // element-wise: layout-agnostic
   }
   return nullptr;
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and process, not once per launch
+cudaError_t allow_max_smem(const void *fn, int bytes) {
+  static std::mutex mu;
+  static std::vector<const void *> done;
+  std::lock_guard<std::mutex> lk(mu);
+  for (const void *d : done)
+    if (d == fn) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) done.push_back(fn);
+  return e;
 }
 
 su3_status cuda_fail(const char *what, cudaError_t e) {
@@ -160,7 +173,7 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
     std::lock_guard<std::mutex> lk(g_tune_mu);
     tn = g_tune;
   }
-  const int nin = (op == su3::OP_MUL) ? 2 : 3;
+  const int nin = (op == su3::OP_MUL || op == su3::OP_ADD) ? 2 : 3;
   const int cb = 2 * prec;
   const bool direct = tn.path == 2;
   stream_kernel_t k = (prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct);
@@ -179,13 +192,16 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     k<<<grid, 256, 0, stream>>>(p);
   } else {
+    // defaults measured on B200: 9 KB operand slots (64 fp64 / 128 fp32 matrices),
+    // a 3-deep ring, 2 persistent CTAs per SM
     int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
     int tm = tn.tile_mats;
-    if (tm == 0) {  // auto: largest tile that still gives every persistent CTA a few tiles
-      tm = 128;
-      while (tm > 32 && (nmat + tm - 1) / tm < 4 * (int64_t)di.sms * ctas) tm >>= 1;
+    if (tm == 0) {
+      tm = 9216 / (9 * cb);
+      // small lattices: shrink the tile until every persistent CTA has at least two tiles
+      while (tm > 32 && (nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
     }
-    if (tm != 32 && tm != 64 && tm != 128 && tm != 256) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128,256}", tm);
+    if (tm != 32 && tm != 64 && tm != 128) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128}", tm);
     const size_t stage_bytes = (size_t)nin * tm * 9 * cb;
     // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
     size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
@@ -197,13 +213,13 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
     const int64_t max_grid = (int64_t)di.sms * ctas;
     int stages = tn.stages;
     if (stages == 0) {
-      stages = (int)((budget - 256) / stage_bytes);
-      if (stages > 8) stages = 8;
+      stages = 3;
+      while (stages > 2 && stages * stage_bytes + 256 > budget) stages--;
     }
     if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);
     const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t);
     if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "pipeline needs %zu B of shared memory, device allows %d", smem, di.smem_optin);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
     if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
     p.tile_mats = tm; p.stages = stages;
     const int64_t ntiles = (nmat + tm - 1) / tm;
@@ -349,6 +365,14 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *s
   if (st != SU3_OK) return st;
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  int path;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    path = g_tune.path;
+  }
+  if (path != 2)  // element-wise, hence layout-agnostic: the W = 1 pipeline over 9-complex records
+    return launch_stream(su3::OP_ADD, z->d.prec, 1, z->ptr, x->ptr, y->ptr, nullptr, z->nmat, 3 * z->nbytes,
+                         (cudaStream_t)stream);
   const size_t n16 = z->nbytes / 16;
   const int nrem = (int)((z->nbytes % 16) / z->d.prec);
   const unsigned grid = flat_grid(n16, 512, 8);
@@ -367,10 +391,38 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
   if (!same_desc(dst->d, src->d)) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors");
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
-  const size_t n16 = dst->nbytes / 16;
-  const int tail8 = (dst->nbytes % 16) ? 1 : 0;
-  const unsigned grid = flat_grid(n16, 1024, 8);
-  su3::su3_copy_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((uint4 *)dst->ptr, (const uint4 *)src->ptr, n16, tail8);
+  if (dst->nbytes == 0) return SU3_OK;
+  su3_tune tn;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    tn = g_tune;
+  }
+  if (tn.path != 2) {  // TMA bulk pipeline: global -> shared -> global, one issuing thread per CTA
+    const int mat_bytes = 18 * dst->d.prec;
+    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 3;
+    unsigned tile = tn.tile_mats > 0 ? (unsigned)tn.tile_mats * mat_bytes : 18432u;  // multiple of 16
+    const size_t n16 = dst->nbytes & ~(size_t)15;
+    while (tile > 2304 && (n16 + tile - 1) / tile < (size_t)2 * di.sms * ctas) tile >>= 1;
+    int stages = tn.stages > 0 ? tn.stages : 2;
+    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    while (stages > 2 && (size_t)stages * tile + 256 > budget) stages--;
+    const size_t smem = (size_t)stages * tile + stages * sizeof(uint64_t);
+    if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "su3_copy pipeline needs %zu B of shared memory", smem);
+    cudaError_t e = allow_max_smem((const void *)su3::su3_bulk_copy_kernel, di.smem_optin);
+    if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
+    su3::CopyParams p;
+    p.dst = dst->ptr; p.src = src->ptr; p.nbytes = dst->nbytes; p.tile_bytes = tile; p.stages = stages;
+    p.hint = tn.l2_hint == 2;
+    size_t ntiles = (n16 + tile - 1) / tile;
+    if (ntiles < 1) ntiles = 1;
+    const size_t cap = (size_t)di.sms * ctas;
+    su3::su3_bulk_copy_kernel<<<(unsigned)(ntiles < cap ? ntiles : cap), 32, smem, (cudaStream_t)stream>>>(p);
+  } else {
+    const size_t n16 = dst->nbytes / 16;
+    const int tail8 = (dst->nbytes % 16) ? 1 : 0;
+    const unsigned grid = flat_grid(n16, 1024, 8);
+    su3::su3_copy_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((uint4 *)dst->ptr, (const uint4 *)src->ptr, n16, tail8);
+  }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_copy launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);
@@ -485,8 +537,8 @@ su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su
 su3_status su3_tune_set(const su3_tune *t) {
   su3_tune v = {0, 0, 0, 0, 0, {0, 0, 0}};
   if (t) v = *t;
-  if (v.tile_mats != 0 && v.tile_mats != 32 && v.tile_mats != 64 && v.tile_mats != 128 && v.tile_mats != 256)
-    return fail(SU3_ERR_INVALID, "tile_mats = %d not in {0,32,64,128,256}", v.tile_mats);
+  if (v.tile_mats != 0 && v.tile_mats != 32 && v.tile_mats != 64 && v.tile_mats != 128)
+    return fail(SU3_ERR_INVALID, "tile_mats = %d not in {0,32,64,128}", v.tile_mats);
   if (v.stages != 0 && (v.stages < 2 || v.stages > 16)) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16", v.stages);
   if (v.ctas_per_sm < 0 || v.ctas_per_sm > 8) return fail(SU3_ERR_INVALID, "ctas_per_sm = %d outside 0..8", v.ctas_per_sm);
   if (v.l2_hint < 0 || v.l2_hint > 2) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..2", v.l2_hint);

@@ -30,7 +30,7 @@
 
 namespace su3 {
 
-enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2 };
+enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2, OP_ADD = 3 };
 
 // ---------------------------------------------------------------- complex helpers
 template <typename R> struct Cplx;
@@ -157,14 +157,14 @@ struct StreamParams {
   int hint;        // 1: L2 evict_first on loads and stores
 };
 
-template <int OP> struct NumInputs { static const int value = (OP == OP_MUL) ? 2 : 3; };
+template <int OP> struct NumInputs { static const int value = (OP == OP_MUL || OP == OP_ADD) ? 2 : 3; };
 
 // One thread's matrix: element e of lane l of record q sits at complex index (q*9 + e)*W + l
 // of the slot.  Thread t owns (q = t / W, l = t % W).  Bank check: with
 // 16-byte (fp64) or 8-byte (fp32) complex numbers every quarter-/half-warp request covers
 // all 32 banks exactly once for every W in {1,2,4,8,16,32}.
 template <typename R, int W, int OP, int NCW>
-__global__ void __launch_bounds__((NCW + 1) * 32) su3_pipe_kernel(const StreamParams p) {
+__global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_pipe_kernel(const StreamParams p) {
   typedef typename Cplx<R>::type C2;
   constexpr int NIN = NumInputs<OP>::value;
   constexpr int CB = (int)sizeof(C2);
@@ -252,7 +252,15 @@ __global__ void __launch_bounds__((NCW + 1) * 32) su3_pipe_kernel(const StreamPa
       for (int e = 0; e < 9; e++) a[e] = sx[e * W];
 #pragma unroll
       for (int e = 0; e < 9; e++) b[e] = sy[e * W];
-      mat33_mul(a, b, c);
+      if (OP == OP_ADD) {
+#pragma unroll
+        for (int e = 0; e < 9; e++) {
+          c[e].x = add_rn(a[e].x, b[e].x);
+          c[e].y = add_rn(a[e].y, b[e].y);
+        }
+      } else {
+        mat33_mul(a, b, c);
+      }
       if (OP == OP_MUL3) {
         const C2 *su = reinterpret_cast<const C2 *>(st + 2 * slot_bytes) + base;
 #pragma unroll
@@ -346,8 +354,72 @@ __global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
 }
 
 // ---------------------------------------------------------------- streaming ceilings (A6) and z = x + y
+// dst = src as a pure TMA pipeline: one thread per CTA moves tiles global -> shared -> global with
+// 1-D bulk copies through a ring of `stages` slots; no register ever holds data.  The ceiling the
+// arithmetic kernels are compared with uses the same memory machinery as they do.
+struct CopyParams {
+  void *dst;
+  const void *src;
+  unsigned long long nbytes;  // multiple of 8
+  unsigned tile_bytes;        // multiple of 16
+  int stages;
+  int hint;
+};
+
+__global__ void __launch_bounds__(32) su3_bulk_copy_kernel(const CopyParams p) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  if (threadIdx.x != 0) return;
+  const int S = p.stages;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)S * p.tile_bytes);
+  for (int s = 0; s < S; s++) mbar_init(&full[s], 1);
+  fence_mbar_init();
+  fence_proxy_async();
+  const unsigned long long n16 = p.nbytes & ~15ull;
+  const unsigned long long ntiles = (n16 + p.tile_bytes - 1) / p.tile_bytes;
+  const unsigned char *src = (const unsigned char *)p.src;
+  unsigned char *dst = (unsigned char *)p.dst;
+  uint64_t pol = 0;
+  if (p.hint) pol = policy_evict_first();
+  // my tiles: blockIdx.x, blockIdx.x + gridDim.x, ...
+  const unsigned long long mine = ntiles > blockIdx.x ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  auto tile_off = [&](unsigned long long i) { return (blockIdx.x + i * gridDim.x) * (unsigned long long)p.tile_bytes; };
+  auto tile_len = [&](unsigned long long off) {
+    const unsigned long long left = n16 - off;
+    return (uint32_t)(left < p.tile_bytes ? left : p.tile_bytes);
+  };
+  auto load = [&](unsigned long long i) {
+    const int s = (int)(i % S);
+    const unsigned long long off = tile_off(i);
+    const uint32_t len = tile_len(off);
+    mbar_arrive_expect_tx(&full[s], len);
+    if (p.hint)
+      bulk_g2s_hint(smem + (size_t)s * p.tile_bytes, src + off, len, &full[s], pol);
+    else
+      bulk_g2s(smem + (size_t)s * p.tile_bytes, src + off, len, &full[s]);
+  };
+  for (unsigned long long i = 0; i < mine && i < (unsigned long long)S; i++) load(i);
+  for (unsigned long long i = 0; i < mine; i++) {
+    const int s = (int)(i % S);
+    mbar_wait(&full[s], (uint32_t)((i / S) & 1));
+    const unsigned long long off = tile_off(i);
+    if (p.hint)
+      bulk_s2g_hint(dst + off, smem + (size_t)s * p.tile_bytes, tile_len(off), pol);
+    else
+      bulk_s2g(dst + off, smem + (size_t)s * p.tile_bytes, tile_len(off));
+    bulk_commit();
+    // the store before this one has finished reading its slot: refill that slot
+    if (i >= 1) {
+      bulk_wait_read<1>();
+      if (i - 1 + S < mine) load(i - 1 + S);
+    }
+  }
+  if (blockIdx.x == 0 && p.nbytes != n16)
+    *reinterpret_cast<uint64_t *>(dst + n16) = *reinterpret_cast<const uint64_t *>(src + n16);
+  bulk_wait_all<0>();
+}
+
 // dst = src over n16 16-byte words (+ an optional 8-byte tail), 4 independent 128-bit loads
-// in flight per thread.
+// in flight per thread (path = 2: the plain LDG/STG copy, kept as the measured comparison).
 __global__ void __launch_bounds__(256) su3_copy_kernel(uint4 *__restrict__ dst, const uint4 *__restrict__ src,
                                                        size_t n16, int tail8) {
   const size_t bd = blockDim.x;

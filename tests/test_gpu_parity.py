@@ -136,7 +136,7 @@ def test_all_ops_every_W(prec, layout, W, path):
 def test_ragged_and_lorentz(prec, L, nl, layout, W):
     desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
     x, y, w = (host_field(desc, 13, f) for f in (su3gen.FIELD_X, su3gen.FIELD_Y, su3gen.FIELD_W))
-    for tile in (0, 32, 256):
+    for tile in (0, 32, 128):
         su3.su3_tune_set(tile_mats=tile)
         check("mul", desc, [x, y])
     su3.su3_tune_set()
@@ -170,7 +170,7 @@ def test_custom_simd_split():
 
 # ------------------------------------------------------------------ launch configurations, aliasing
 @pytest.mark.parametrize("tile,stages,ctas,hint", [(32, 2, 1, 1), (64, 3, 2, 2), (128, 2, 4, 1), (128, 6, 1, 2),
-                                                   (256, 3, 1, 1), (256, 2, 2, 2), (64, 16, 1, 1)])
+                                                   (128, 3, 3, 1), (32, 2, 4, 2), (64, 16, 1, 1)])
 def test_launch_configurations_are_equivalent(tile, stages, ctas, hint):
     desc = su3.make_desc((16, 16, 8, 9), prec=F32)  # 18432 matrices; many tiles per CTA at ctas=1
     x, y = host_field(desc, 19, su3gen.FIELD_X), host_field(desc, 19, su3gen.FIELD_Y)
