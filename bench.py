@@ -273,12 +273,10 @@ def run_ours(args, rank, world, local_rank):
     clk = clocks.stop()
     total_ms = evs[0][0].elapsed_time(evs[K - 1][len(rows)])
     row_ms = [float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)])) for i in range(len(rows))]
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    # whole-job value: bytes of all ranks / max-over-ranks device time (independent shards, no collective)
+    rate, total_ms, _ = shard.job_throughput(K * step_bytes, total_ms, dist, dev)
     ms_per_step = total_ms / K
-    value = world * step_bytes / (ms_per_step * 1e-3) / 1e9
+    value = rate / 1e9
 
     # ---- correctness tripwires on the full-size outputs (the parity tests proper are tests/ -m gpu)
     torch.cuda.synchronize()
@@ -356,13 +354,10 @@ def run_e2e(args, r, world):
         e2e_step()
     b.record()
     b.synchronize()
-    ms = a.elapsed_time(b) / n
-    if r["dist"] is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=r["dev"])
-        r["dist"].all_reduce(t, op=r["dist"].ReduceOp.MAX)
-        ms = float(t.item())
+    from paper_1710_09409_b200 import shard
+    rate, ms, _ = shard.job_throughput(r["step_bytes"], a.elapsed_time(b) / n, r["dist"], r["dev"])
     ok = bool(torch.equal(hz[0], f["zs"].tensor.cpu()))
-    return {"value": world * r["step_bytes"] / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
+    return {"value": rate / 1e9, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
             "d2h_bytes_per_step": 4 * B, "ms_per_step": ms, "steps": n,
             "api": "su3_mul_host (A1) + pinned async copies around su3_convert/su3_mul/su3_mul3/su3_mul_add/su3_copy",
             "host_result_matches_device": ok}

@@ -29,3 +29,18 @@ def matrix_range(global_L, n_lorentz, rank, world):
     """[m0, m1) of the global logical matrix index m = site*n_lorentz + mu owned by rank."""
     _, s0, vol = local_extents(global_L, rank, world)
     return s0 * n_lorentz, (s0 + vol) * n_lorentz
+
+
+def job_throughput(local_units, local_ms, dist=None, device=None):
+    """Whole-job throughput of independent shards: (sum over ranks of units) / (max over ranks of time).
+    `dist` is an initialised torch.distributed module (or None for one process).  Returns
+    (units_per_second, max_ms, total_units)."""
+    total, worst = float(local_units), float(local_ms)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        import torch
+        t = torch.tensor([worst], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        u = torch.tensor([total], dtype=torch.float64, device=device)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        worst, total = float(t.item()), float(u.item())
+    return total / (worst * 1e-3), worst, total
