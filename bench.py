@@ -331,19 +331,41 @@ def run_e2e(args, r, world):
     B = r["B"]
     hx, hy, hw, hv = (hbytes(host[k]) for k in ("x", "y", "w", "v"))
 
+    h2d_s, d2h_s = torch.cuda.Stream(), torch.cuda.Stream()
+
     def e2e_step():
-        su3.su3_mul_host(hz[0], hx, hy, f["zs"], f["xs"], f["ys"], chunks=8)       # A1 (+ x, y now resident)
-        f["ws"].tensor.copy_(hw, non_blocking=True)
-        f["vs"].tensor.copy_(hv, non_blocking=True)
-        su3.su3_convert(f["xv"], f["xs"]); su3.su3_convert(f["yv"], f["ys"]); su3.su3_convert(f["wv"], f["ws"])
+        main = torch.cuda.current_stream()
+        start = torch.cuda.Event(); start.record(main)
+        # A1: x, y in and z out, chunked and overlapped inside the library; x, y stay resident for A2-A4
+        su3.su3_mul_host(hz[0], hx, hy, f["zs"], f["xs"], f["ys"], chunks=8)
+        # w, v follow x, y on the H2D engine while the A1 result is already flowing back
+        h2d_s.wait_event(start)
+        with torch.cuda.stream(h2d_s):
+            f["ws"].tensor.copy_(hw, non_blocking=True)
+            ev_w = torch.cuda.Event(); ev_w.record(h2d_s)
+            f["vs"].tensor.copy_(hv, non_blocking=True)
+            ev_v = torch.cuda.Event(); ev_v.record(h2d_s)
+
+        def result_to_host(field):
+            ev = torch.cuda.Event(); ev.record(main)
+            d2h_s.wait_event(ev)
+            with torch.cuda.stream(d2h_s):
+                hz[1].copy_(field.tensor, non_blocking=True)
+
+        su3.su3_convert(f["xv"], f["xs"]); su3.su3_convert(f["yv"], f["ys"])
         su3.su3_mul(f["zv"], f["xv"], f["yv"])                                        # A2
         su3.su3_convert(f["zb"], f["zv"])
-        hz[1].copy_(f["zb"].tensor, non_blocking=True)
-        su3.su3_mul3(f["z3"], f["xv"], f["yv"], f["wv"])                              # A3
-        hz[1].copy_(f["z3"].tensor, non_blocking=True)
-        su3.su3_mul_add(f["z4"], f["xs"], f["ys"], f["vs"])                           # A4
-        hz[1].copy_(f["z4"].tensor, non_blocking=True)
+        result_to_host(f["zb"])
         su3.su3_copy(f["zc"], f["zs"])                                                # A6
+        main.wait_event(ev_w)
+        su3.su3_convert(f["wv"], f["ws"])
+        su3.su3_mul3(f["z3"], f["xv"], f["yv"], f["wv"])                              # A3
+        result_to_host(f["z3"])
+        main.wait_event(ev_v)
+        su3.su3_mul_add(f["z4"], f["xs"], f["ys"], f["vs"])                           # A4
+        result_to_host(f["z4"])
+        done = torch.cuda.Event(); done.record(d2h_s)
+        main.wait_event(done)
 
     n = max(2, min(args.steps, 5))
     e2e_step()
@@ -359,7 +381,7 @@ def run_e2e(args, r, world):
     ok = bool(torch.equal(hz[0], f["zs"].tensor.cpu()))
     return {"value": rate / 1e9, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
             "d2h_bytes_per_step": 4 * B, "ms_per_step": ms, "steps": n,
-            "api": "su3_mul_host (A1) + pinned async copies around su3_convert/su3_mul/su3_mul3/su3_mul_add/su3_copy",
+            "api": "su3_mul_host (A1) + pinned async copies on H2D/D2H side streams around su3_convert/su3_mul/su3_mul3/su3_mul_add/su3_copy",
             "host_result_matches_device": ok}
 
 
