@@ -87,7 +87,7 @@ typedef struct {
   int32_t stages;       /* shared-memory ring depth, 2..16                             */
   int32_t ctas_per_sm;  /* persistent CTAs per SM, 1..8                                 */
   int32_t l2_hint;      /* 0 auto (by footprint), 1 none, 2 evict_first loads+stores   */
-  int32_t path;         /* 0 auto, 1 TMA-bulk staged pipeline, 2 direct per-lane LDG   */
+  int32_t path;         /* 0 auto (by footprint and layout), 1 TMA-bulk pipeline, 2 direct per-lane LDG, 3 warp-staged */
   int32_t reserved[3];
 } su3_tune;
 

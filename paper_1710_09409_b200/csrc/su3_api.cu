@@ -136,6 +136,26 @@ template <typename R, int OP> stream_kernel_t direct_for_w(int W) {
   }
   return nullptr;
 }
+template <typename R, int OP> stream_kernel_t warp_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_warp_kernel<R, 1, OP>;
+    case 2: return su3::su3_warp_kernel<R, 2, OP>;
+    case 4: return su3::su3_warp_kernel<R, 4, OP>;
+    case 8: return su3::su3_warp_kernel<R, 8, OP>;
+    case 16: return su3::su3_warp_kernel<R, 16, OP>;
+    case 32: return su3::su3_warp_kernel<R, 32, OP>;
+  }
+  return nullptr;
+}
+template <typename R> stream_kernel_t pick_warp(int op, int W) {
+  switch (op) {
+    case su3::OP_MUL: return warp_for_w<R, su3::OP_MUL>(W);
+    case su3::OP_MUL3: return warp_for_w<R, su3::OP_MUL3>(W);
+    case su3::OP_MUL_ADD: return warp_for_w<R, su3::OP_MUL_ADD>(W);
+    case su3::OP_ADD: return warp_for_w<R, su3::OP_ADD>(1);
+  }
+  return nullptr;
+}
 template <typename R> stream_kernel_t pick(int op, int W, bool direct) {
   switch (op) {
     case su3::OP_MUL: return direct ? direct_for_w<R, su3::OP_MUL>(W) : pipe_for_w<R, su3::OP_MUL>(W);
@@ -175,8 +195,14 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   }
   const int nin = (op == su3::OP_MUL || op == su3::OP_ADD) ? 2 : 3;
   const int cb = 2 * prec;
-  const bool direct = tn.path == 2;
-  stream_kernel_t k = (prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct);
+  // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
+  // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
+  // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
+  const bool direct = tn.path == 2 || (tn.path == 0 && op != su3::OP_ADD && W * cb >= 32 &&
+                                       footprint_bytes <= (size_t)di.l2 / 2);
+  const bool warp = !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
+  stream_kernel_t k = warp ? ((prec == SU3_F64) ? pick_warp<double>(op, W) : pick_warp<float>(op, W))
+                           : ((prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct));
   if (!k) return fail(SU3_ERR_INVALID, "no kernel for op %d prec %d W %d", op, prec, W);
 
   su3::StreamParams p;
@@ -185,12 +211,25 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   if (hint == 0) hint = (footprint_bytes > (size_t)di.l2) ? 1 : 1;  // auto: no hint (measured: DESIGN.md section 6)
   p.hint = (hint == 2) ? 1 : 0;
 
-  if (direct) {
+  if (warp) {
+    p.tile_mats = 32; p.stages = 0;
+    const int64_t nwt = (nmat + 31) / 32;
+    int wpb = 4;  // warps per block; fewer on small lattices so that every SM gets a block
+    while (wpb > 1 && (nwt + wpb - 1) / wpb < 2 * (int64_t)di.sms) wpb >>= 1;
+    const size_t smem = (size_t)wpb * nin * 288 * cb;
+    cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
+    if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
+    const int64_t blocks_needed = (nwt + wpb - 1) / wpb;
+    const int64_t cap = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 8) * (4 / wpb);
+    k<<<(unsigned)(blocks_needed < cap ? blocks_needed : cap), wpb * 32, smem, stream>>>(p);
+  } else if (direct) {
     p.tile_mats = 0; p.stages = 0;
-    const int64_t blocks_needed = (nmat + 255) / 256;
-    const int64_t cap = (int64_t)di.sms * 8 * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 1);
+    int bs = 256;  // small lattices: smaller blocks so that every SM gets one
+    while (bs > 32 && (nmat + bs - 1) / bs < 2 * (int64_t)di.sms) bs >>= 1;
+    const int64_t blocks_needed = (nmat + bs - 1) / bs;
+    const int64_t cap = (int64_t)di.sms * 8 * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 1) * (256 / bs);
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    k<<<grid, 256, 0, stream>>>(p);
+    k<<<grid, bs, 0, stream>>>(p);
   } else {
     // defaults measured on B200: 9 KB operand slots (64 fp64 / 128 fp32 matrices),
     // a 3-deep ring, 2 persistent CTAs per SM
@@ -542,7 +581,7 @@ su3_status su3_tune_set(const su3_tune *t) {
   if (v.stages != 0 && (v.stages < 2 || v.stages > 16)) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16", v.stages);
   if (v.ctas_per_sm < 0 || v.ctas_per_sm > 8) return fail(SU3_ERR_INVALID, "ctas_per_sm = %d outside 0..8", v.ctas_per_sm);
   if (v.l2_hint < 0 || v.l2_hint > 2) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..2", v.l2_hint);
-  if (v.path < 0 || v.path > 2) return fail(SU3_ERR_INVALID, "path = %d outside 0..2", v.path);
+  if (v.path < 0 || v.path > 3) return fail(SU3_ERR_INVALID, "path = %d outside 0..3", v.path);
   std::lock_guard<std::mutex> lk(g_tune_mu);
   g_tune = v;
   return SU3_OK;

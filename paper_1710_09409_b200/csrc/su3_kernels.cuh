@@ -353,6 +353,81 @@ __global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
   }
 }
 
+// ---------------------------------------------------------------- warp-staged path (path = 3)
+// For L2-resident lattices the pipeline's fixed latency (mbarrier set-up, TMA in, TMA out) is what one
+// measures.  Here every warp stages its own 32 matrices with coalesced per-lane loads of one complex
+// number each (lane i of request j reads complex j*32+i of the warp's contiguous 32*9-complex range),
+// multiplies out of shared memory exactly like the pipeline's consumers, and stores the same way.
+// Only __syncwarp() is needed; any layout (W | 32) works through the same shared-memory index.
+template <typename R, int W, int OP>
+__global__ void __launch_bounds__(128) su3_warp_kernel(const StreamParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int NIN = NumInputs<OP>::value;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  C2 *sw = reinterpret_cast<C2 *>(smem) + (size_t)wib * NIN * 288;
+  const long long nwt = (p.nmat + 31) / 32;
+  const int base = (lane / W) * 9 * W + (lane % W);
+  const C2 *src[3] = {reinterpret_cast<const C2 *>(p.x), reinterpret_cast<const C2 *>(p.y),
+                      reinterpret_cast<const C2 *>(p.u)};
+  C2 *gz = reinterpret_cast<C2 *>(p.z);
+  for (long long wt = (long long)blockIdx.x * wpb + wib; wt < nwt; wt += (long long)gridDim.x * wpb) {
+    const long long c0 = wt * 288;
+    const long long left = p.nmat - wt * 32;
+    const int nm = left < 32 ? (int)left : 32;
+    const int nc = nm * 9;
+    C2 r[NIN][9];
+#pragma unroll
+    for (int o = 0; o < NIN; o++)
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) r[o][j] = src[o][c0 + j * 32 + lane];
+#pragma unroll
+    for (int o = 0; o < NIN; o++)
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) sw[o * 288 + j * 32 + lane] = r[o][j];
+    __syncwarp();
+    if (lane < nm) {
+      C2 a[9], b[9], c[9];
+#pragma unroll
+      for (int e = 0; e < 9; e++) a[e] = sw[base + e * W];
+#pragma unroll
+      for (int e = 0; e < 9; e++) b[e] = sw[288 + base + e * W];
+      if (OP == OP_ADD) {
+#pragma unroll
+        for (int e = 0; e < 9; e++) {
+          c[e].x = add_rn(a[e].x, b[e].x);
+          c[e].y = add_rn(a[e].y, b[e].y);
+        }
+      } else {
+        mat33_mul(a, b, c);
+      }
+      if (OP == OP_MUL3) {
+#pragma unroll
+        for (int e = 0; e < 9; e++) b[e] = sw[2 * 288 + base + e * W];
+        mat33_mul(c, b, a);
+#pragma unroll
+        for (int e = 0; e < 9; e++) c[e] = a[e];
+      } else if (OP == OP_MUL_ADD) {
+#pragma unroll
+        for (int e = 0; e < 9; e++) {
+          C2 v = sw[2 * 288 + base + e * W];
+          c[e].x = add_rn(c[e].x, v.x);
+          c[e].y = add_rn(c[e].y, v.y);
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < 9; e++) sw[base + e * W] = c[e];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < 9; j++)
+      if (j * 32 + lane < nc) gz[c0 + j * 32 + lane] = sw[j * 32 + lane];
+    __syncwarp();
+  }
+}
+
 // ---------------------------------------------------------------- streaming ceilings (A6) and z = x + y
 // dst = src as a pure TMA pipeline: one thread per CTA moves tiles global -> shared -> global with
 // 1-D bulk copies through a ring of `stages` slots; no register ever holds data.  The ceiling the

@@ -51,7 +51,7 @@ ALL_W = [(SC, 1), (VE, 1), (VE, 2), (VE, 4), (VE, 8), (VE, 16), (VE, 32)]
 
 
 # ------------------------------------------------------------------ exact integer case (bit-equal)
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
 @pytest.mark.parametrize("prec", [F64, F32])
 @pytest.mark.parametrize("layout,W", ALL_W)
 def test_integer_case_bit_exact(prec, layout, W, path):
@@ -109,7 +109,7 @@ def test_config2_16x4_both_layouts_and_roundtrip():
 
 
 # ------------------------------------------------------------------ every W, ragged sizes, Lorentz index
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
 @pytest.mark.parametrize("prec", [F64, F32])
 @pytest.mark.parametrize("layout,W", ALL_W)
 def test_all_ops_every_W(prec, layout, W, path):
