@@ -199,7 +199,7 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
   // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
   const bool direct = tn.path == 2 || (tn.path == 0 && op != su3::OP_ADD && W * cb >= 32 &&
-                                       footprint_bytes <= (size_t)di.l2 / 2);
+                                       footprint_bytes <= (size_t)di.l2 / 5 * 3);
   const bool warp = !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
   stream_kernel_t k = warp ? ((prec == SU3_F64) ? pick_warp<double>(op, W) : pick_warp<float>(op, W))
                            : ((prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct));
