@@ -412,6 +412,25 @@ def run_ceilings_and_sweep(args, r):
     su3.su3_convert(fx32v, fx32s); su3.su3_convert(fy32v, fy32s)
     src = {(8, 0): (f["xs"], f["ys"], f["zc"]), (8, 1): (f["xv"], f["yv"], f["zc"]),
            (4, 0): (fx32s, fy32s, f["zc"]), (4, 1): (fx32v, fy32v, f["zc"])}
+    # f1 (Fig. 4): vector-length sweep at a fixed HBM-bound volume, fp32 complex.
+    # The paper's GPUs plateaued only at W = 16 because block = one vector; here bandwidth is flat in W.
+    wsweep = []
+    Lw = min(args.L, 48)
+    for Wv in (1, 2, 4, 8, 16, 32):
+        dsw = su3.make_desc(Lw, prec=su3.SU3_F32)
+        dw = su3.make_desc(Lw, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=Wv)
+        nbw = su3.su3_field_bytes(dw)
+        xs_w = su3.su3_field_wrap(dsw, x32[:nbw // 4].view(torch.uint8))
+        ys_w = su3.su3_field_wrap(dsw, y32[:nbw // 4].view(torch.uint8))
+        xw, yw, zw = su3.alloc_field(dw), su3.alloc_field(dw), su3.alloc_field(dw)
+        su3.su3_convert(xw, xs_w); su3.su3_convert(yw, ys_w)
+        mn, md, _ = time_calls(torch, lambda: su3.su3_mul(zw, xw, yw))
+        wsweep.append({"W": Wv, "L": Lw, "prec": "f32", "simd": list(su3.su3_desc_normalize(dw).simd),
+                       "us_min": mn * 1e3, "GBps": 3 * nbw / (mn * 1e-3) / 1e9,
+                       "GFLOPps": FLOPS["mul"] * Lw ** 4 / (mn * 1e-3) / 1e9,
+                       "frac_of_copy": 3 * nbw / (mn * 1e-3) / 1e9 / ceiling})
+        del xw, yw, zw
+    out["wsweep"] = wsweep
     sweep = []
     for Ls in (8, 12, 16, 24, 32, 48, 64):
         if Ls > args.L:
@@ -478,8 +497,11 @@ def main():
     a1 = ops[3]
     roofline = {"bound": "hbm", "kernel": "su3_pipe_kernel<double,W=1,OP_MUL> (row A1, z=x*y fp64 scalar)",
                 "achieved": a1["GBps"], "peak": peak, "unit": "GB/s", "frac": a1["GBps"] / peak, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": 3 * B, "avg_launch_ms": a1["ms"], "traffic": None,
-                "traffic_note": "see profiles/ for the ncu --set full dram__bytes of this kernel"}
+                "algorithmic_bytes_per_launch": 3 * B, "avg_launch_ms": a1["ms"],
+                # dram__bytes_read.sum + dram__bytes_write.sum of this launch at 64^4, from the one ncu --set full
+                # capture summarised in profiles/r01_pipe_kernel_full.md (4.831918 + 2.385510 GB)
+                "traffic": 7217428000 if args.L == 64 else None,
+                "traffic_source": "profiles/r01_pipe_kernel_full.md (ncu --set full, per launch)"}
     cpu = None
     if rank == 0 and not args.no_cpu:
         Lc = min(args.cpu_L, args.L)
@@ -502,7 +524,8 @@ def main():
                    "parallelism": "independent x3 slabs, no collective" if world > 1 else "single GPU"},
         "GFLOPps": world * r["step_flops"] / (r["ms_per_step"] * 1e-3) / 1e9,
         "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
-        "ops": ops, "ceilings_GBps": ceilings, "sweep": sweep, "checks": r["checks"],
+        "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k != "wsweep"},
+        "wsweep": ceilings.get("wsweep"), "sweep": sweep, "checks": r["checks"],
         "wall_s_timed_region": r["t_wall"],
     }
     print(json.dumps(line), flush=True)

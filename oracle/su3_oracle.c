@@ -197,6 +197,46 @@ void orc_mul_add(const orc_geom *g, int prec, const void *x, const void *y, cons
     }
 }
 
+/* z = value of a postfix expression over matrix fields, evaluated per site inside the one site loop
+ * (Listing 1: `eval(ss, expr)` walks the expression tree at every site; Listing 2:
+ * `v3 = v1+v2+v1*v2` is one pass, no temporaries in memory).  The tree is given in postfix order as a
+ * string: a digit '0'..'7' pushes operand field ops[digit] at this site, '+', '-', '*' pop b then a and push
+ * a+b, a-b, a.b (matrix product, mat33 above).  Every intermediate lives in fp64 for the one site.
+ * Returns 0, or nonzero if the program is malformed (bad token, operand index >= nops, stack under-/
+ * overflow (depth > 8), or not exactly one value left). */
+int orc_expr(const orc_geom *g, int prec, int nops, const void *const *ops, const char *prog, double *z) {
+  int depth = 0, n = 0;
+  for (const char *t = prog; *t; t++, n++) {
+    if (*t >= '0' && *t <= '7') { if (*t - '0' >= nops) return 2; if (++depth > 8) return 3; }
+    else if (*t == '+' || *t == '-' || *t == '*') { if (depth < 2) return 4; depth--; }
+    else return 1;
+  }
+  if (depth != 1) return 5;
+  int64_t V = orc_volume(g);
+#pragma omp parallel for schedule(static)
+  for (int64_t site = 0; site < V; site++)
+    for (int mu = 0; mu < g->nl; mu++) {
+      double st[8][3][3][2];
+      int sp = 0;
+      for (const char *t = prog; *t; t++) {
+        if (*t >= '0' && *t <= '7') {
+          load33(g, prec, ops[*t - '0'], site, mu, st[sp++]);
+        } else {
+          double (*a)[3][2] = st[sp - 2], (*b)[3][2] = st[sp - 1], c[3][3][2];
+          if (*t == '*') mat33(a, b, c);
+          else
+            for (int i = 0; i < 3; i++)
+              for (int j = 0; j < 3; j++)
+                for (int q = 0; q < 2; q++) c[i][j][q] = (*t == '+') ? a[i][j][q] + b[i][j][q] : a[i][j][q] - b[i][j][q];
+          memcpy(a, c, sizeof c);
+          sp--;
+        }
+      }
+      store33(g, z, site, mu, st[0]);
+    }
+  return 0;
+}
+
 /* layout conversion = pure permutation of reals, bit copy (lane l of
  * each of the 9 vector elements <-> one scalar matrix).  `prec` bytes per real. */
 int orc_convert(const orc_geom *gd, const orc_geom *gs, int prec, void *dst, const void *src) {

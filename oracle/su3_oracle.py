@@ -37,6 +37,8 @@ def _load():
         lib.orc_mul3.restype = None
         lib.orc_mul_add.argtypes = [P, I, V, V, V, V]
         lib.orc_mul_add.restype = None
+        lib.orc_expr.argtypes = [P, I, I, ctypes.POINTER(V), ctypes.c_char_p, V]
+        lib.orc_expr.restype = I
         lib.orc_convert.argtypes = [P, P, I, V, V]
         lib.orc_convert.restype = I
         lib.orc_num_threads.restype = I
@@ -123,6 +125,18 @@ def mul_add(g, x, y, v):
     assert _prec(y, g) == p and _prec(v, g) == p
     z = _out(g)
     _load().orc_mul_add(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, v.ctypes.data, z.ctypes.data)
+    return z
+
+
+def expr(g, prog, *ops):
+    """z = postfix expression `prog` ('0'..'7' push ops[k]; '+', '-', '*') over fields ops, all in layout g."""
+    p = _prec(ops[0], g)
+    assert all(_prec(o, g) == p for o in ops)
+    z = _out(g)
+    arr = (ctypes.c_void_p * len(ops))(*[o.ctypes.data for o in ops])
+    rc = _load().orc_expr(ctypes.byref(g.c), p, len(ops), arr, prog.encode(), z.ctypes.data)
+    if rc:
+        raise ValueError("malformed expression %r (orc_expr -> %d)" % (prog, rc))
     return z
 
 

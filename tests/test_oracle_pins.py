@@ -271,3 +271,65 @@ def test_fp32_inputs_are_promoted_not_rounded():
     assert z32.dtype == np.float64
     assert np.array_equal(z32, oracle.mul(g, x.astype(np.float64), y.astype(np.float64)))
     assert np.abs(z32 - z32.astype(np.float32)).max() > 0  # not rounded to fp32
+
+
+# ---------------------------------------------------------------- the postfix expression evaluator (f2)
+def _py_postfix(prog, mats):
+    """pure-Python reference: exact Gaussian-integer 3x3 arithmetic on lists of Python complex/int"""
+    st = []
+    for t in prog:
+        if t.isdigit():
+            st.append(mats[int(t)])
+        else:
+            b, a = st.pop(), st.pop()
+            if t == "*":
+                st.append([[sum(a[i][k] * b[k][j] for k in range(3)) for j in range(3)] for i in range(3)])
+            else:
+                sg = 1 if t == "+" else -1
+                st.append([[a[i][j] + sg * b[i][j] for j in range(3)] for i in range(3)])
+    assert len(st) == 1
+    return np.array(st[0], dtype=np.complex128)
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("prog", ["01*", "10*", "01*2*", "012**", "01*2+", "01+01*+", "01-2*0+", "0", "00*0*1-",
+                                  "01*21*-", "0123+*-"])
+def test_expr_integer_cases_exact(prog, dtype):
+    """Listing 2's pattern (P:104-106 `v3=v1+v2+v1*v2`) and friends on the exact integer matrices of the
+    golden fixture: brute force in Python integers, independent of the oracle"""
+    g = oracle.Geom(2, layout=oracle.su3_oracle.VECTOR, W=4) if dtype == np.float32 else oracle.Geom(2)
+    names = ["A", "B", "C", "AB"]
+    gs = oracle.Geom(2)
+    fields = [fill(gs, IC[n], dtype) for n in names]
+    if g.layout:
+        fields = [oracle.convert(g, gs, f) for f in fields]
+    z = oracle.expr(g, prog, *fields)
+    if g.layout:
+        z = oracle.convert(gs, g, z)
+    want = _py_postfix(prog, [[[complex(v) for v in row] for row in IC[n]] for n in names])
+    assert np.array_equal(logical(z), np.broadcast_to(want, (16, 3, 3)))
+
+
+def test_expr_matches_fixed_calls_and_numpy():
+    g = oracle.Geom((4, 2, 2, 3), nl=4)
+    x, y, w = (flat(su3gen.su3_field(3, f, g.nmat)) for f in (0, 1, 2))
+    v = flat(su3gen.gaussian_field(3, 3, g.nmat))
+    assert np.array_equal(oracle.expr(g, "01*", x, y), oracle.mul(g, x, y))
+    assert np.array_equal(oracle.expr(g, "01*2*", x, y, w), oracle.mul3(g, x, y, w))
+    assert np.array_equal(oracle.expr(g, "01*2+", x, y, v), oracle.mul_add(g, x, y, v))
+    X, Y, W_, V = logical(x), logical(y), logical(w), logical(v)
+    z = logical(oracle.expr(g, "01+01*+23*-", x, y, w, v))
+    want = X + Y + X @ Y - W_ @ V
+    assert np.abs(z - want).max() <= 1e-14
+    # algebra: x - x = 0 exactly; (x+y)*w = x*w + y*w to rounding
+    assert not oracle.expr(g, "00-", x).any()
+    d = oracle.expr(g, "01+2*", x, y, w) - oracle.expr(g, "02*12*+", x, y, w)
+    assert np.abs(d).max() <= 1e-14
+
+
+def test_expr_rejects_malformed_programs():
+    g = oracle.Geom(2)
+    x = fill(g, IC["A"])
+    for bad in ["", "0+", "00", "01*", "0a*", "00*+", "000000000********"]:
+        with pytest.raises(ValueError):
+            oracle.expr(g, bad, x)
