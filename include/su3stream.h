@@ -130,6 +130,22 @@ su3_status su3_mul_add(su3_field *z, const su3_field *x, const su3_field *y, con
  * reference (the analogue of the paper's STREAM line). */
 su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *cuda_stream);
 
+/* z = value of a small expression tree over matrix fields, evaluated site by site in ONE pass, intermediates
+ * in registers / shared memory only (Listings 1-2: `eval(ss, expr)` inside the site loop, e.g.
+ * `v3 = v1+v2+v1*v2`).  `program` is the tree in postfix order as a NUL-terminated string: a digit '0'..'7'
+ * pushes operands[digit] at this site; '+', '-', '*' pop b, then a, and push a+b, a-b, a.b (3x3 complex
+ * product).  Examples: "01*" = su3_mul, "01*2*" = su3_mul3, "01*2+" = su3_mul_add (bit-identical to them),
+ * "01+01*+" = v1+v2+v1*v2.  At most 32 tokens, 16 operators, stack depth 8; every operand 0..n_operands-1
+ * must be used; exactly one value must remain (SU3_ERR_INVALID otherwise).  All fields must have identical
+ * descriptors (SU3_ERR_MISMATCH); z may be the same field as any operand.  Every distinct operand adds one
+ * read stream: bytes = (n_operands + 1) * field bytes. */
+su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *operands, int n_operands,
+                    void *cuda_stream);
+
+/* Accounting of a program by reading S9: field streams (n_operands + 1) and flops per matrix (198 per '*',
+ * 18 per '+' or '-').  Validates the program like su3_expr.  Host-only. */
+su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix);
+
 /* Layout conversion scalar <-> vector: a pure, bit-exact permutation of complex numbers,
  * vec[o][mu][e][l] = sca[site(o,l)][mu][e] (extract/merge).  Exactly one of
  * dst/src must be SU3_SCALAR and the other SU3_VECTOR; L, n_lorentz, prec must agree

@@ -294,6 +294,82 @@ unsigned flat_grid(size_t n_items, size_t per_block, int blocks_per_sm) {
   return (unsigned)(need < cap ? need : cap);
 }
 
+// ---------------------------------------------------------------- su3_expr: postfix -> register machine
+struct ExprProgram {
+  su3::ExprIns ins[16];
+  int nins = 0, ntemp = 0, nmul = 0, naddsub = 0;
+};
+
+// Simulates the evaluation stack.  A stack entry is an operand slot (0..7), a temporary (8..15) or the
+// accumulator (255); at most one entry lives in the accumulator: it is spilled to a temporary when a new
+// result is produced while it is still needed.
+su3_status compile_expr(const char *prog, int nops, ExprProgram *out) {
+  if (!prog) return fail(SU3_ERR_NULL, "program is NULL");
+  if (nops < 1 || nops > 8) return fail(SU3_ERR_INVALID, "n_operands = %d outside 1..8", nops);
+  const size_t len = strlen(prog);
+  if (len == 0 || len > 32) return fail(SU3_ERR_INVALID, "program has %zu tokens (1..32 allowed)", len);
+  unsigned char stack[8];
+  int sp = 0;
+  bool used[8] = {false}, temp_busy[8] = {false};
+  ExprProgram pr;
+  for (size_t i = 0; i < len; i++) {
+    const char t = prog[i];
+    if (t >= '0' && t <= '7') {
+      if (t - '0' >= nops) return fail(SU3_ERR_INVALID, "token %zu: operand %c but n_operands = %d", i, t, nops);
+      if (sp == 8) return fail(SU3_ERR_INVALID, "token %zu: stack deeper than 8", i);
+      used[t - '0'] = true;
+      stack[sp++] = (unsigned char)(t - '0');
+    } else if (t == '+' || t == '-' || t == '*') {
+      if (sp < 2) return fail(SU3_ERR_INVALID, "token %zu: operator '%c' needs two values", i, t);
+      if (pr.nins == 16) return fail(SU3_ERR_INVALID, "more than 16 operators");
+      const unsigned char b = stack[--sp], a = stack[--sp];
+      su3::ExprIns in;
+      in.op = t == '*' ? su3::EX_MUL : (t == '+' ? su3::EX_ADD : su3::EX_SUB);
+      in.a = a; in.b = b; in.spill = su3::EX_NONE;
+      for (int k = 0; k < sp; k++)
+        if (stack[k] == su3::EX_SRC_ACC) {  // an older result is still needed: park it in a temporary
+          int tmp = 0;
+          while (tmp < 8 && temp_busy[tmp]) tmp++;
+          if (tmp == 8) return fail(SU3_ERR_INVALID, "expression needs more than 8 temporaries");
+          temp_busy[tmp] = true;
+          if (tmp + 1 > pr.ntemp) pr.ntemp = tmp + 1;
+          in.spill = (unsigned char)(su3::EX_TEMP0 + tmp);
+          stack[k] = in.spill;
+        }
+      if (a >= su3::EX_TEMP0 && a != su3::EX_SRC_ACC) temp_busy[a - su3::EX_TEMP0] = false;
+      if (b >= su3::EX_TEMP0 && b != su3::EX_SRC_ACC) temp_busy[b - su3::EX_TEMP0] = false;
+      (t == '*' ? pr.nmul : pr.naddsub)++;
+      pr.ins[pr.nins++] = in;
+      stack[sp++] = su3::EX_SRC_ACC;
+    } else {
+      return fail(SU3_ERR_INVALID, "token %zu: '%c' is not a digit 0..7 or one of + - *", i, t);
+    }
+  }
+  if (sp != 1) return fail(SU3_ERR_INVALID, "program leaves %d values on the stack (must be 1)", sp);
+  for (int k = 0; k < nops; k++)
+    if (!used[k]) return fail(SU3_ERR_INVALID, "operand %d is never used", k);
+  if (stack[0] != su3::EX_SRC_ACC) {  // the program is a bare operand: z = operand
+    su3::ExprIns in;
+    in.op = su3::EX_COPY; in.a = stack[0]; in.b = su3::EX_NONE; in.spill = su3::EX_NONE;
+    pr.ins[pr.nins++] = in;
+  }
+  *out = pr;
+  return SU3_OK;
+}
+
+typedef void (*expr_kernel_t)(const su3::ExprParams);
+template <typename R> expr_kernel_t expr_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_expr_kernel<R, 1, NCW>;
+    case 2: return su3::su3_expr_kernel<R, 2, NCW>;
+    case 4: return su3::su3_expr_kernel<R, 4, NCW>;
+    case 8: return su3::su3_expr_kernel<R, 8, NCW>;
+    case 16: return su3::su3_expr_kernel<R, 16, NCW>;
+    case 32: return su3::su3_expr_kernel<R, 32, NCW>;
+  }
+  return nullptr;
+}
+
 // ---------------------------------------------------------------- su3_mul_host resources
 struct HostPipe {
   std::mutex mu;
@@ -397,6 +473,68 @@ su3_status su3_mul3(su3_field *z, const su3_field *x, const su3_field *y, const 
 }
 su3_status su3_mul_add(su3_field *z, const su3_field *x, const su3_field *y, const su3_field *v, void *s) {
   return arith(su3::OP_MUL_ADD, z, x, y, v, s);
+}
+
+su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix) {
+  ExprProgram pr;
+  su3_status st = compile_expr(program, n_operands, &pr);
+  if (st != SU3_OK) return st;
+  if (streams) *streams = n_operands + 1;
+  if (flops_per_matrix) *flops_per_matrix = 198 * pr.nmul + 18 * pr.naddsub;
+  return SU3_OK;
+}
+
+su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *operands, int n_operands,
+                    void *cuda_stream) {
+  if (!z || !operands) return fail(SU3_ERR_NULL, "NULL argument");
+  ExprProgram pr;
+  su3_status st = compile_expr(program, n_operands, &pr);
+  if (st != SU3_OK) return st;
+  for (int k = 0; k < n_operands; k++) {
+    if (!operands[k]) return fail(SU3_ERR_NULL, "operand %d is NULL", k);
+    if (!same_desc(z->d, operands[k]->d)) return fail(SU3_ERR_MISMATCH, "operand %d: descriptor differs from z", k);
+  }
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (z->nmat == 0) return SU3_OK;
+  su3_tune tn;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    tn = g_tune;
+  }
+  const int cb = 2 * z->d.prec;
+  expr_kernel_t k = z->d.prec == SU3_F64 ? expr_for_w<double>(z->d.W) : expr_for_w<float>(z->d.W);
+  if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", z->d.W);
+  int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
+  int tm = tn.tile_mats > 0 ? tn.tile_mats : 9216 / (9 * cb);
+  while (tn.tile_mats == 0 && tm > 32 && (z->nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
+  int stages = tn.stages > 0 ? tn.stages : 3;
+  size_t smem = 0;
+  for (;;) {  // shrink ring, then CTAs/SM, then the tile until the operand slots and temporaries fit
+    const size_t slot = (size_t)tm * 9 * cb;
+    smem = ((size_t)stages * n_operands + pr.ntemp) * slot + 2 * stages * sizeof(uint64_t);
+    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    if (smem + 256 <= budget) break;
+    if (tn.stages == 0 && stages > 2) stages--;
+    else if (tn.ctas_per_sm == 0 && ctas > 1) ctas--;
+    else if (tn.tile_mats == 0 && tm > 32) tm >>= 1;
+    else return fail(SU3_ERR_INVALID, "expression needs %zu B of shared memory (tile %d, %d stages, %d operands, %d temporaries)",
+                     smem, tm, stages, n_operands, pr.ntemp);
+  }
+  cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
+  if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
+  su3::ExprParams p;
+  memset(&p, 0, sizeof p);
+  p.z = z->ptr;
+  for (int i = 0; i < n_operands; i++) p.ops[i] = operands[i]->ptr;
+  p.nmat = z->nmat; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp;
+  for (int i = 0; i < pr.nins; i++) p.ins[i] = pr.ins[i];
+  const int64_t ntiles = (z->nmat + tm - 1) / tm, max_grid = (int64_t)di.sms * ctas;
+  k<<<(unsigned)(ntiles < max_grid ? ntiles : max_grid), (NCW + 1) * 32, smem, (cudaStream_t)cuda_stream>>>(p);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_expr launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
 }
 
 su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *stream) {

@@ -353,6 +353,163 @@ __global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
   }
 }
 
+// ---------------------------------------------------------------- general one-pass expression (f2)
+// z = value of a small expression tree over matrix fields, evaluated per site in ONE pass (P:76-109,
+// Listings 1-2: `eval(ss, expr)` inside the site loop; every extra operand adds one read stream, no
+// intermediate ever goes to memory).  The host compiles the postfix program into at most 16 register-
+// machine instructions (su3_api.cu): each takes its two sources from an operand slot of the stage, a
+// thread-private temporary in shared memory, or the accumulator registers, and leaves its result in the
+// accumulator.  The program is uniform over the grid, so the interpreter's branches never diverge.
+// Same pipeline as su3_pipe_kernel (TMA bulk in, TMA bulk out), same mat33_mul, hence bit-identical
+// to su3_mul / su3_mul3 / su3_mul_add on their three programs.
+enum { EX_MUL = 0, EX_ADD = 1, EX_SUB = 2, EX_COPY = 3, EX_SRC_ACC = 255, EX_NONE = 255, EX_TEMP0 = 8 };
+struct ExprIns {
+  unsigned char op, a, b, spill;  // sources: 0..7 operand slot, 8..15 temporary, 255 accumulator
+};
+struct ExprParams {
+  void *z;
+  const void *ops[8];
+  long long nmat;
+  int tile_mats, stages, nops, nins, ntemp, hint;
+  ExprIns ins[16];
+};
+
+template <typename R, int W, int NCW>
+__global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int CB = (int)sizeof(C2);
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int TM = p.tile_mats, S = p.stages, NIN = p.nops;
+  const uint32_t slot_bytes = (uint32_t)TM * 9u * CB;
+  const uint32_t stage_bytes = NIN * slot_bytes;
+  unsigned char *temps = smem + (size_t)S * stage_bytes;
+  uint64_t *full = reinterpret_cast<uint64_t *>(temps + (size_t)p.ntemp * slot_bytes);
+  uint64_t *empty = full + S;
+  const int tid = threadIdx.x;
+  const long long ntiles = (p.nmat + TM - 1) / TM;
+  if (tid == 0) {
+    for (int s = 0; s < S; s++) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], 1);
+    }
+    fence_mbar_init();
+    fence_proxy_async();
+  }
+  __syncthreads();
+
+  if (tid >= NCW * 32) {
+    if (tid == NCW * 32) {
+      int s = 0;
+      uint32_t ph = 0;
+      for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(&empty[s], ph ^ 1u);
+        const long long m0 = tile * TM;
+        const long long left = p.nmat - m0;
+        const int nm = left < TM ? (int)left : TM;
+        const uint32_t bytes = (uint32_t)nm * 9u * CB;
+        const uint32_t b16 = bytes & ~15u;
+        unsigned char *st = smem + (size_t)s * stage_bytes;
+        const size_t goff = (size_t)m0 * 9u * CB;
+        if (bytes != b16)
+          for (int o = 0; o < NIN; o++)
+            *reinterpret_cast<uint64_t *>(st + o * slot_bytes + b16) =
+                *reinterpret_cast<const uint64_t *>((const unsigned char *)p.ops[o] + goff + b16);
+        mbar_arrive_expect_tx(&full[s], NIN * b16);
+        for (int o = 0; o < NIN; o++)
+          bulk_g2s(st + o * slot_bytes, (const unsigned char *)p.ops[o] + goff, b16, &full[s]);
+        if (++s == S) {
+          s = 0;
+          ph ^= 1u;
+        }
+      }
+    }
+    return;
+  }
+
+  const int t = tid;
+  const int base = (t / W) * 9 * W + (t % W);
+  int s = 0, prev_s = -1;
+  uint32_t ph = 0;
+  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const long long m0 = tile * TM;
+    const long long left = p.nmat - m0;
+    const int nm = left < TM ? (int)left : TM;
+    unsigned char *st = smem + (size_t)s * stage_bytes;
+    mbar_wait(&full[s], ph);
+    if (t < nm) {
+      C2 acc[9], a[9], b[9];
+#pragma unroll 1
+      for (int i = 0; i < p.nins; i++) {
+        const ExprIns in = p.ins[i];
+        if (in.spill != EX_NONE) {
+          C2 *sp = reinterpret_cast<C2 *>(temps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + base;
+#pragma unroll
+          for (int e = 0; e < 9; e++) sp[e * W] = acc[e];
+        }
+        if (in.a == EX_SRC_ACC) {
+#pragma unroll
+          for (int e = 0; e < 9; e++) a[e] = acc[e];
+        } else {
+          const C2 *sa = reinterpret_cast<const C2 *>(in.a < EX_TEMP0 ? st + in.a * slot_bytes
+                                                                     : temps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + base;
+#pragma unroll
+          for (int e = 0; e < 9; e++) a[e] = sa[e * W];
+        }
+        if (in.op != EX_COPY) {
+          if (in.b == EX_SRC_ACC) {
+#pragma unroll
+            for (int e = 0; e < 9; e++) b[e] = acc[e];
+          } else {
+            const C2 *sb = reinterpret_cast<const C2 *>(in.b < EX_TEMP0 ? st + in.b * slot_bytes
+                                                                       : temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
+#pragma unroll
+            for (int e = 0; e < 9; e++) b[e] = sb[e * W];
+          }
+        }
+        if (in.op == EX_MUL) {
+          mat33_mul(a, b, acc);
+        } else if (in.op == EX_ADD) {
+#pragma unroll
+          for (int e = 0; e < 9; e++) {
+            acc[e].x = add_rn(a[e].x, b[e].x);
+            acc[e].y = add_rn(a[e].y, b[e].y);
+          }
+        } else if (in.op == EX_SUB) {
+#pragma unroll
+          for (int e = 0; e < 9; e++) {
+            acc[e].x = add_rn(a[e].x, -b[e].x);
+            acc[e].y = add_rn(a[e].y, -b[e].y);
+          }
+        } else {
+#pragma unroll
+          for (int e = 0; e < 9; e++) acc[e] = a[e];
+        }
+      }
+      C2 *so = reinterpret_cast<C2 *>(st) + base;  // result over operand slot 0: every read of this thread is done
+#pragma unroll
+      for (int e = 0; e < 9; e++) so[e * W] = acc[e];
+    }
+    fence_proxy_async();
+    named_bar_sync(1, NCW * 32);
+    if (t == 0) {
+      const uint32_t bytes = (uint32_t)nm * 9u * CB;
+      const uint32_t b16 = bytes & ~15u;
+      unsigned char *zdst = (unsigned char *)p.z + (size_t)m0 * 9u * CB;
+      bulk_s2g(zdst, st, b16);
+      bulk_commit();
+      if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(st + b16);
+      bulk_wait_read<1>();
+      if (prev_s >= 0) mbar_arrive(&empty[prev_s]);
+    }
+    prev_s = s;
+    if (++s == S) {
+      s = 0;
+      ph ^= 1u;
+    }
+  }
+  if (t == 0) bulk_wait_all<0>();
+}
+
 // ---------------------------------------------------------------- warp-staged path (path = 3)
 // For L2-resident lattices the pipeline's fixed latency (mbarrier set-up, TMA in, TMA out) is what one
 // measures.  Here every warp stages its own 32 matrices with coalesced per-lane loads of one complex

@@ -126,3 +126,17 @@ def test_no_cpu_fallback_without_a_gpu():
     assert su3.lib.su3_mul(h, h, h, None) == su3.SU3_ERR_CUDA  # fails loudly, computes nothing
     assert "CUDA" in su3.su3_last_error()
     su3.lib.su3_field_free(h)
+
+
+def test_expr_program_validation_and_cost():
+    """host-only: su3_expr_cost runs the same compiler as su3_expr (no launch)"""
+    assert su3.su3_expr_cost("01*", 2) == (3, 198)
+    assert su3.su3_expr_cost("01*2*", 3) == (4, 396)
+    assert su3.su3_expr_cost("01*2+", 3) == (4, 216)
+    assert su3.su3_expr_cost("01+01*+", 2) == (3, 198 + 36)
+    assert su3.su3_expr_cost("0", 1) == (2, 0)
+    for bad, n in [("", 1), ("0+", 1), ("00", 1), ("01*", 1), ("0a*", 1), ("00*+", 1), ("01*", 3), ("0" * 9 + "*" * 8, 1),
+                   ("00*" + "0*" * 16, 1), ("0", 0), ("0", 9)]:
+        with pytest.raises(su3.Su3Error) as e:
+            su3.su3_expr_cost(bad, n)
+        assert e.value.status == su3.SU3_ERR_INVALID, bad

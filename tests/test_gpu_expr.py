@@ -1,0 +1,102 @@
+"""-m gpu: the one-pass expression evaluator su3_expr (PAPER.md P:76-109,
+Listings 1-2) against the oracle's orc_expr, element by element; exact on integer inputs; bit-identical to
+the fixed calls on their three programs."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1710_09409_b200 as su3
+import su3gen
+from gpu_util import const_field, download, geom_of, host_field, upload
+from helpers import TOL, load_integer_case, rel_err
+
+pytestmark = pytest.mark.gpu
+IC = load_integer_case()
+F64, F32, SC, VE = su3.SU3_F64, su3.SU3_F32, su3.SU3_SCALAR, su3.SU3_VECTOR
+PROGS = ["01*", "10*", "01*2*", "012**", "01*2+", "01+01*+", "01-2*0+", "0", "00*0*1-", "01*21*-", "0123+*-",
+         "01*23*+", "01*23*45*++", "01234567*******", "01+2+3+", "01*23*-01+23+*-"]
+
+
+@pytest.fixture(autouse=True)
+def _defaults():
+    su3.su3_tune_set()
+    yield
+    su3.su3_tune_set()
+
+
+def nops(prog):
+    return max(int(c) for c in prog if c.isdigit()) + 1
+
+
+def run_expr(desc, prog, hosts):
+    fs = [upload(desc, h) for h in hosts]
+    z = su3.alloc_field(desc)
+    z.tensor.fill_(0xFF)
+    su3.su3_expr(z, prog, fs)
+    return download(z)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("layout,W", [(SC, 1), (VE, 4), (VE, 8), (VE, 32)])
+def test_expr_integer_inputs_bit_exact(prec, layout, W):
+    desc = su3.make_desc((4, 4, 4, 8), prec=prec, layout=layout, W=W)
+    k = np.arange(1, 4).reshape(-1, 1, 1)
+    mats = [IC["A"] * k, IC["B"], IC["C"], IC["A"] - IC["C"], IC["B"] + IC["C"], IC["C"], IC["A"], IC["B"]]
+    hosts = [const_field(desc, m) for m in mats]
+    for prog in PROGS:
+        if prog in ("01234567*******", "00*0*1-"):   # entries beyond 2^24 would not be exact in fp32
+            continue
+        n = nops(prog)
+        z = run_expr(desc, prog, hosts[:n])
+        assert np.array_equal(z.astype(np.float64), oracle.expr(geom_of(desc), prog, *hosts[:n])), prog
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", [((4, 6, 4, 8), 1, SC, 1), ((3, 3, 3, 3), 1, SC, 1), ((6, 2, 10, 2), 4, VE, 8),
+                                           ((8, 8, 8, 8), 1, VE, 4), ((2, 2, 2, 2), 4, VE, 16)])
+def test_expr_random_su3_against_oracle(prec, L, nl, layout, W):
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    hosts = [host_field(desc, 41, f, kind="su3" if f % 2 == 0 else "gauss") for f in range(8)]
+    Wn = su3.su3_desc_normalize(desc).W
+    for prog in PROGS:
+        n = nops(prog)
+        z = run_expr(desc, prog, hosts[:n])
+        err, _ = rel_err(z, oracle.expr(geom_of(desc), prog, *hosts[:n]), Wn)
+        # products of up to 8 unit-variance Gaussian matrices: a few more roundings than one product
+        assert np.isfinite(z).all() and err <= 4 * TOL[prec], (prog, err)
+
+
+def test_expr_is_bit_identical_to_the_fixed_calls_and_tuning_invariant():
+    for desc in (su3.make_desc((8, 8, 8, 6)), su3.make_desc((8, 8, 8, 6), prec=F32, layout=VE, W=8)):
+        x, y, w = (host_field(desc, 43, f) for f in (0, 1, 2))
+        v = host_field(desc, 43, 3, kind="gauss")
+        fx, fy, fw, fv, z = upload(desc, x), upload(desc, y), upload(desc, w), upload(desc, v), su3.alloc_field(desc)
+        su3.su3_tune_set(path=1)
+        su3.su3_mul(z, fx, fy)
+        assert np.array_equal(download(z), run_expr(desc, "01*", [x, y]))
+        su3.su3_mul3(z, fx, fy, fw)
+        ref3 = download(z)
+        assert np.array_equal(ref3, run_expr(desc, "01*2*", [x, y, w]))
+        su3.su3_mul_add(z, fx, fy, fv)
+        assert np.array_equal(download(z), run_expr(desc, "01*2+", [x, y, v]))
+        for tile, stages, ctas in [(32, 2, 1), (64, 4, 1), (32, 3, 3)]:
+            su3.su3_tune_set(tile_mats=tile, stages=stages, ctas_per_sm=ctas)
+            assert np.array_equal(ref3, run_expr(desc, "01*2*", [x, y, w]))
+        su3.su3_tune_set()
+        # z may alias an operand
+        su3.su3_expr(fx, "01*2*", [fx, fy, fw])
+        assert np.array_equal(download(fx), ref3)
+
+
+def test_expr_errors_launch_nothing():
+    desc = su3.make_desc(4)
+    a, b = su3.alloc_field(desc), su3.alloc_field(su3.make_desc(4, prec=F32))
+    n0 = su3.su3_launch_count()
+    with pytest.raises(su3.Su3Error) as e:
+        su3.su3_expr(a, "01*", [a, b])
+    assert e.value.status == su3.SU3_ERR_MISMATCH
+    with pytest.raises(su3.Su3Error) as e:
+        su3.su3_expr(a, "0+", [a])
+    assert e.value.status == su3.SU3_ERR_INVALID
+    assert su3.su3_launch_count() == n0
