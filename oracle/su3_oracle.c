@@ -254,6 +254,55 @@ int orc_convert(const orc_geom *gd, const orc_geom *gs, int prec, void *dst, con
   return 0;
 }
 
+/* Neighbour of `site` at displacement `disp` (any integer) along dimension `dim`, periodic:
+ * x[dim] -> (x[dim] + disp) mod L[dim], site order S2 (x0 fastest). */
+int64_t orc_neighbour(const orc_geom *g, int64_t site, int dim, int disp) {
+  int64_t stride = 1;
+  for (int d = 0; d < dim; d++) stride *= g->L[d];
+  int64_t xd = (site / stride) % g->L[dim];
+  int64_t nd = ((xd + disp) % g->L[dim] + g->L[dim]) % g->L[dim];
+  return site + (nd - xd) * stride;
+}
+
+/* Circular shift, Grid's `Cshift(x, dim, disp)` (named by the paper as the next obstacle):
+ * z[s] = x[s + disp*dim_hat] for every site s and every mu; a pure permutation of matrices, bit copy,
+ * `prec` bytes per real, any layout (in the vector layout a shift across a sub-lattice boundary moves
+ * a matrix to another lane -- here that is simply what the index function says). */
+int orc_cshift(const orc_geom *g, int prec, void *z, const void *x, int dim, int disp) {
+  if (dim < 0 || dim > 3) return 1;
+  int64_t V = orc_volume(g);
+#pragma omp parallel for schedule(static)
+  for (int64_t site = 0; site < V; site++) {
+    int64_t from = orc_neighbour(g, site, dim, disp);
+    for (int mu = 0; mu < g->nl; mu++)
+      for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++)
+          for (int c = 0; c < 2; c++)
+            memcpy((char *)z + prec * orc_index(g, site, mu, i, j, c),
+                   (const char *)x + prec * orc_index(g, from, mu, i, j, c), (size_t)prec);
+  }
+  return 0;
+}
+
+/* z[s] = x[s] . y[s + disp*dim_hat]: the site-local product with a shifted second operand, the building
+ * block of covariant shifts / plaquettes ("Cshift ... stencil operators").  fp64 result. */
+int orc_mul_shift(const orc_geom *g, int prec, const void *x, const void *y, int dim, int disp, double *z) {
+  if (dim < 0 || dim > 3) return 1;
+  int64_t V = orc_volume(g);
+#pragma omp parallel for schedule(static)
+  for (int64_t site = 0; site < V; site++) {
+    int64_t from = orc_neighbour(g, site, dim, disp);
+    for (int mu = 0; mu < g->nl; mu++) {
+      double a[3][3][2], b[3][3][2], c[3][3][2];
+      load33(g, prec, x, site, mu, a);
+      load33(g, prec, y, from, mu, b);
+      mat33(a, b, c);
+      store33(g, z, site, mu, c);
+    }
+  }
+  return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -39,6 +39,12 @@ def _load():
         lib.orc_mul_add.restype = None
         lib.orc_expr.argtypes = [P, I, I, ctypes.POINTER(V), ctypes.c_char_p, V]
         lib.orc_expr.restype = I
+        lib.orc_cshift.argtypes = [P, I, V, V, I, I]
+        lib.orc_cshift.restype = I
+        lib.orc_mul_shift.argtypes = [P, I, V, V, I, I, V]
+        lib.orc_mul_shift.restype = I
+        lib.orc_neighbour.argtypes = [P, I64, I, I]
+        lib.orc_neighbour.restype = I64
         lib.orc_convert.argtypes = [P, P, I, V, V]
         lib.orc_convert.restype = I
         lib.orc_num_threads.restype = I
@@ -137,6 +143,29 @@ def expr(g, prog, *ops):
     rc = _load().orc_expr(ctypes.byref(g.c), p, len(ops), arr, prog.encode(), z.ctypes.data)
     if rc:
         raise ValueError("malformed expression %r (orc_expr -> %d)" % (prog, rc))
+    return z
+
+
+def neighbour(g, site, dim, disp):
+    return int(_load().orc_neighbour(ctypes.byref(g.c), int(site), int(dim), int(disp)))
+
+
+def cshift(g, x, dim, disp):
+    """z[s] = x[s + disp*dim_hat] (Grid's Cshift), bit copy in x's precision, layout g."""
+    p = _prec(x, g)
+    z = np.empty_like(x)
+    if _load().orc_cshift(ctypes.byref(g.c), p, z.ctypes.data, x.ctypes.data, int(dim), int(disp)):
+        raise ValueError("dim %r outside 0..3" % (dim,))
+    return z
+
+
+def mul_shift(g, x, y, dim, disp):
+    """z[s] = x[s] * y[s + disp*dim_hat]; fp64 result."""
+    p = _prec(x, g)
+    assert _prec(y, g) == p
+    z = _out(g)
+    if _load().orc_mul_shift(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, int(dim), int(disp), z.ctypes.data):
+        raise ValueError("dim %r outside 0..3" % (dim,))
     return z
 
 

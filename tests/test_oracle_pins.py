@@ -333,3 +333,47 @@ def test_expr_rejects_malformed_programs():
     for bad in ["", "0+", "00", "01*", "0a*", "00*+", "000000000********"]:
         with pytest.raises(ValueError):
             oracle.expr(g, bad, x)
+
+
+# ---------------------------------------------------------------- Cshift and the shifted product (f3)
+def test_neighbour_spot_values_by_hand():
+    g = oracle.Geom((4, 2, 3, 2))  # strides 1, 4, 8, 24
+    assert oracle.neighbour(g, 0, 0, 1) == 1 and oracle.neighbour(g, 3, 0, 1) == 0      # wrap in x0
+    assert oracle.neighbour(g, 0, 0, -1) == 3 and oracle.neighbour(g, 5, 1, 1) == 1      # x=(1,1,..) -> (1,0,..)
+    assert oracle.neighbour(g, 5, 2, 1) == 13 and oracle.neighbour(g, 21, 2, 1) == 5     # x2: 2 -> 0 wraps
+    assert oracle.neighbour(g, 47, 3, 1) == 23 and oracle.neighbour(g, 47, 3, 2) == 47
+    assert oracle.neighbour(g, 7, 0, 9) == oracle.neighbour(g, 7, 0, 1)
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("L,nl,W", [((4, 2, 6, 2), 1, 1), ((4, 4, 4, 4), 4, 4), ((2, 4, 6, 4), 1, 8), ((4, 4, 4, 8), 1, 32)])
+def test_cshift_equals_numpy_roll_in_every_layout(L, nl, W, dtype):
+    gs = oracle.Geom(L, nl=nl)
+    g = gs if W == 1 else oracle.Geom(L, nl=nl, layout=oracle.su3_oracle.VECTOR, W=W)
+    a = su3gen.gaussian_field(9, 0, gs.nmat)
+    x = flat(a, dtype)
+    xl = x if W == 1 else oracle.convert(g, gs, x)
+    grid = x.reshape(L[3], L[2], L[1], L[0], nl, 18)
+    for dim in range(4):
+        for disp in (1, -1, 2, L[dim], -L[dim] - 1):
+            z = oracle.cshift(g, xl, dim, disp)
+            zs = z if W == 1 else oracle.convert(gs, g, z)
+            want = np.roll(grid, -disp, axis=3 - dim).reshape(-1)   # z[x] = x[x + disp]
+            assert np.array_equal(zs, want), (dim, disp)
+
+
+def test_cshift_group_structure_and_mul_shift():
+    g = oracle.Geom((4, 4, 2, 6), nl=1, layout=oracle.su3_oracle.VECTOR, W=4)
+    gs = oracle.Geom((4, 4, 2, 6))
+    x, y = (oracle.convert(g, gs, flat(su3gen.su3_field(9, f, gs.nmat))) for f in (0, 1))
+    assert np.array_equal(oracle.cshift(g, oracle.cshift(g, x, 2, 1), 2, -1), x)
+    assert np.array_equal(oracle.cshift(g, oracle.cshift(g, x, 3, 2), 3, 3), oracle.cshift(g, x, 3, 5))
+    assert np.array_equal(oracle.cshift(g, oracle.cshift(g, x, 0, 1), 3, 1), oracle.cshift(g, oracle.cshift(g, x, 3, 1), 0, 1))
+    assert np.array_equal(oracle.cshift(g, x, 1, 4), x)
+    for dim, disp in [(0, 1), (3, -1), (2, 1)]:
+        assert np.array_equal(oracle.mul_shift(g, x, y, dim, disp), oracle.mul(g, x, oracle.cshift(g, y, dim, disp)))
+    # the shifted product of SU(3) fields is SU(3); with y = x^dagger-free check: unitarity only
+    z = logical(oracle.convert(gs, g, oracle.mul_shift(g, x, y, 1, 1)))
+    assert np.abs(z @ z.conj().transpose(0, 2, 1) - np.eye(3)).max() <= 1e-13
+    with pytest.raises(ValueError):
+        oracle.cshift(g, x, 4, 1)
