@@ -146,6 +146,18 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
  * 18 per '+' or '-').  Validates the program like su3_expr.  Host-only. */
 su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix);
 
+/* Circular shift, Grid's Cshift(x, dim, disp) (P:219 names it as the next obstacle after the site-local
+ * product): z[s] = x[s + disp*dim_hat], periodic, for every site s and every mu; dim in 0..3, disp any
+ * integer.  A pure, bit-exact permutation of matrices in either layout (in the vector layout a step across
+ * a sub-lattice boundary moves a matrix to another lane).  Identical descriptors (SU3_ERR_MISMATCH); z and
+ * x must not be the same field (SU3_ERR_MISMATCH); dim outside 0..3 -> SU3_ERR_INVALID. */
+su3_status su3_cshift(su3_field *z, const su3_field *x, int dim, int disp, void *cuda_stream);
+
+/* z[s] = x[s] . y[s + disp*dim_hat] in one pass: the site-local product with a shifted second operand (the
+ * building block of covariant shifts and plaquettes).  Same FMA chain as su3_mul: bit-identical to
+ * su3_cshift followed by su3_mul.  z may be the same field as x but not as y. */
+su3_status su3_mul_shift(su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *cuda_stream);
+
 /* Layout conversion scalar <-> vector: a pure, bit-exact permutation of complex numbers,
  * vec[o][mu][e][l] = sca[site(o,l)][mu][e] (extract/merge).  Exactly one of
  * dst/src must be SU3_SCALAR and the other SU3_VECTOR; L, n_lorentz, prec must agree

@@ -16,7 +16,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
-           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_convert", "su3_copy", "su3_mul_host", "su3_tune_set",
+           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_cshift", "su3_mul_shift", "su3_convert", "su3_copy", "su3_mul_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info"]
 
 
@@ -54,6 +54,8 @@ def _load():
         "su3_mul3": (i32, [vp, vp, vp, vp, vp]),
         "su3_mul_add": (i32, [vp, vp, vp, vp, vp]),
         "su3_add": (i32, [vp, vp, vp, vp]),
+        "su3_cshift": (i32, [vp, vp, ctypes.c_int, ctypes.c_int, vp]),
+        "su3_mul_shift": (i32, [vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]),
         "su3_expr": (i32, [vp, ctypes.c_char_p, ctypes.POINTER(vp), ctypes.c_int, vp]),
         "su3_expr_cost": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.POINTER(i32), ctypes.POINTER(i32)]),
         "su3_convert": (i32, [vp, vp, vp]),
@@ -187,6 +189,14 @@ def su3_expr_cost(program, n_operands):
     st, fl = ctypes.c_int32(), ctypes.c_int32()
     _ck(lib.su3_expr_cost(program.encode(), int(n_operands), ctypes.byref(st), ctypes.byref(fl)))
     return st.value, fl.value
+
+
+def su3_cshift(z, x, dim, disp, stream=None):
+    _ck(lib.su3_cshift(z.handle, x.handle, int(dim), int(disp), _stream(stream)))
+
+
+def su3_mul_shift(z, x, y, dim, disp, stream=None):
+    _ck(lib.su3_mul_shift(z.handle, x.handle, y.handle, int(dim), int(disp), _stream(stream)))
 
 
 def su3_convert(dst, src, stream=None):

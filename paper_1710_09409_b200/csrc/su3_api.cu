@@ -370,6 +370,60 @@ template <typename R> expr_kernel_t expr_for_w(int W) {
   return nullptr;
 }
 
+// ---------------------------------------------------------------- Cshift / shifted product
+typedef void (*shift_kernel_t)(const su3::ShiftParams);
+template <typename R, int OP> shift_kernel_t shift_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_shift_kernel<R, 1, OP>;
+    case 2: return su3::su3_shift_kernel<R, 2, OP>;
+    case 4: return su3::su3_shift_kernel<R, 4, OP>;
+    case 8: return su3::su3_shift_kernel<R, 8, OP>;
+    case 16: return su3::su3_shift_kernel<R, 16, OP>;
+    case 32: return su3::su3_shift_kernel<R, 32, OP>;
+  }
+  return nullptr;
+}
+
+su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
+  if (!z || !y || (op == su3::SH_MUL && !x)) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_desc(z->d, y->d) || (x && !same_desc(z->d, x->d))) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
+  if (dim < 0 || dim > 3) return fail(SU3_ERR_INVALID, "dim = %d outside 0..3", dim);
+  if (z->ptr == y->ptr) return fail(SU3_ERR_MISMATCH, "the output must not be the shifted operand's field");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (z->nmat == 0) return SU3_OK;
+  const su3_desc &d = z->d;
+  su3::ShiftParams p;
+  memset(&p, 0, sizeof p);
+  p.z = z->ptr; p.x = x ? x->ptr : nullptr; p.y = y->ptr; p.nmat = z->nmat; p.nl = d.n_lorentz;
+  p.ostride = 1; p.lstride = 1;
+  for (int k = 0; k < dim; k++) {
+    p.ostride *= d.L[k] / d.simd[k];
+    p.lstride *= d.simd[k];
+  }
+  p.Ld = d.L[dim]; p.simd_d = d.simd[dim]; p.rd = d.L[dim] / d.simd[dim];
+  p.disp = ((disp % p.Ld) + p.Ld) % p.Ld;
+  shift_kernel_t k = d.prec == SU3_F64 ? (op == su3::SH_MUL ? shift_for_w<double, su3::SH_MUL>(d.W) : shift_for_w<double, su3::SH_COPY>(d.W))
+                                       : (op == su3::SH_MUL ? shift_for_w<float, su3::SH_MUL>(d.W) : shift_for_w<float, su3::SH_COPY>(d.W));
+  if (!k) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
+  su3_tune tn;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    tn = g_tune;
+  }
+  const int64_t nwt = (z->nmat + 31) / 32;
+  int wpb = 4;
+  while (wpb > 1 && (nwt + wpb - 1) / wpb < 2 * (int64_t)di.sms) wpb >>= 1;
+  const size_t smem = op == su3::SH_MUL ? (size_t)wpb * 2 * 288 * 2 * d.prec : 0;
+  const int64_t blocks_needed = (nwt + wpb - 1) / wpb;
+  const int64_t cap = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 8) * (4 / wpb);
+  k<<<(unsigned)(blocks_needed < cap ? blocks_needed : cap), wpb * 32, smem, (cudaStream_t)stream>>>(p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("shift kernel launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
 // ---------------------------------------------------------------- su3_mul_host resources
 struct HostPipe {
   std::mutex mu;
@@ -535,6 +589,13 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   if (e != cudaSuccess) return cuda_fail("su3_expr launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return SU3_OK;
+}
+
+su3_status su3_cshift(su3_field *z, const su3_field *x, int dim, int disp, void *cuda_stream) {
+  return launch_shift(su3::SH_COPY, z, nullptr, x, dim, disp, cuda_stream);
+}
+su3_status su3_mul_shift(su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *cuda_stream) {
+  return launch_shift(su3::SH_MUL, z, x, y, dim, disp, cuda_stream);
 }
 
 su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *stream) {

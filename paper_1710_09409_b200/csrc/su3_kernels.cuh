@@ -585,6 +585,100 @@ __global__ void __launch_bounds__(128) su3_warp_kernel(const StreamParams p) {
   }
 }
 
+// ---------------------------------------------------------------- Cshift and the shifted product (f3)
+// z[s] = y[s + disp*dim_hat] (SH_COPY, Grid's Cshift) and z[s] = x[s] . y[s + disp*dim_hat] (SH_MUL).
+// Warp-staged like su3_warp_kernel, but the shifted operand is GATHERED: lane t works out, once per tile,
+// where the neighbour of its own matrix lives -- in the vector layout a step across the sub-lattice
+// boundary lands in another lane of outer site oc' (the virtual-node map S3), so the source is
+// (record', lane') -- and every element load fetches that base from the owning lane with one shuffle.
+// Neighbouring lanes read neighbouring addresses except at the wrap, so the loads stay coalesced.
+enum { SH_COPY = 0, SH_MUL = 1 };
+struct ShiftParams {
+  void *z;
+  const void *x;  // unshifted operand (SH_MUL only)
+  const void *y;  // shifted operand
+  long long nmat;
+  long long ostride;  // prod_{k<dim} r[k]
+  int nl, rd, Ld, lstride, simd_d, disp;  // r[dim], L[dim], prod_{k<dim} simd[k], simd[dim], 0 <= disp < L[dim]
+};
+
+template <typename R, int W, int OP>
+__global__ void __launch_bounds__(128) su3_shift_kernel(const ShiftParams p) {
+  typedef typename Cplx<R>::type C2;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  C2 *sw = reinterpret_cast<C2 *>(smem) + (size_t)wib * 2 * 288;
+  const long long nwt = (p.nmat + 31) / 32;
+  const int base = (lane / W) * 9 * W + (lane % W);
+  const C2 *gx = reinterpret_cast<const C2 *>(p.x);
+  const C2 *gy = reinterpret_cast<const C2 *>(p.y);
+  C2 *gz = reinterpret_cast<C2 *>(p.z);
+  for (long long wt = (long long)blockIdx.x * wpb + wib; wt < nwt; wt += (long long)gridDim.x * wpb) {
+    const long long c0 = wt * 288;
+    const long long left = p.nmat - wt * 32;
+    const int nm = left < 32 ? (int)left : 32;
+    const int nc = nm * 9;
+    // where does the neighbour of MY matrix (slot `lane` of this tile) live?
+    long long srcbase = 0;
+    if (lane < nm) {
+      const long long g = wt * 32 + lane;
+      const long long rec = g / W;
+      const int l = (int)(g % W);
+      const long long o = rec / p.nl;
+      const int mu = (int)(rec - o * p.nl);
+      const int oc = (int)((o / p.ostride) % p.rd);
+      const int ic = (l / p.lstride) % p.simd_d;
+      int xn = ic * p.rd + oc + p.disp;
+      if (xn >= p.Ld) xn -= p.Ld;
+      const int icn = xn / p.rd, ocn = xn - icn * p.rd;
+      const long long on = o + (long long)(ocn - oc) * p.ostride;
+      const int ln = l + (icn - ic) * p.lstride;
+      srcbase = ((on * p.nl + mu) * 9) * W + ln;
+    }
+    C2 ry[9];
+#pragma unroll
+    for (int j = 0; j < 9; j++) {
+      const int idx = j * 32 + lane;
+      const int q = idx / (9 * W), rem = idx - q * 9 * W;
+      const int e = rem / W, l = rem - e * W;
+      const long long sb = __shfl_sync(0xffffffffu, srcbase, q * W + l);
+      if (idx < nc) ry[j] = gy[sb + e * W];
+    }
+    if (OP == SH_COPY) {
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) gz[c0 + j * 32 + lane] = ry[j];
+    } else {
+      C2 rx[9];
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) rx[j] = gx[c0 + j * 32 + lane];
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) {
+          sw[j * 32 + lane] = rx[j];
+          sw[288 + j * 32 + lane] = ry[j];
+        }
+      __syncwarp();
+      if (lane < nm) {
+        C2 a[9], b[9], c[9];
+#pragma unroll
+        for (int e = 0; e < 9; e++) a[e] = sw[base + e * W];
+#pragma unroll
+        for (int e = 0; e < 9; e++) b[e] = sw[288 + base + e * W];
+        mat33_mul(a, b, c);
+#pragma unroll
+        for (int e = 0; e < 9; e++) sw[base + e * W] = c[e];
+      }
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < 9; j++)
+        if (j * 32 + lane < nc) gz[c0 + j * 32 + lane] = sw[j * 32 + lane];
+      __syncwarp();
+    }
+  }
+}
+
 // ---------------------------------------------------------------- streaming ceilings (A6) and z = x + y
 // dst = src as a pure TMA pipeline: one thread per CTA moves tiles global -> shared -> global with
 // 1-D bulk copies through a ring of `stages` slots; no register ever holds data.  The ceiling the

@@ -1,0 +1,81 @@
+"""-m gpu: Cshift and the shifted product against the oracle.
+su3_cshift is a permutation: bit-exact.  su3_mul_shift: north_star tolerances, and bit-identical to
+su3_cshift followed by su3_mul."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1710_09409_b200 as su3
+from gpu_util import download, geom_of, host_field, upload
+from helpers import TOL, rel_err
+
+pytestmark = pytest.mark.gpu
+F64, F32, SC, VE = su3.SU3_F64, su3.SU3_F32, su3.SU3_SCALAR, su3.SU3_VECTOR
+
+CASES = [((4, 6, 4, 8), 1, SC, 1), ((3, 3, 3, 3), 1, SC, 1), ((5, 3, 1, 7), 4, SC, 1), ((6, 2, 10, 2), 4, VE, 8),
+         ((8, 8, 8, 8), 1, VE, 4), ((2, 2, 2, 2), 4, VE, 16), ((4, 4, 4, 8), 1, VE, 32), ((10, 6, 6, 2), 1, VE, 2),
+         ((12, 12, 12, 12), 1, VE, 8)]
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", CASES)
+def test_cshift_bit_exact_and_mul_shift(prec, L, nl, layout, W):
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    g = geom_of(desc)
+    x, y = host_field(desc, 51, 0), host_field(desc, 51, 1)
+    fx, fy, fz, fs = upload(desc, x), upload(desc, y), su3.alloc_field(desc), su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    for dim in range(4):
+        for disp in (1, -1, 3, L[dim], -2 * L[dim] - 1):
+            fz.tensor.fill_(0xFF)
+            su3.su3_cshift(fz, fy, dim, disp)
+            assert np.array_equal(download(fz), oracle.cshift(g, y, dim, disp)), (dim, disp)
+        for disp in (1, -1):
+            fz.tensor.fill_(0xFF)
+            su3.su3_mul_shift(fz, fx, fy, dim, disp)
+            z = download(fz)
+            err, _ = rel_err(z, oracle.mul_shift(g, x, y, dim, disp), Wn)
+            assert np.isfinite(z).all() and err <= TOL[prec], (dim, disp, err)
+            # fused == two passes, bit for bit (same FMA chain)
+            su3.su3_cshift(fs, fy, dim, disp)
+            su3.su3_tune_set(path=1)
+            su3.su3_mul(fs, fx, fs)
+            su3.su3_tune_set()
+            assert torch.equal(fs.tensor, fz.tensor)
+
+
+def test_custom_split_and_aliasing_rules():
+    desc = su3.make_desc((8, 4, 4, 4), layout=VE, W=8, simd=(4, 2, 1, 1), prec=F32)
+    g = geom_of(desc)
+    x, y = host_field(desc, 53, 0), host_field(desc, 53, 1)
+    fx, fy, fz = upload(desc, x), upload(desc, y), su3.alloc_field(desc)
+    for dim in range(4):
+        su3.su3_cshift(fz, fx, dim, 1)
+        assert np.array_equal(download(fz), oracle.cshift(g, x, dim, 1))
+    ref = oracle.mul_shift(g, x, y, 0, 1)
+    su3.su3_mul_shift(fx, fx, fy, 0, 1)           # z may be x
+    assert rel_err(download(fx), ref, 8)[0] <= TOL[F32]
+    n0 = su3.su3_launch_count()
+    for call in (lambda: su3.su3_cshift(fy, fy, 0, 1), lambda: su3.su3_mul_shift(fy, fx, fy, 0, 1)):
+        with pytest.raises(su3.Su3Error) as e:
+            call()
+        assert e.value.status == su3.SU3_ERR_MISMATCH
+    with pytest.raises(su3.Su3Error) as e:
+        su3.su3_cshift(fz, fy, 4, 1)
+    assert e.value.status == su3.SU3_ERR_INVALID
+    assert su3.su3_launch_count() == n0
+
+
+def test_cshift_full_size_32x4_lorentz_properties():
+    """any-size properties at config 3's size: shift by +1 then -1 is the identity; L shifts of 1 are the identity"""
+    desc = su3.make_desc(32, n_lorentz=4, layout=VE, W=4)
+    a, b, c = (su3.alloc_field(desc) for _ in range(3))
+    a.tensor.view(torch.float64).normal_()
+    for dim in range(4):
+        su3.su3_cshift(b, a, dim, 1)
+        su3.su3_cshift(c, b, dim, -1)
+        assert torch.equal(c.tensor, a.tensor)
+        assert not torch.equal(b.tensor, a.tensor)
+        su3.su3_cshift(c, a, dim, 32)
+        assert torch.equal(c.tensor, a.tensor)
