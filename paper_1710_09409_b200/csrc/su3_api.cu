@@ -416,7 +416,9 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   while (wpb > 1 && (nwt + wpb - 1) / wpb < 2 * (int64_t)di.sms) wpb >>= 1;
   const size_t smem = op == su3::SH_MUL ? (size_t)wpb * 2 * 288 * 2 * d.prec : 0;
   const int64_t blocks_needed = (nwt + wpb - 1) / wpb;
-  const int64_t cap = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 8) * (4 / wpb);
+  // measured defaults: Cshift one tile per warp (no grid-stride loop); the shifted product 8 persistent blocks/SM
+  const int64_t cap = tn.ctas_per_sm > 0 ? (int64_t)di.sms * tn.ctas_per_sm * (4 / wpb)
+                                         : (op == su3::SH_COPY ? 0x7fffffffLL : (int64_t)di.sms * 8 * (4 / wpb));
   k<<<(unsigned)(blocks_needed < cap ? blocks_needed : cap), wpb * 32, smem, (cudaStream_t)stream>>>(p);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("shift kernel launch", e);

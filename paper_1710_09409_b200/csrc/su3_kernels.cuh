@@ -603,7 +603,7 @@ struct ShiftParams {
 };
 
 template <typename R, int W, int OP>
-__global__ void __launch_bounds__(128) su3_shift_kernel(const ShiftParams p) {
+__global__ void __launch_bounds__(128, OP == SH_COPY ? 8 : 3) su3_shift_kernel(const ShiftParams p) {
   typedef typename Cplx<R>::type C2;
   extern __shared__ __align__(128) unsigned char smem[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
