@@ -470,6 +470,33 @@ def run_ceilings_and_sweep(args, r):
     return out, sweep
 
 
+def run_next_rows(args, r):
+    """SURVEY 8(f) rows beyond A1-A6, measured at an HBM-bound volume (48^4, fp64 scalar and vector W=4) with the
+    same protocol: f2 the one-pass expression evaluator, f3 Cshift and the shifted product."""
+    torch, su3, f = r["torch"], r["su3"], r["f"]
+    Ln = min(args.L, 48)
+    out = {"L": Ln, "prec": "f64", "expr": [], "shift": []}
+    for layout, W, names in ((0, 1, ("xs", "ys", "ws", "vs")), (1, W64, ("xv", "yv", "wv", "z3"))):
+        d = su3.make_desc(Ln, layout=layout, W=W)
+        nb = su3.su3_field_bytes(d)
+        ops = [su3.su3_field_wrap(d, f[n].tensor[:nb]) for n in names]
+        z = su3.su3_field_wrap(d, f["zc"].tensor[:nb])
+        lay = "scalar" if layout == 0 else "vector W=%d" % W
+        for prog in ("01*", "01*2*", "01*2+", "01+01*+", "01*23*+", "01+2+3+"):
+            n = max(int(c) for c in prog if c.isdigit()) + 1
+            st, fl = su3.su3_expr_cost(prog, n)
+            mn, _, _ = time_calls(torch, lambda: su3.su3_expr(z, prog, ops[:n]))
+            out["expr"].append({"program": prog, "layout": lay, "streams": st, "flops_per_matrix": fl,
+                                "GBps": st * nb / (mn * 1e-3) / 1e9, "GFLOPps": fl * Ln ** 4 / (mn * 1e-3) / 1e9})
+        for dim in range(4):
+            mn, _, _ = time_calls(torch, lambda: su3.su3_cshift(z, ops[1], dim, 1))
+            mn2, _, _ = time_calls(torch, lambda: su3.su3_mul_shift(z, ops[0], ops[1], dim, 1))
+            out["shift"].append({"dim": dim, "disp": 1, "layout": lay, "cshift_GBps": 2 * nb / (mn * 1e-3) / 1e9,
+                                 "mul_shift_GBps": 3 * nb / (mn2 * 1e-3) / 1e9,
+                                 "mul_shift_GFLOPps": FLOPS["mul"] * Ln ** 4 / (mn2 * 1e-3) / 1e9})
+    return out
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -484,8 +511,11 @@ def main():
     torch = r["torch"]
     e2e = None if args.no_e2e else run_e2e(args, r, world)
     ceilings, sweep = ({}, [])
+    next_rows = None
     if rank == 0:
         ceilings, sweep = run_ceilings_and_sweep(args, r)
+        if not args.no_sweep:
+            next_rows = run_next_rows(args, r)
     peak, peak_src = measured_peak()
     B, nmat = r["B"], r["nmat"]
     ops = []
@@ -525,7 +555,7 @@ def main():
         "GFLOPps": world * r["step_flops"] / (r["ms_per_step"] * 1e-3) / 1e9,
         "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
         "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k != "wsweep"},
-        "wsweep": ceilings.get("wsweep"), "sweep": sweep, "checks": r["checks"],
+        "wsweep": ceilings.get("wsweep"), "next_rows": next_rows, "sweep": sweep, "checks": r["checks"],
         "wall_s_timed_region": r["t_wall"],
     }
     print(json.dumps(line), flush=True)
