@@ -303,6 +303,53 @@ int orc_mul_shift(const orc_geom *g, int prec, const void *x, const void *y, int
   return 0;
 }
 
+/* ---- colour-vector fields (3 complex per (site, mu)) and y = U.psi (f4; the building block
+ * of the Dslash-type stencil operators the paper says it is porting).  Layout by the same readings as the
+ * matrix field with 3 components instead of 9:
+ *   scalar: ((site*nl + mu)*3 + i)*2 + reim        vector: (((o*nl + mu)*3 + i)*W + l)*2 + reim          */
+int64_t orc_index_vec(const orc_geom *g, int64_t site, int mu, int i, int reim) {
+  if (g->layout == 0) return ((site * g->nl + mu) * 3 + i) * 2 + reim;
+  int64_t o; int32_t l;
+  orc_site_to_outer(g, site, &o, &l);
+  return (((o * g->nl + mu) * 3 + i) * g->W + l) * 2 + reim;
+}
+
+/* y_i = sum_j U_ij psi_j, j ascending, 4 real mul + 2 add per term (S7); fp64 result. */
+void orc_matvec(const orc_geom *g, int prec, const void *U, const void *psi, double *y) {
+  int64_t V = orc_volume(g);
+#pragma omp parallel for schedule(static)
+  for (int64_t site = 0; site < V; site++)
+    for (int mu = 0; mu < g->nl; mu++) {
+      double a[3][3][2];
+      load33(g, prec, U, site, mu, a);
+      for (int i = 0; i < 3; i++) {
+        double re = 0.0, im = 0.0;
+        for (int j = 0; j < 3; j++) {
+          double br = rd(psi, prec, orc_index_vec(g, site, mu, j, 0)), bi = rd(psi, prec, orc_index_vec(g, site, mu, j, 1));
+          re += a[i][j][0] * br - a[i][j][1] * bi;
+          im += a[i][j][0] * bi + a[i][j][1] * br;
+        }
+        y[orc_index_vec(g, site, mu, i, 0)] = re;
+        y[orc_index_vec(g, site, mu, i, 1)] = im;
+      }
+    }
+}
+
+/* layout permutation of a colour-vector field, bit copy */
+int orc_convert_vec(const orc_geom *gd, const orc_geom *gs, int prec, void *dst, const void *src) {
+  for (int d = 0; d < 4; d++) if (gd->L[d] != gs->L[d]) return 3;
+  if (gd->nl != gs->nl) return 3;
+  int64_t V = orc_volume(gs);
+#pragma omp parallel for schedule(static)
+  for (int64_t site = 0; site < V; site++)
+    for (int mu = 0; mu < gs->nl; mu++)
+      for (int i = 0; i < 3; i++)
+        for (int c = 0; c < 2; c++)
+          memcpy((char *)dst + prec * orc_index_vec(gd, site, mu, i, c),
+                 (const char *)src + prec * orc_index_vec(gs, site, mu, i, c), (size_t)prec);
+  return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

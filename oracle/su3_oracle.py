@@ -45,6 +45,12 @@ def _load():
         lib.orc_mul_shift.restype = I
         lib.orc_neighbour.argtypes = [P, I64, I, I]
         lib.orc_neighbour.restype = I64
+        lib.orc_index_vec.argtypes = [P, I64, I, I, I]
+        lib.orc_index_vec.restype = I64
+        lib.orc_matvec.argtypes = [P, I, V, V, V]
+        lib.orc_matvec.restype = None
+        lib.orc_convert_vec.argtypes = [P, P, I, V, V]
+        lib.orc_convert_vec.restype = I
         lib.orc_convert.argtypes = [P, P, I, V, V]
         lib.orc_convert.restype = I
         lib.orc_num_threads.restype = I
@@ -167,6 +173,27 @@ def mul_shift(g, x, y, dim, disp):
     if _load().orc_mul_shift(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, int(dim), int(disp), z.ctypes.data):
         raise ValueError("dim %r outside 0..3" % (dim,))
     return z
+
+
+def index_vec(g, site, mu, i, reim):
+    return int(_load().orc_index_vec(ctypes.byref(g.c), int(site), int(mu), int(i), int(reim)))
+
+
+def matvec(g, U, psi):
+    """y = U.psi per (site, mu): U a matrix field, psi a colour-vector field (nmat*6 reals), layout g; fp64 result."""
+    p = _prec(U, g)
+    assert psi.flags.c_contiguous and psi.size == g.nmat * 6 and psi.dtype == U.dtype
+    y = np.empty(g.nmat * 6, dtype=np.float64)
+    _load().orc_matvec(ctypes.byref(g.c), p, U.ctypes.data, psi.ctypes.data, y.ctypes.data)
+    return y
+
+
+def convert_vec(g_dst, g_src, src):
+    assert src.flags.c_contiguous and src.size == g_src.nmat * 6
+    dst = np.empty_like(src)
+    if _load().orc_convert_vec(ctypes.byref(g_dst.c), ctypes.byref(g_src.c), src.dtype.itemsize, dst.ctypes.data, src.ctypes.data):
+        raise ValueError("geometry mismatch")
+    return dst
 
 
 def convert(g_dst, g_src, src):

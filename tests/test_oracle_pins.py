@@ -377,3 +377,65 @@ def test_cshift_group_structure_and_mul_shift():
     assert np.abs(z @ z.conj().transpose(0, 2, 1) - np.eye(3)).max() <= 1e-13
     with pytest.raises(ValueError):
         oracle.cshift(g, x, 4, 1)
+
+
+# ---------------------------------------------------------------- colour vectors and y = U.psi (f4)
+def test_matvec_integer_case_by_hand_and_numpy():
+    """A.(1, i, 2-i)^T by hand: row0 = (1+2i) + (-i)(i) + 3(2-i) = 8-i; row1 = (2-i) + (1+i)i = 1;
+    row2 = i - 2i + (1-i)(2-i) = 1-4i"""
+    g = oracle.Geom(2)
+    psi1 = np.array([1, 1j, 2 - 1j])
+    U = fill(g, IC["A"])
+    psi = np.ascontiguousarray(np.broadcast_to(psi1, (g.nmat, 3))).view(np.float64).reshape(-1)
+    y = oracle.matvec(g, U, psi).view(np.complex128).reshape(-1, 3)
+    assert np.array_equal(y, np.broadcast_to(np.array([8 - 1j, 1, 1 - 4j]), (16, 3)))
+    assert np.array_equal(IC["A"] @ psi1, np.array([8 - 1j, 1, 1 - 4j]))
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_matvec_invariants_layouts_and_einsum(dtype):
+    L, nl = (4, 2, 4, 2), 4
+    gs = oracle.Geom(L, nl=nl)
+    U = flat(su3gen.su3_field(21, 0, gs.nmat), dtype)
+    V = flat(su3gen.su3_field(21, 1, gs.nmat), dtype)
+    psi = su3gen.gaussian_field(21, 3, gs.nmat)[:, 0, :].copy().view(np.float64).reshape(-1).astype(dtype)
+    y = oracle.matvec(gs, U, psi)
+    Ul, pl = logical(U), psi.astype(np.float64).view(np.complex128).reshape(-1, 3)
+    want = np.einsum("mij,mj->mi", Ul, pl)
+    assert np.abs(y.view(np.complex128).reshape(-1, 3) - want).max() <= 1e-14
+    # SU(3) preserves the norm (fp32 storage perturbs unitarity of U at the 1e-7 level)
+    ny, npsi = np.linalg.norm(want, axis=1), np.linalg.norm(pl, axis=1)
+    assert np.abs(ny / npsi - 1).max() <= (1e-13 if dtype == np.float64 else 1e-6)
+    # identity and zero, exact
+    one = flat(np.broadcast_to(np.eye(3), (gs.nmat, 3, 3)).copy(), dtype)
+    assert np.array_equal(oracle.matvec(gs, one, psi), psi.astype(np.float64))
+    assert not oracle.matvec(gs, np.zeros_like(U), psi).any()
+    # (U.V).psi = U.(V.psi) to rounding (fp64 operands only: the intermediate is fp64)
+    if dtype == np.float64:
+        lhs = oracle.matvec(gs, oracle.mul(gs, U, V), psi)
+        rhs = oracle.matvec(gs, U, oracle.matvec(gs, V, psi))
+        assert np.abs(lhs - rhs).max() <= 1e-14
+    # every vector layout gives the same numbers, bit for bit, after the permutation
+    for W in (2, 4, 8, 16):
+        gv = oracle.Geom(L, nl=nl, layout=oracle.su3_oracle.VECTOR, W=W)
+        yv = oracle.matvec(gv, oracle.convert(gv, gs, U), oracle.convert_vec(gv, gs, psi))
+        assert np.array_equal(oracle.convert_vec(gs, gv, yv), y)
+        back = oracle.convert_vec(gs, gv, oracle.convert_vec(gv, gs, psi))
+        assert np.array_equal(back, psi)
+
+
+def test_index_vec_is_a_bijection_and_matches_the_matrix_map():
+    g = oracle.Geom((4, 2, 2, 4), nl=4, layout=oracle.su3_oracle.VECTOR, W=8)
+    seen = set()
+    for site in range(g.volume):
+        for mu in range(4):
+            for i in range(3):
+                for c in range(2):
+                    seen.add(oracle.index_vec(g, site, mu, i, c))
+        # same (outer site, lane) as the matrix map: component i of the vector sits where column-0 element i would
+        # sit in a 3-component record
+        o, l = oracle.site_to_outer(g, site)
+        assert oracle.index_vec(g, site, 2, 1, 1) == (((o * 4 + 2) * 3 + 1) * 8 + l) * 2 + 1
+    assert seen == set(range(g.nmat * 6))
+    gs = oracle.Geom((4, 2, 2, 4), nl=4)
+    assert oracle.index_vec(gs, 5, 3, 2, 1) == ((5 * 4 + 3) * 3 + 2) * 2 + 1
