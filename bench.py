@@ -494,6 +494,17 @@ def run_next_rows(args, r):
             out["shift"].append({"dim": dim, "disp": 1, "layout": lay, "cshift_GBps": 2 * nb / (mn * 1e-3) / 1e9,
                                  "mul_shift_GBps": 3 * nb / (mn2 * 1e-3) / 1e9,
                                  "mul_shift_GFLOPps": FLOPS["mul"] * Ln ** 4 / (mn2 * 1e-3) / 1e9})
+    # f4: colour vectors, y = U.psi (66 flops, 240 B fp64 / 120 B fp32 per site)
+    out["matvec"] = []
+    for prec, layout, W in ((8, 0, 1), (8, 1, W64), (4, 0, 1), (4, 1, W32)):
+        d = su3.make_desc(Ln, prec=prec, layout=layout, W=W)
+        U = su3.su3_field_wrap(d, f["xs"].tensor[:su3.su3_field_bytes(d)])      # bandwidth is data-independent
+        nv = su3.su3_vec_bytes(d)
+        psi, yv = su3.su3_vec_wrap(d, f["ys"].tensor[:nv]), su3.su3_vec_wrap(d, f["zc"].tensor[:nv])
+        mn, _, _ = time_calls(torch, lambda: su3.su3_matvec(yv, U, psi))
+        nb = su3.su3_field_bytes(d) + 2 * nv
+        out["matvec"].append({"prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector W=%d" % W,
+                              "GBps": nb / (mn * 1e-3) / 1e9, "GFLOPps": 66 * Ln ** 4 / (mn * 1e-3) / 1e9})
     return out
 
 

@@ -158,6 +158,20 @@ su3_status su3_cshift(su3_field *z, const su3_field *x, int dim, int disp, void 
  * su3_cshift followed by su3_mul.  z may be the same field as x but not as y. */
 su3_status su3_mul_shift(su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *cuda_stream);
 
+/* Colour-vector fields (f4; the operand of the Dslash-type stencils): 3 complex numbers per
+ * (site, mu) instead of 9, same descriptor, same two layouts with 3 in place of 9:
+ *   SU3_SCALAR : real offset = ((m*3) + i)*2 + reim        SU3_VECTOR : (((o*nl + mu)*3 + i)*W + l)*2 + reim
+ * su3_vec_bytes = volume * n_lorentz * 6 * prec.  A handle made by su3_vec_wrap is a su3_field of vector kind:
+ * su3_field_free / su3_field_desc / su3_field_ptr / su3_copy / su3_convert take it (both operands of the same
+ * kind); the matrix-only calls return SU3_ERR_MISMATCH for it. */
+su3_status su3_vec_bytes(const su3_desc *desc, size_t *nbytes);
+su3_status su3_vec_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out);
+su3_status su3_vec_index(const su3_desc *desc, int64_t site, int mu, int i, int reim, int64_t *off);
+
+/* y = U.psi, site by site: y_i = sum_j U_ij psi_j (66 flops, 144+48+48 B in fp64 per (site, mu)).  U a
+ * colour-matrix field, psi and y colour-vector fields, identical descriptors.  y may be the same field as psi. */
+su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, void *cuda_stream);
+
 /* Layout conversion scalar <-> vector: a pure, bit-exact permutation of complex numbers,
  * vec[o][mu][e][l] = sca[site(o,l)][mu][e] (extract/merge).  Exactly one of
  * dst/src must be SU3_SCALAR and the other SU3_VECTOR; L, n_lorentz, prec must agree

@@ -20,6 +20,7 @@ struct su3_field {
   size_t nbytes;
   int64_t volume;
   int64_t nmat;
+  int ncomp;  // complex numbers per (site, mu): 9 = colour matrix, 3 = colour vector
 };
 
 namespace {
@@ -273,6 +274,8 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
 
 su3_status check_arith(const su3_field *z, const su3_field *x, const su3_field *y, const su3_field *u, bool has_u) {
   if (!z || !x || !y || (has_u && !u)) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (z->ncomp != 9 || x->ncomp != 9 || y->ncomp != 9 || (has_u && u->ncomp != 9))
+    return fail(SU3_ERR_MISMATCH, "this call takes colour-matrix fields, not colour-vector fields");
   if (!same_desc(z->d, x->d) || !same_desc(z->d, y->d) || (has_u && !same_desc(z->d, u->d)))
     return fail(SU3_ERR_MISMATCH, "operand descriptors differ (L, n_lorentz, prec, layout, W, simd must all agree)");
   return SU3_OK;
@@ -387,6 +390,7 @@ template <typename R, int OP> shift_kernel_t shift_for_w(int W) {
 su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
   if (!z || !y || (op == su3::SH_MUL && !x)) return fail(SU3_ERR_NULL, "field handle is NULL");
   if (!same_desc(z->d, y->d) || (x && !same_desc(z->d, x->d))) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
+  if (z->ncomp != 9 || y->ncomp != 9 || (x && x->ncomp != 9)) return fail(SU3_ERR_MISMATCH, "colour-matrix fields expected");
   if (dim < 0 || dim > 3) return fail(SU3_ERR_INVALID, "dim = %d outside 0..3", dim);
   if (z->ptr == y->ptr) return fail(SU3_ERR_MISMATCH, "the output must not be the shifted operand's field");
   const DevInfo &di = devinfo();
@@ -426,6 +430,19 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   return SU3_OK;
 }
 
+// ---------------------------------------------------------------- y = U.psi
+template <typename R> stream_kernel_t matvec_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_matvec_kernel<R, 1, NCW>;
+    case 2: return su3::su3_matvec_kernel<R, 2, NCW>;
+    case 4: return su3::su3_matvec_kernel<R, 4, NCW>;
+    case 8: return su3::su3_matvec_kernel<R, 8, NCW>;
+    case 16: return su3::su3_matvec_kernel<R, 16, NCW>;
+    case 32: return su3::su3_matvec_kernel<R, 32, NCW>;
+  }
+  return nullptr;
+}
+
 // ---------------------------------------------------------------- su3_mul_host resources
 struct HostPipe {
   std::mutex mu;
@@ -463,19 +480,37 @@ su3_status su3_field_bytes(const su3_desc *desc, size_t *nbytes) {
   return SU3_OK;
 }
 
-su3_status su3_field_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
+static su3_status wrap_kind(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out, int ncomp) {
   if (!out) return fail(SU3_ERR_NULL, "out is NULL");
   su3_desc d;
   su3_status st = normalize(desc, &d);
   if (st != SU3_OK) return st;
   if (!dev_ptr) return fail(SU3_ERR_NULL, "device pointer is NULL");
   if ((uintptr_t)dev_ptr & 15) return fail(SU3_ERR_ALIGN, "device pointer %p is not 16-byte aligned", dev_ptr);
-  const size_t need = (size_t)volume_of(d) * d.n_lorentz * 18 * d.prec;
+  const size_t need = (size_t)volume_of(d) * d.n_lorentz * 2 * ncomp * d.prec;
   if (nbytes < need) return fail(SU3_ERR_SIZE, "buffer of %zu bytes is smaller than the %zu the field needs", nbytes, need);
   su3_field *f = new (std::nothrow) su3_field;
   if (!f) return fail(SU3_ERR_SIZE, "out of host memory");
   f->d = d; f->ptr = dev_ptr; f->nbytes = need; f->volume = volume_of(d); f->nmat = f->volume * d.n_lorentz;
+  f->ncomp = ncomp;
   *out = f;
+  return SU3_OK;
+}
+
+su3_status su3_field_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
+  return wrap_kind(desc, dev_ptr, nbytes, out, 9);
+}
+
+su3_status su3_vec_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
+  return wrap_kind(desc, dev_ptr, nbytes, out, 3);
+}
+
+su3_status su3_vec_bytes(const su3_desc *desc, size_t *nbytes) {
+  if (!nbytes) return fail(SU3_ERR_NULL, "nbytes is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  *nbytes = (size_t)volume_of(d) * d.n_lorentz * 6 * d.prec;
   return SU3_OK;
 }
 
@@ -548,7 +583,8 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   if (st != SU3_OK) return st;
   for (int k = 0; k < n_operands; k++) {
     if (!operands[k]) return fail(SU3_ERR_NULL, "operand %d is NULL", k);
-    if (!same_desc(z->d, operands[k]->d)) return fail(SU3_ERR_MISMATCH, "operand %d: descriptor differs from z", k);
+    if (!same_desc(z->d, operands[k]->d) || operands[k]->ncomp != 9 || z->ncomp != 9)
+      return fail(SU3_ERR_MISMATCH, "operand %d: descriptor differs from z (or not a colour-matrix field)", k);
   }
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
@@ -600,6 +636,70 @@ su3_status su3_mul_shift(su3_field *z, const su3_field *x, const su3_field *y, i
   return launch_shift(su3::SH_MUL, z, x, y, dim, disp, cuda_stream);
 }
 
+su3_status su3_vec_index(const su3_desc *desc, int64_t site, int mu, int i, int reim, int64_t *off) {
+  if (!off) return fail(SU3_ERR_NULL, "off is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  if (site < 0 || site >= volume_of(d) || mu < 0 || mu >= d.n_lorentz || i < 0 || i > 2 || reim < 0 || reim > 1)
+    return fail(SU3_ERR_INVALID, "index (site %lld, mu %d, i %d, reim %d) out of range", (long long)site, mu, i, reim);
+  if (d.layout == SU3_SCALAR) {
+    *off = ((site * d.n_lorentz + mu) * 3 + i) * 2 + reim;
+    return SU3_OK;
+  }
+  int64_t o = 0, ostride = 1, l = 0, lstride = 1, s = site;
+  for (int k = 0; k < 4; k++) {
+    const int64_t xk = s % d.L[k];
+    s /= d.L[k];
+    const int64_t r = d.L[k] / d.simd[k];
+    o += (xk % r) * ostride; ostride *= r;
+    l += (xk / r) * lstride; lstride *= d.simd[k];
+  }
+  *off = (((o * d.n_lorentz + mu) * 3 + i) * d.W + l) * 2 + reim;
+  return SU3_OK;
+}
+
+su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, void *stream) {
+  if (!y || !U || !psi) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (U->ncomp != 9 || psi->ncomp != 3 || y->ncomp != 3)
+    return fail(SU3_ERR_MISMATCH, "su3_matvec takes y, psi colour-vector fields and U a colour-matrix field");
+  if (!same_desc(y->d, U->d) || !same_desc(y->d, psi->d)) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (y->nmat == 0) return SU3_OK;
+  su3_tune tn;
+  {
+    std::lock_guard<std::mutex> lk(g_tune_mu);
+    tn = g_tune;
+  }
+  const int cb = 2 * y->d.prec;
+  stream_kernel_t k = y->d.prec == SU3_F64 ? matvec_for_w<double>(y->d.W) : matvec_for_w<float>(y->d.W);
+  if (!k) return fail(SU3_ERR_INVALID, "no matvec kernel for W %d", y->d.W);
+  // measured (48^4): ~110 KB in flight per SM is the sweet spot -> 2 CTAs/SM of 24.6 KB stages (fp64), 4 of 12.3 KB (fp32)
+  const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (y->d.prec == SU3_F64 ? 2 : 4);
+  int tm = tn.tile_mats;
+  if (tm == 0) {
+    tm = 128;
+    while (tm > 32 && (y->nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
+  }
+  const size_t stage_bytes = (size_t)tm * 12 * cb;
+  const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+  int stages = tn.stages > 0 ? tn.stages : 3;
+  while (tn.stages == 0 && stages > 2 && stages * stage_bytes + 256 > budget) stages--;
+  const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t);
+  if (smem + 256 > budget) return fail(SU3_ERR_INVALID, "su3_matvec pipeline needs %zu B of shared memory (tile %d, %d stages, %d CTAs/SM)", smem, tm, stages, ctas);
+  cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
+  if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
+  su3::StreamParams p;
+  p.z = y->ptr; p.x = U->ptr; p.y = psi->ptr; p.u = nullptr; p.nmat = y->nmat; p.tile_mats = tm; p.stages = stages; p.hint = 0;
+  const int64_t ntiles = (y->nmat + tm - 1) / tm, max_grid = (int64_t)di.sms * ctas;
+  k<<<(unsigned)(ntiles < max_grid ? ntiles : max_grid), (NCW + 1) * 32, smem, (cudaStream_t)stream>>>(p);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_matvec launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
 su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *stream) {
   su3_status st = check_arith(z, x, y, nullptr, false);
   if (st != SU3_OK) return st;
@@ -628,7 +728,7 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *s
 
 su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
   if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
-  if (!same_desc(dst->d, src->d)) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors");
+  if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds");
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (dst->nbytes == 0) return SU3_OK;
@@ -675,6 +775,8 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   if (dst->d.layout == src->d.layout)
     return fail(SU3_ERR_MISMATCH, "su3_convert: exactly one of dst/src must be SU3_SCALAR and the other SU3_VECTOR");
   if (dst->ptr == src->ptr) return fail(SU3_ERR_MISMATCH, "su3_convert: dst and src must not alias");
+  if (dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_convert: matrix and vector fields cannot be mixed");
+  const int nc = dst->ncomp;
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   const su3_desc &v = (dst->d.layout == SU3_VECTOR) ? dst->d : src->d;
@@ -698,7 +800,7 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
       rem /= v.simd[k];
       off += (long long)ic * p.r[k] * p.sstride[k];
     }
-    p.lane_off[l] = off * v.n_lorentz * 9;
+    p.lane_off[l] = off * v.n_lorentz * nc;
   }
   if (p.nrec == 0) return SU3_OK;
   constexpr int TR = 64;
@@ -708,8 +810,10 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   const unsigned grid = (unsigned)blocks;
 #define SU3_CONVERT_CASE(WW)                                                                     \
   case WW:                                                                                       \
-    if (v.prec == SU3_F64) su3::su3_convert_kernel<double2, WW, TR><<<grid, 256, 0, s>>>(p);     \
-    else su3::su3_convert_kernel<float2, WW, TR><<<grid, 256, 0, s>>>(p);                        \
+    if (v.prec == SU3_F64 && nc == 9) su3::su3_convert_kernel<double2, WW, TR, 9><<<grid, 256, 0, s>>>(p);      \
+    else if (v.prec == SU3_F64) su3::su3_convert_kernel<double2, WW, TR, 3><<<grid, 256, 0, s>>>(p);            \
+    else if (nc == 9) su3::su3_convert_kernel<float2, WW, TR, 9><<<grid, 256, 0, s>>>(p);                       \
+    else su3::su3_convert_kernel<float2, WW, TR, 3><<<grid, 256, 0, s>>>(p);                                    \
     break;
   switch (v.W) {
     SU3_CONVERT_CASE(1) SU3_CONVERT_CASE(2) SU3_CONVERT_CASE(4) SU3_CONVERT_CASE(8) SU3_CONVERT_CASE(16) SU3_CONVERT_CASE(32)

@@ -510,6 +510,118 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprP
   if (t == 0) bulk_wait_all<0>();
 }
 
+// ---------------------------------------------------------------- y = U.psi on colour vectors (f4)
+// Same pipeline as su3_pipe_kernel with two operand slots of different record size: U (9 complex per
+// matrix) and psi (3 complex per vector; record of the vector layout = 3 element vectors of W lanes).
+// p.x = U, p.y = psi, p.z = y.  y overwrites the psi slot and leaves by a bulk store.  66 flops and
+// 144+48+48 B (fp64) per (site, mu).
+template <typename R, int W, int NCW>
+__global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_matvec_kernel(const StreamParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int CB = (int)sizeof(C2);
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int TM = p.tile_mats, S = p.stages;
+  const uint32_t uslot = (uint32_t)TM * 9u * CB, vslot = (uint32_t)TM * 3u * CB;
+  const uint32_t stage_bytes = uslot + vslot;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)S * stage_bytes);
+  uint64_t *empty = full + S;
+  const int tid = threadIdx.x;
+  const long long ntiles = (p.nmat + TM - 1) / TM;
+  if (tid == 0) {
+    for (int s = 0; s < S; s++) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], 1);
+    }
+    fence_mbar_init();
+    fence_proxy_async();
+  }
+  __syncthreads();
+  if (tid >= NCW * 32) {
+    if (tid == NCW * 32) {
+      const unsigned char *gu = (const unsigned char *)p.x, *gv = (const unsigned char *)p.y;
+      int s = 0;
+      uint32_t ph = 0;
+      for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(&empty[s], ph ^ 1u);
+        const long long m0 = tile * TM;
+        const long long left = p.nmat - m0;
+        const int nm = left < TM ? (int)left : TM;
+        const uint32_t ub = (uint32_t)nm * 9u * CB, vb = (uint32_t)nm * 3u * CB;
+        const uint32_t ub16 = ub & ~15u, vb16 = vb & ~15u;
+        unsigned char *st = smem + (size_t)s * stage_bytes;
+        if (ub != ub16)
+          *reinterpret_cast<uint64_t *>(st + ub16) = *reinterpret_cast<const uint64_t *>(gu + (size_t)m0 * 9u * CB + ub16);
+        if (vb != vb16)
+          *reinterpret_cast<uint64_t *>(st + uslot + vb16) =
+              *reinterpret_cast<const uint64_t *>(gv + (size_t)m0 * 3u * CB + vb16);
+        mbar_arrive_expect_tx(&full[s], ub16 + vb16);
+        bulk_g2s(st, gu + (size_t)m0 * 9u * CB, ub16, &full[s]);
+        if (vb16) bulk_g2s(st + uslot, gv + (size_t)m0 * 3u * CB, vb16, &full[s]);
+        if (++s == S) {
+          s = 0;
+          ph ^= 1u;
+        }
+      }
+    }
+    return;
+  }
+  const int t = tid;
+  const int ubase = (t / W) * 9 * W + (t % W), vbase = (t / W) * 3 * W + (t % W);
+  int s = 0, prev_s = -1;
+  uint32_t ph = 0;
+  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const long long m0 = tile * TM;
+    const long long left = p.nmat - m0;
+    const int nm = left < TM ? (int)left : TM;
+    unsigned char *st = smem + (size_t)s * stage_bytes;
+    mbar_wait(&full[s], ph);
+    if (t < nm) {
+      const C2 *su = reinterpret_cast<const C2 *>(st) + ubase;
+      C2 *sv = reinterpret_cast<C2 *>(st + uslot) + vbase;
+      C2 a[9], b[3], c[3];
+#pragma unroll
+      for (int e = 0; e < 9; e++) a[e] = su[e * W];
+#pragma unroll
+      for (int j = 0; j < 3; j++) b[j] = sv[j * W];
+#pragma unroll
+      for (int i = 0; i < 3; i++) {  // y_i = sum_j U_ij psi_j, j ascending: the FMA chain of mat33_mul
+        auto re = mul_rn(a[3 * i].x, b[0].x);
+        auto im = mul_rn(a[3 * i].x, b[0].y);
+        re = fma_rn(-a[3 * i].y, b[0].y, re);
+        im = fma_rn(a[3 * i].y, b[0].x, im);
+#pragma unroll
+        for (int j = 1; j < 3; j++) {
+          re = fma_rn(a[3 * i + j].x, b[j].x, re);
+          im = fma_rn(a[3 * i + j].x, b[j].y, im);
+          re = fma_rn(-a[3 * i + j].y, b[j].y, re);
+          im = fma_rn(a[3 * i + j].y, b[j].x, im);
+        }
+        c[i].x = re;
+        c[i].y = im;
+      }
+#pragma unroll
+      for (int i = 0; i < 3; i++) sv[i * W] = c[i];
+    }
+    fence_proxy_async();
+    named_bar_sync(1, NCW * 32);
+    if (t == 0) {
+      const uint32_t vb = (uint32_t)nm * 3u * CB, vb16 = vb & ~15u;
+      unsigned char *ydst = (unsigned char *)p.z + (size_t)m0 * 3u * CB;
+      if (vb16) bulk_s2g(ydst, st + uslot, vb16);
+      bulk_commit();
+      if (vb != vb16) *reinterpret_cast<uint64_t *>(ydst + vb16) = *reinterpret_cast<const uint64_t *>(st + uslot + vb16);
+      bulk_wait_read<1>();
+      if (prev_s >= 0) mbar_arrive(&empty[prev_s]);
+    }
+    prev_s = s;
+    if (++s == S) {
+      s = 0;
+      ph ^= 1u;
+    }
+  }
+  if (t == 0) bulk_wait_all<0>();
+}
+
 // ---------------------------------------------------------------- warp-staged path (path = 3)
 // For L2-resident lattices the pipeline's fixed latency (mbarrier set-up, TMA in, TMA out) is what one
 // measures.  Here every warp stages its own 32 matrices with coalesced per-lane loads of one complex
@@ -810,11 +922,11 @@ struct ConvertParams {
   int nl;
   int r[4];             // sub-lattice extents L[d] / simd[d]
   long long sstride[4]; // scalar-site stride of dimension d: 1, L0, L0*L1, L0*L1*L2
-  long long lane_off[32]; // (site offset of lane l) * nl * 9, in complex numbers
+  long long lane_off[32]; // (site offset of lane l) * nl * NC, in complex numbers (NC = 9 matrix, 3 colour vector)
   int to_vector;        // 1: dst is the vector layout; 0: dst is the scalar layout
 };
 
-template <typename C2, int W, int TR>
+template <typename C2, int W, int TR, int NC>
 __global__ void __launch_bounds__(256) su3_convert_kernel(const ConvertParams p) {
   __shared__ long long sbase[TR];  // scalar-side complex index of (rec, lane 0, e = 0)
   const long long rec0 = (long long)blockIdx.x * TR;
@@ -831,13 +943,13 @@ __global__ void __launch_bounds__(256) su3_convert_kernel(const ConvertParams p)
       site += (o - q * p.r[d]) * p.sstride[d];
       o = q;
     }
-    sbase[threadIdx.x] = (site * p.nl + mu) * 9;
+    sbase[threadIdx.x] = (site * p.nl + mu) * NC;
   }
   __syncthreads();
   const C2 *src = reinterpret_cast<const C2 *>(p.src);
   C2 *dst = reinterpret_cast<C2 *>(p.dst);
-  const long long vbase = rec0 * 9 * W;
-  const int n = nr * 9 * W;
+  const long long vbase = rec0 * NC * W;
+  const int n = nr * NC * W;
   constexpr int U = 4;
   for (int i0 = threadIdx.x; i0 < n; i0 += 256 * U) {
     long long vi[U], si[U];
@@ -846,9 +958,9 @@ __global__ void __launch_bounds__(256) su3_convert_kernel(const ConvertParams p)
     for (int u = 0; u < U; u++) {
       const int idx = i0 + u * 256;
       const int l = idx % W;
-      const int q = idx / W;  // = rl*9 + e
-      const int rl = q / 9;
-      const int e = q - rl * 9;
+      const int q = idx / W;  // = rl*NC + e
+      const int rl = q / NC;
+      const int e = q - rl * NC;
       vi[u] = vbase + idx;
       si[u] = (idx < n) ? sbase[rl] + p.lane_off[l] + e : 0;
     }

@@ -140,3 +140,18 @@ def test_expr_program_validation_and_cost():
         with pytest.raises(su3.Su3Error) as e:
             su3.su3_expr_cost(bad, n)
         assert e.value.status == su3.SU3_ERR_INVALID, bad
+
+
+def test_colour_vector_boundary_host_side():
+    d = su3.make_desc((4, 2, 2, 4), n_lorentz=4, layout=su3.SU3_VECTOR, W=8, prec=su3.SU3_F32)
+    assert su3.su3_vec_bytes(d) == 64 * 4 * 6 * 4
+    assert su3.su3_vec_bytes(su3.make_desc(8)) == 4096 * 48
+    import oracle
+    g = oracle.Geom((4, 2, 2, 4), nl=4, layout=1, W=8)
+    for site in (0, 5, 17, 63):
+        for mu in (0, 3):
+            for i in range(3):
+                assert su3.su3_vec_index(d, site, mu, i, 1) == oracle.index_vec(g, site, mu, i, 1)
+    with pytest.raises(su3.Su3Error) as e:
+        su3.su3_vec_index(d, 0, 0, 3, 0)
+    assert e.value.status == su3.SU3_ERR_INVALID
