@@ -57,6 +57,9 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true", help="skip the volume sweep (configs[4]) after the timed steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--profile-pass", action="store_true",
+                    help="launch every kernel variant of the library once at 48^4 (no timing): the command ncu wraps "
+                         "for profiles/*_all_kernels.md")
     ap.add_argument("--cpu-L", type=int, default=32, help="lattice extent of the oracle's bounded sample")
     return ap.parse_args()
 
@@ -508,6 +511,48 @@ def run_next_rows(args, r):
     return out
 
 
+def profile_pass(args):
+    """One launch of every kernel variant at an HBM-bound size (inputs: Gaussian reals -- bandwidth and the
+    counters ncu reads do not depend on the values).  Prints one JSON line with the launch count."""
+    import torch
+
+    import paper_1710_09409_b200 as su3
+    torch.cuda.set_device(0)
+    L = min(args.L, 48)
+    n0 = su3.su3_launch_count()
+    order = []
+    for prec, W in ((su3.SU3_F64, W64), (su3.SU3_F32, W32)):
+        dt = torch.float64 if prec == su3.SU3_F64 else torch.float32
+        ds, dv = su3.make_desc(L, prec=prec), su3.make_desc(L, prec=prec, layout=su3.SU3_VECTOR, W=W)
+        xs, ys, ws, zs = (su3.alloc_field(ds) for _ in range(4))
+        xv, yv, wv, zv = (su3.alloc_field(dv) for _ in range(4))
+        for fld in (xs, ys, ws):
+            fld.tensor.view(dt).normal_()
+        for dst, src in ((xv, xs), (yv, ys), (wv, ws)):
+            su3.su3_convert(dst, src)
+        order.append("convert s->v x3")
+        for name, (x, y, w, z) in (("scalar", (xs, ys, ws, zs)), ("vector", (xv, yv, wv, zv))):
+            for path, pname in ((1, "pipe"), (2, "direct"), (3, "warp")):
+                su3.su3_tune_set(path=path)
+                su3.su3_mul(z, x, y); su3.su3_mul3(z, x, y, w); su3.su3_mul_add(z, x, y, w)
+                order.append("%s %s: mul mul3 mul_add" % (name, pname))
+            su3.su3_tune_set(path=1)
+            su3.su3_add(z, x, y); su3.su3_copy(z, x)
+            su3.su3_tune_set(path=2)
+            su3.su3_add(z, x, y); su3.su3_copy(z, x)
+            su3.su3_tune_set()
+            su3.su3_expr(z, "01+01*+", [x, y]); su3.su3_expr(z, "01*23*+", [x, y, w, x])
+            su3.su3_cshift(z, y, 0, 1); su3.su3_cshift(z, y, 3, 1); su3.su3_mul_shift(z, x, y, 1, 1)
+            psi = su3.su3_vec_wrap(x.desc, w.tensor[:su3.su3_vec_bytes(x.desc)])
+            yv_ = su3.su3_vec_wrap(x.desc, z.tensor[:su3.su3_vec_bytes(x.desc)])
+            su3.su3_matvec(yv_, x, psi)
+        su3.su3_convert(zs, zv)
+        torch.cuda.synchronize()
+        del xs, ys, ws, zs, xv, yv, wv, zv
+        torch.cuda.empty_cache()
+    print(json.dumps({"profile_pass": True, "L": L, "launches": su3.su3_launch_count() - n0}), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -515,6 +560,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.profile_pass:
+        if rank == 0:
+            profile_pass(args)
         return
     if world != args.gpus:
         log("note: --gpus %d but WORLD_SIZE=%d; using WORLD_SIZE (launch N>1 with torch.distributed.run)" % (args.gpus, world))
