@@ -585,9 +585,12 @@ def main():
                     "frac_of_measured_peak": gbs / peak,
                     "frac_of_copy": gbs / ceilings["bar_denominator"] if ceilings else None})
     a1 = ops[3]
+    # nominal pin-rate peak from device properties: memory clock x 2 (DDR) x bus width / 8
+    pin_rate = r["info"]["mem_clock_khz"] * 1e3 * 2 * r["info"]["bus_width_bits"] / 8 / 1e9
     roofline = {"bound": "hbm", "kernel": "su3_pipe_kernel<double,W=1,OP_MUL> (row A1, z=x*y fp64 scalar)",
                 "achieved": a1["GBps"], "peak": peak, "unit": "GB/s", "frac": a1["GBps"] / peak, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": 3 * B, "avg_launch_ms": a1["ms"],
+                "frac_of_same_run_copy": a1["frac_of_copy"], "pin_rate_peak": pin_rate, "frac_of_pin_rate_peak": a1["GBps"] / pin_rate,
                 # dram__bytes_read.sum + dram__bytes_write.sum of this launch at 64^4, from the one ncu --set full
                 # capture summarised in profiles/r01_pipe_kernel_full.md (4.831918 + 2.385510 GB)
                 "traffic": 7217428000 if args.L == 64 else None,
@@ -598,6 +601,9 @@ def main():
         times, nbytes, threads = oracle_step(Lc, 3)
         cpu = {"value": nbytes / min(times) / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": "rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep), best of 3 passes" % Lc}
+        t1, nb1, _ = oracle_step(min(Lc, 24), 1, threads=1)
+        cpu["one_thread_value"] = nb1 / min(t1) / 1e9
+        cpu["one_thread_sample"] = "the same rows on a %d^4 lattice, 1 thread, 1 pass" % min(Lc, 24)
     if r["dist"] is not None:
         r["dist"].barrier()
         r["dist"].destroy_process_group()
