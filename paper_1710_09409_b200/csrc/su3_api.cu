@@ -375,16 +375,20 @@ template <typename R> expr_kernel_t expr_for_w(int W) {
 
 // ---------------------------------------------------------------- Cshift / shifted product
 typedef void (*shift_kernel_t)(const su3::ShiftParams);
-template <typename R, int OP> shift_kernel_t shift_for_w(int W) {
+template <typename R, int OP, typename IT> shift_kernel_t shift_for_w(int W) {
   switch (W) {
-    case 1: return su3::su3_shift_kernel<R, 1, OP>;
-    case 2: return su3::su3_shift_kernel<R, 2, OP>;
-    case 4: return su3::su3_shift_kernel<R, 4, OP>;
-    case 8: return su3::su3_shift_kernel<R, 8, OP>;
-    case 16: return su3::su3_shift_kernel<R, 16, OP>;
-    case 32: return su3::su3_shift_kernel<R, 32, OP>;
+    case 1: return su3::su3_shift_kernel<R, 1, OP, IT>;
+    case 2: return su3::su3_shift_kernel<R, 2, OP, IT>;
+    case 4: return su3::su3_shift_kernel<R, 4, OP, IT>;
+    case 8: return su3::su3_shift_kernel<R, 8, OP, IT>;
+    case 16: return su3::su3_shift_kernel<R, 16, OP, IT>;
+    case 32: return su3::su3_shift_kernel<R, 32, OP, IT>;
   }
   return nullptr;
+}
+template <typename IT> shift_kernel_t shift_pick(int prec, int op, int W) {
+  if (prec == SU3_F64) return op == su3::SH_MUL ? shift_for_w<double, su3::SH_MUL, IT>(W) : shift_for_w<double, su3::SH_COPY, IT>(W);
+  return op == su3::SH_MUL ? shift_for_w<float, su3::SH_MUL, IT>(W) : shift_for_w<float, su3::SH_COPY, IT>(W);
 }
 
 su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
@@ -407,8 +411,8 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   }
   p.Ld = d.L[dim]; p.simd_d = d.simd[dim]; p.rd = d.L[dim] / d.simd[dim];
   p.disp = ((disp % p.Ld) + p.Ld) % p.Ld;
-  shift_kernel_t k = d.prec == SU3_F64 ? (op == su3::SH_MUL ? shift_for_w<double, su3::SH_MUL>(d.W) : shift_for_w<double, su3::SH_COPY>(d.W))
-                                       : (op == su3::SH_MUL ? shift_for_w<float, su3::SH_MUL>(d.W) : shift_for_w<float, su3::SH_COPY>(d.W));
+  // 32-bit index arithmetic whenever every complex index (plus one tile of slack) fits 31 bits
+  shift_kernel_t k = (z->nmat + 64) * 9 < 0x7fffffffLL ? shift_pick<int>(d.prec, op, d.W) : shift_pick<long long>(d.prec, op, d.W);
   if (!k) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
   su3_tune tn;
   {

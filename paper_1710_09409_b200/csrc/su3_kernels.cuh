@@ -714,36 +714,38 @@ struct ShiftParams {
   int nl, rd, Ld, lstride, simd_d, disp;  // r[dim], L[dim], prod_{k<dim} simd[k], simd[dim], 0 <= disp < L[dim]
 };
 
-template <typename R, int W, int OP>
-__global__ void __launch_bounds__(128, OP == SH_COPY ? 8 : 3) su3_shift_kernel(const ShiftParams p) {
+// IT = index type: int when every complex index of the field fits 31 bits (all configs), else long long.
+template <typename R, int W, int OP, typename IT>
+__global__ void __launch_bounds__(128, OP == SH_COPY ? (sizeof(R) == 4 ? 12 : 8) : 3) su3_shift_kernel(const ShiftParams p) {
   typedef typename Cplx<R>::type C2;
   extern __shared__ __align__(128) unsigned char smem[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
   C2 *sw = reinterpret_cast<C2 *>(smem) + (size_t)wib * 2 * 288;
-  const long long nwt = (p.nmat + 31) / 32;
+  const IT nwt = (IT)((p.nmat + 31) / 32);
+  const IT ostride = (IT)p.ostride;
   const int base = (lane / W) * 9 * W + (lane % W);
   const C2 *gx = reinterpret_cast<const C2 *>(p.x);
   const C2 *gy = reinterpret_cast<const C2 *>(p.y);
   C2 *gz = reinterpret_cast<C2 *>(p.z);
-  for (long long wt = (long long)blockIdx.x * wpb + wib; wt < nwt; wt += (long long)gridDim.x * wpb) {
-    const long long c0 = wt * 288;
-    const long long left = p.nmat - wt * 32;
+  for (IT wt = (IT)blockIdx.x * wpb + wib; wt < nwt; wt += (IT)gridDim.x * wpb) {
+    const IT c0 = wt * 288;
+    const IT left = (IT)p.nmat - wt * 32;
     const int nm = left < 32 ? (int)left : 32;
     const int nc = nm * 9;
     // where does the neighbour of MY matrix (slot `lane` of this tile) live?
-    long long srcbase = 0;
+    IT srcbase = 0;
     if (lane < nm) {
-      const long long g = wt * 32 + lane;
-      const long long rec = g / W;
+      const IT g = wt * 32 + lane;
+      const IT rec = g / W;
       const int l = (int)(g % W);
-      const long long o = rec / p.nl;
+      const IT o = rec / p.nl;
       const int mu = (int)(rec - o * p.nl);
-      const int oc = (int)((o / p.ostride) % p.rd);
+      const int oc = (int)((o / ostride) % p.rd);
       const int ic = (l / p.lstride) % p.simd_d;
       int xn = ic * p.rd + oc + p.disp;
       if (xn >= p.Ld) xn -= p.Ld;
       const int icn = xn / p.rd, ocn = xn - icn * p.rd;
-      const long long on = o + (long long)(ocn - oc) * p.ostride;
+      const IT on = o + (IT)(ocn - oc) * ostride;
       const int ln = l + (icn - ic) * p.lstride;
       srcbase = ((on * p.nl + mu) * 9) * W + ln;
     }
@@ -753,7 +755,7 @@ __global__ void __launch_bounds__(128, OP == SH_COPY ? 8 : 3) su3_shift_kernel(c
       const int idx = j * 32 + lane;
       const int q = idx / (9 * W), rem = idx - q * 9 * W;
       const int e = rem / W, l = rem - e * W;
-      const long long sb = __shfl_sync(0xffffffffu, srcbase, q * W + l);
+      const IT sb = __shfl_sync(0xffffffffu, srcbase, q * W + l);
       if (idx < nc) ry[j] = gy[sb + e * W];
     }
     if (OP == SH_COPY) {
