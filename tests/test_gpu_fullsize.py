@@ -137,3 +137,54 @@ def test_config3_32x4_lorentz4_fp64():
 
 def test_config4_48x4_fp32_W8_fused():
     run_config(48, 1, F32, 8, su3gen.config_seed(4), ["mul3", "mul_add"])
+
+
+def test_maximum_size_64x4_lorentz4_fp64():
+    """the largest field of the configs' shapes: 64^4 x 4 Lorentz matrices, fp64 = 9.66 GB per field (byte
+    offsets beyond 2^32, 67M matrices): sampled parity for mul in both layouts, convert, Cshift"""
+    L, nl, seed = 64, 4, su3gen.config_seed(3)
+    ds = su3.make_desc(L, n_lorentz=nl)
+    dv = su3.make_desc(L, n_lorentz=nl, layout=VE, W=4)
+    gs, gv = geom_of(ds), geom_of(dv)
+    sites = sample_sites(gs.volume, seed)[::3]
+    off_s, off_v = offsets(gs, sites), offsets(gv, sites)
+    small = oracle.Geom((len(sites), 1, 1, 1), nl=nl)
+    hx = host_logical(ds, seed, su3gen.FIELD_X)
+    sx = hx[off_s.reshape(-1)]
+    xs = up(ds, hx)
+    # neighbours of the sampled sites in x3 (the slowest dimension: source 64^3*4 matrices = 151 MB away)
+    nb_sites = np.array([oracle.neighbour(gs, int(s), 3, 1) for s in sites], dtype=np.int64)
+    sx_nb = hx[offsets(gs, nb_sites).reshape(-1)]
+    del hx
+    hy = host_logical(ds, seed, su3gen.FIELD_Y)
+    sy = hy[off_s.reshape(-1)]
+    ys = up(ds, hy)
+    del hy
+    zs = su3.alloc_field(ds)
+    zs.tensor.fill_(0xFF)
+    su3.su3_mul(zs, xs, ys)
+    ref = oracle.mul(small, sx, sy)
+    err, _ = rel_err(gather(zs, off_s), ref, 1)
+    assert err <= TOL[F64], err
+    assert not torch.isnan(zs.tensor.view(torch.float64)[-18 * 4096:]).any()      # the far end was written
+    # Cshift along x3, then the scalar -> vector permutation, at full size
+    su3.su3_cshift(zs, xs, 3, 1)
+    assert np.array_equal(gather(zs, off_s), sx_nb)
+    xv = su3.alloc_field(dv)
+    su3.su3_convert(xv, xs)
+    assert np.array_equal(gather(xv, off_v), sx)
+    del zs
+    yv, zv = su3.alloc_field(dv), su3.alloc_field(dv)
+    su3.su3_convert(yv, ys)
+    su3.su3_mul(zv, xv, yv)
+    err, _ = rel_err(gather(zv, off_v), ref, 1)
+    assert err <= TOL[F64], err
+    su3.su3_mul_shift(zv, xv, yv, 3, 1)
+    err, _ = rel_err(gather(zv, off_v), oracle.mul(small, sx, hy_nb(gs, ys, sites)), 1)
+    assert err <= TOL[F64], err
+
+
+def hy_nb(gs, ys, sites):
+    """y at the x3-neighbours of the sampled sites, gathered from the device copy of the scalar-layout field"""
+    nb_sites = np.array([oracle.neighbour(gs, int(s), 3, 1) for s in sites], dtype=np.int64)
+    return gather(ys, offsets(gs, nb_sites))
