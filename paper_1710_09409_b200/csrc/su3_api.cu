@@ -807,6 +807,27 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
     p.lane_off[l] = off * v.n_lorentz * nc;
   }
   if (p.nrec == 0) return SU3_OK;
+  const su3_tune tn_c = [] { std::lock_guard<std::mutex> lk(g_tune_mu); return g_tune; }();
+  if (v.prec == SU3_F32 && tn_c.path != 2) {  // staged through shared memory: 256-byte requests on both sides
+    cudaStream_t s = (cudaStream_t)stream;
+#define SU3_STAGED(WW, TRR)                                                                                        \
+  case WW: {                                                                                                       \
+    const long long blocks = (p.nrec + TRR - 1) / TRR;                                                             \
+    if (blocks > 0x7fffffffLL) return fail(SU3_ERR_SIZE, "su3_convert: lattice too large for one launch");         \
+    const size_t smem = sizeof(float2) * TRR * nc * (WW + 1) + sizeof(long long) * TRR;                                  \
+    if (nc == 9) su3::su3_convert_staged_kernel<float2, WW, TRR, 9><<<(unsigned)blocks, 256, smem, s>>>(p);        \
+    else su3::su3_convert_staged_kernel<float2, WW, TRR, 3><<<(unsigned)blocks, 256, smem, s>>>(p);                \
+  } break;
+    switch (v.W) {
+      SU3_STAGED(1, 64) SU3_STAGED(2, 64) SU3_STAGED(4, 64) SU3_STAGED(8, 64) SU3_STAGED(16, 32) SU3_STAGED(32, 16)
+      default: return fail(SU3_ERR_INVALID, "su3_convert: W = %d", v.W);
+    }
+#undef SU3_STAGED
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return SU3_OK;
+  }
   constexpr int TR = 64;
   const long long blocks = (p.nrec + TR - 1) / TR;
   if (blocks > 0x7fffffffLL) return fail(SU3_ERR_SIZE, "su3_convert: lattice too large for one launch");
