@@ -593,6 +593,26 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (z->nmat == 0) return SU3_OK;
+  {
+    // the fixed menu: programs that ARE one of the ahead-of-time kernels run on them (same FMA chain, so the
+    // result is bit-identical either way; IEEE addition is commutative, so v + x*y is x*y + v)
+    const su3::ExprIns *in = pr.ins;
+    const bool first_on_operands = in[0].a < su3::EX_TEMP0 && in[0].b < su3::EX_TEMP0;
+    int op = -1;
+    const su3_field *fx = nullptr, *fy = nullptr, *fu = nullptr;
+    if (pr.nins >= 1 && first_on_operands && in[0].op != su3::EX_SUB && in[0].op != su3::EX_COPY) {
+      fx = operands[in[0].a]; fy = operands[in[0].b];
+      if (pr.nins == 1) op = in[0].op == su3::EX_MUL ? su3::OP_MUL : su3::OP_ADD;
+      else if (pr.nins == 2 && in[0].op == su3::EX_MUL && in[1].spill == su3::EX_NONE) {
+        if (in[1].op == su3::EX_MUL && in[1].a == su3::EX_SRC_ACC && in[1].b < su3::EX_TEMP0) { op = su3::OP_MUL3; fu = operands[in[1].b]; }
+        else if (in[1].op == su3::EX_ADD && in[1].a == su3::EX_SRC_ACC && in[1].b < su3::EX_TEMP0) { op = su3::OP_MUL_ADD; fu = operands[in[1].b]; }
+        else if (in[1].op == su3::EX_ADD && in[1].b == su3::EX_SRC_ACC && in[1].a < su3::EX_TEMP0) { op = su3::OP_MUL_ADD; fu = operands[in[1].a]; }
+      }
+    }
+    if (op >= 0)
+      return launch_stream(op, z->d.prec, op == su3::OP_ADD ? 1 : z->d.W, z->ptr, fx->ptr, fy->ptr, fu ? fu->ptr : nullptr, z->nmat,
+                           z->nbytes * (fu ? 4 : 3), (cudaStream_t)cuda_stream);
+  }
   su3_tune tn;
   {
     std::lock_guard<std::mutex> lk(g_tune_mu);
@@ -601,32 +621,39 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   const int cb = 2 * z->d.prec;
   expr_kernel_t k = z->d.prec == SU3_F64 ? expr_for_w<double>(z->d.W) : expr_for_w<float>(z->d.W);
   if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", z->d.W);
-  int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
-  int tm = tn.tile_mats > 0 ? tn.tile_mats : 9216 / (9 * cb);
-  while (tn.tile_mats == 0 && tm > 32 && (z->nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
-  int stages = tn.stages > 0 ? tn.stages : 3;
-  size_t smem = 0;
-  for (;;) {  // shrink ring, then CTAs/SM, then the tile until the operand slots and temporaries fit
-    const size_t slot = (size_t)tm * 9 * cb;
-    smem = ((size_t)stages * n_operands + pr.ntemp) * slot + 2 * stages * sizeof(uint64_t);
-    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
-    if (smem + 256 <= budget) break;
-    if (tn.stages == 0 && stages > 2) stages--;
-    else if (tn.ctas_per_sm == 0 && ctas > 1) ctas--;
-    else if (tn.tile_mats == 0 && tm > 32) tm >>= 1;
-    else return fail(SU3_ERR_INVALID, "expression needs %zu B of shared memory (tile %d, %d stages, %d operands, %d temporaries)",
-                     smem, tm, stages, n_operands, pr.ntemp);
+  // Every warp is a self-contained pipeline with a private ring of `sw` stages of 32 matrices per operand.  Long programs are latency-bound per tile, so the launch maximises resident warps per SM
+  // under the shared-memory budget (ring depth 2, 3 if there is room for >= 8 warps anyway), at most 16.
+  const int mps = 32;
+  const size_t slot = (size_t)mps * 9 * cb;
+  const size_t stage_bytes = (size_t)n_operands * slot;
+  const size_t sm_bytes = (size_t)di.smem_optin - 4096;  // what one SM can give to its resident CTAs, minus slack
+  int sw = tn.stages > 0 ? tn.stages : 3;
+  int warps = (int)(sm_bytes / (sw * stage_bytes + pr.ntemp * slot + 64));
+  if (tn.stages == 0 && warps < 8) {
+    sw = 2;
+    warps = (int)(sm_bytes / (sw * stage_bytes + pr.ntemp * slot + 64));
   }
+  const int reg_cap = z->d.prec == SU3_F64 ? 12 : 16;  // warps/SM the kernel's registers allow in whole CTAs of NCW warps
+  if (warps > reg_cap) warps = reg_cap;
+  if (warps < 1 || sw < 2) return fail(SU3_ERR_INVALID, "expression needs more shared memory than the device has (%d operands, %d temporaries)",
+                                       n_operands, pr.ntemp);
+  int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (warps + NCW - 1) / NCW;
+  int ncw = warps / ctas;
+  if (ncw > NCW) ncw = NCW;
+  if (ncw < 1) { ncw = 1; ctas = warps; }
+  const int stages = sw;
+  const size_t smem = (size_t)ncw * sw * stage_bytes + (size_t)ncw * pr.ntemp * slot + (size_t)ncw * sw * sizeof(uint64_t) + 16;
+  const int tm = mps;
   cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
   if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
   su3::ExprParams p;
   memset(&p, 0, sizeof p);
   p.z = z->ptr;
   for (int i = 0; i < n_operands; i++) p.ops[i] = operands[i]->ptr;
-  p.nmat = z->nmat; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp;
+  p.nmat = z->nmat; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.ncw = ncw;
   for (int i = 0; i < pr.nins; i++) p.ins[i] = pr.ins[i];
-  const int64_t ntiles = (z->nmat + tm - 1) / tm, max_grid = (int64_t)di.sms * ctas;
-  k<<<(unsigned)(ntiles < max_grid ? ntiles : max_grid), (NCW + 1) * 32, smem, (cudaStream_t)cuda_stream>>>(p);
+  const int64_t ntiles = (z->nmat + tm - 1) / tm, blocks_needed = (ntiles + ncw - 1) / ncw, max_grid = (int64_t)di.sms * ctas;
+  k<<<(unsigned)(blocks_needed < max_grid ? blocks_needed : max_grid), NCW * 32, smem, (cudaStream_t)cuda_stream>>>(p);
   e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_expr launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);

@@ -370,79 +370,79 @@ struct ExprParams {
   void *z;
   const void *ops[8];
   long long nmat;
-  int tile_mats, stages, nops, nins, ntemp, hint;
+  int tile_mats, stages, nops, nins, ntemp, hint;  // stages = ring depth PER consumer warp
+  int ncw;                                          // active consumer warps (<= NCW of the kernel)
   ExprIns ins[16];
 };
 
+// Pipeline granularity: unlike su3_pipe_kernel, every consumer WARP owns whole stages (tile k of the CTA goes
+// to consumer warp w = k % ncw and to stage (k / ncw) % SW of that warp's PRIVATE ring, so every mbarrier has one
+// waiting warp that sees its phases strictly in order), so ncw tiles are evaluated concurrently per CTA without
+// any barrier between warps.  Long programs are bound by the latency of the interpreter's LDS/FMA/STS chain per
+// tile, not by throughput (measured: 3 CTAs/SM of the CTA-wide design gave 6.85 instead of 5.47 TB/s on
+// `01+01*+`, but do not fit once there are more than two operands); warp-granular stages give that concurrency
+// without spending shared memory on it.  A stage holds MPS = 32 matrices per operand (one per lane): 4608 B
+// (fp64) / 2304 B (fp32) per bulk copy.  There is no producer warp: lane 0 of every warp issues the warp's own loads.
 template <typename R, int W, int NCW>
-__global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprParams p) {
+__global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams p) {
   typedef typename Cplx<R>::type C2;
   constexpr int CB = (int)sizeof(C2);
+  constexpr int MPS = 32;
   extern __shared__ __align__(128) unsigned char smem[];
-  const int TM = p.tile_mats, S = p.stages, NIN = p.nops;
-  const uint32_t slot_bytes = (uint32_t)TM * 9u * CB;
+  const int SW = p.stages, ncw = p.ncw, S = SW * ncw, NIN = p.nops;
+  constexpr uint32_t slot_bytes = (uint32_t)MPS * 9u * CB;
   const uint32_t stage_bytes = NIN * slot_bytes;
-  unsigned char *temps = smem + (size_t)S * stage_bytes;
-  uint64_t *full = reinterpret_cast<uint64_t *>(temps + (size_t)p.ntemp * slot_bytes);
-  uint64_t *empty = full + S;
+  unsigned char *temps = smem + (size_t)S * stage_bytes;  // [ncw][ntemp] slots, private to a warp
+  uint64_t *full = reinterpret_cast<uint64_t *>(temps + (size_t)ncw * p.ntemp * slot_bytes);
   const int tid = threadIdx.x;
-  const long long ntiles = (p.nmat + TM - 1) / TM;
-  if (tid == 0) {
-    for (int s = 0; s < S; s++) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], 1);
-    }
+  const long long ntiles = (p.nmat + MPS - 1) / MPS;
+  // every warp is a self-contained pipeline: lane 0 issues the bulk loads of the warp's own tiles into the
+  // warp's private ring of SW stages and re-arms a stage as soon as the warp's store has read it
+  const int lane = tid & 31, w = tid >> 5;
+  if (w >= ncw) return;
+  unsigned char *mytemps = temps + (size_t)w * p.ntemp * slot_bytes;
+  const long long gw = (long long)blockIdx.x * ncw + w, GW = (long long)gridDim.x * ncw;
+  const long long mine = ntiles > gw ? (ntiles - gw + GW - 1) / GW : 0;  // my tiles: gw, gw + GW, ...
+  auto load = [&](long long j) {  // lane 0 only
+    const int s = w * SW + (int)(j % SW);
+    const long long m0 = (gw + j * GW) * MPS;
+    const long long left = p.nmat - m0;
+    const int nm = left < MPS ? (int)left : MPS;
+    const uint32_t bytes = (uint32_t)nm * 9u * CB;
+    const uint32_t b16 = bytes & ~15u;
+    unsigned char *st = smem + (size_t)s * stage_bytes;
+    const size_t goff = (size_t)m0 * 9u * CB;
+    if (bytes != b16)
+      for (int o = 0; o < NIN; o++)
+        *reinterpret_cast<uint64_t *>(st + o * slot_bytes + b16) =
+            *reinterpret_cast<const uint64_t *>((const unsigned char *)p.ops[o] + goff + b16);
+    mbar_arrive_expect_tx(&full[s], NIN * b16);
+    for (int o = 0; o < NIN; o++)
+      bulk_g2s(st + o * slot_bytes, (const unsigned char *)p.ops[o] + goff, b16, &full[s]);
+  };
+  if (lane == 0) {
+    for (int q = 0; q < SW; q++) mbar_init(&full[w * SW + q], 1);
     fence_mbar_init();
     fence_proxy_async();
+    for (long long j = 0; j < mine && j < SW; j++) load(j);
   }
-  __syncthreads();
-
-  if (tid >= NCW * 32) {
-    if (tid == NCW * 32) {
-      int s = 0;
-      uint32_t ph = 0;
-      for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        mbar_wait(&empty[s], ph ^ 1u);
-        const long long m0 = tile * TM;
-        const long long left = p.nmat - m0;
-        const int nm = left < TM ? (int)left : TM;
-        const uint32_t bytes = (uint32_t)nm * 9u * CB;
-        const uint32_t b16 = bytes & ~15u;
-        unsigned char *st = smem + (size_t)s * stage_bytes;
-        const size_t goff = (size_t)m0 * 9u * CB;
-        if (bytes != b16)
-          for (int o = 0; o < NIN; o++)
-            *reinterpret_cast<uint64_t *>(st + o * slot_bytes + b16) =
-                *reinterpret_cast<const uint64_t *>((const unsigned char *)p.ops[o] + goff + b16);
-        mbar_arrive_expect_tx(&full[s], NIN * b16);
-        for (int o = 0; o < NIN; o++)
-          bulk_g2s(st + o * slot_bytes, (const unsigned char *)p.ops[o] + goff, b16, &full[s]);
-        if (++s == S) {
-          s = 0;
-          ph ^= 1u;
-        }
-      }
-    }
-    return;
-  }
-
-  const int t = tid;
-  const int base = (t / W) * 9 * W + (t % W);
-  int s = 0, prev_s = -1;
-  uint32_t ph = 0;
-  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const long long m0 = tile * TM;
+  __syncwarp();
+  for (long long j = 0; j < mine; j++) {
+    const int s = w * SW + (int)(j % SW);
+    const long long m0 = (gw + j * GW) * MPS;
     const long long left = p.nmat - m0;
-    const int nm = left < TM ? (int)left : TM;
+    const int nm = left < MPS ? (int)left : MPS;
     unsigned char *st = smem + (size_t)s * stage_bytes;
-    mbar_wait(&full[s], ph);
-    if (t < nm) {
+    mbar_wait(&full[s], (uint32_t)((j / SW) & 1));
+#pragma unroll 1
+    for (int t = lane; t < nm; t += 32) {
+      const int base = (t / W) * 9 * W + (t % W);
       C2 acc[9], a[9], b[9];
 #pragma unroll 1
       for (int i = 0; i < p.nins; i++) {
         const ExprIns in = p.ins[i];
         if (in.spill != EX_NONE) {
-          C2 *sp = reinterpret_cast<C2 *>(temps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + base;
+          C2 *sp = reinterpret_cast<C2 *>(mytemps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + base;
 #pragma unroll
           for (int e = 0; e < 9; e++) sp[e * W] = acc[e];
         }
@@ -451,7 +451,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprP
           for (int e = 0; e < 9; e++) a[e] = acc[e];
         } else {
           const C2 *sa = reinterpret_cast<const C2 *>(in.a < EX_TEMP0 ? st + in.a * slot_bytes
-                                                                     : temps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + base;
+                                                                     : mytemps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + base;
 #pragma unroll
           for (int e = 0; e < 9; e++) a[e] = sa[e * W];
         }
@@ -461,7 +461,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprP
             for (int e = 0; e < 9; e++) b[e] = acc[e];
           } else {
             const C2 *sb = reinterpret_cast<const C2 *>(in.b < EX_TEMP0 ? st + in.b * slot_bytes
-                                                                       : temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
+                                                                       : mytemps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
 #pragma unroll
             for (int e = 0; e < 9; e++) b[e] = sb[e * W];
           }
@@ -490,24 +490,20 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 2) su3_expr_kernel(const ExprP
       for (int e = 0; e < 9; e++) so[e * W] = acc[e];
     }
     fence_proxy_async();
-    named_bar_sync(1, NCW * 32);
-    if (t == 0) {
+    __syncwarp();
+    if (lane == 0) {
       const uint32_t bytes = (uint32_t)nm * 9u * CB;
       const uint32_t b16 = bytes & ~15u;
       unsigned char *zdst = (unsigned char *)p.z + (size_t)m0 * 9u * CB;
       bulk_s2g(zdst, st, b16);
       bulk_commit();
       if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(st + b16);
-      bulk_wait_read<1>();
-      if (prev_s >= 0) mbar_arrive(&empty[prev_s]);
+      bulk_wait_read<0>();  // the store has read the stage: refill it with my tile j + SW
+      if (j + SW < mine) load(j + SW);
     }
-    prev_s = s;
-    if (++s == S) {
-      s = 0;
-      ph ^= 1u;
-    }
+    __syncwarp();
   }
-  if (t == 0) bulk_wait_all<0>();
+  if (lane == 0) bulk_wait_all<0>();
 }
 
 // ---------------------------------------------------------------- y = U.psi on colour vectors (f4)
