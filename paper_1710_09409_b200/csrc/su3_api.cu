@@ -386,6 +386,17 @@ template <typename R, int OP, typename IT> shift_kernel_t shift_for_w(int W) {
   }
   return nullptr;
 }
+template <typename R, typename IT> shift_kernel_t cshift_async_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_cshift_async_kernel<R, 1, IT>;
+    case 2: return su3::su3_cshift_async_kernel<R, 2, IT>;
+    case 4: return su3::su3_cshift_async_kernel<R, 4, IT>;
+    case 8: return su3::su3_cshift_async_kernel<R, 8, IT>;
+    case 16: return su3::su3_cshift_async_kernel<R, 16, IT>;
+    case 32: return su3::su3_cshift_async_kernel<R, 32, IT>;
+  }
+  return nullptr;
+}
 template <typename IT> shift_kernel_t shift_pick(int prec, int op, int W) {
   if (prec == SU3_F64) return op == su3::SH_MUL ? shift_for_w<double, su3::SH_MUL, IT>(W) : shift_for_w<double, su3::SH_COPY, IT>(W);
   return op == su3::SH_MUL ? shift_for_w<float, su3::SH_MUL, IT>(W) : shift_for_w<float, su3::SH_COPY, IT>(W);
@@ -418,6 +429,21 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   {
     std::lock_guard<std::mutex> lk(g_tune_mu);
     tn = g_tune;
+  }
+  if (op == su3::SH_COPY && tn.path != 2) {  // cp.async gather + TMA store (path = 2 keeps the register version)
+    const bool small = (z->nmat + 64) * 9 < 0x7fffffffLL;
+    shift_kernel_t ka = d.prec == SU3_F64 ? (small ? cshift_async_for_w<double, int>(d.W) : cshift_async_for_w<double, long long>(d.W))
+                                          : (small ? cshift_async_for_w<float, int>(d.W) : cshift_async_for_w<float, long long>(d.W));
+    if (!ka) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
+    const size_t smem_a = 4 * 18432;
+    cudaError_t ea = allow_max_smem((const void *)ka, di.smem_optin);
+    if (ea != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", ea);
+    const int64_t nwt_a = (z->nmat + 31) / 32, need = (nwt_a + 3) / 4, cap_a = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (d.prec == SU3_F64 ? 6 : 3));  // 3 resident per SM; measured
+    ka<<<(unsigned)(need < cap_a ? need : cap_a), 128, smem_a, (cudaStream_t)stream>>>(p);
+    ea = cudaGetLastError();
+    if (ea != cudaSuccess) return cuda_fail("cshift kernel launch", ea);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return SU3_OK;
   }
   const int64_t nwt = (z->nmat + 31) / 32;
   int wpb = 4;

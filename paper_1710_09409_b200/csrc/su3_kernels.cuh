@@ -789,6 +789,95 @@ __global__ void __launch_bounds__(128, OP == SH_COPY ? (sizeof(R) == 4 ? 12 : 8)
   }
 }
 
+// Cshift without registers in the data path: every warp GATHERS its tile with per-lane cp.async (LDGSTS, 16 B
+// for fp64 / 8 B for fp32 complex numbers, addresses as in su3_shift_kernel) into a private ring of NS stages
+// and STORES each finished tile with one TMA bulk copy (the destination tile is contiguous).  The register
+// version above is latency-bound (ncu: 55-67 % DRAM, throughput proportional to resident blocks); here the
+// bytes in flight are bounded by shared memory instead: 12 warps x (NS-2) tiles per SM.
+__device__ __forceinline__ void cp_async_c2(double2 *dst_smem, const double2 *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_c2(float2 *dst_smem, const float2 *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+template <typename R, int W, typename IT>
+__global__ void __launch_bounds__(128, 3) su3_cshift_async_kernel(const ShiftParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int CB = (int)sizeof(C2);
+  constexpr int NS = sizeof(R) == 8 ? 4 : 8;  // 18.4 KB ring per warp either way
+  constexpr int D = NS - 2;                   // a tile is stored D iterations after its gather was issued
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
+  C2 *ring = reinterpret_cast<C2 *>(smem) + (size_t)wib * NS * 288;
+  const IT nwt = (IT)((p.nmat + 31) / 32);
+  const IT ostride = (IT)p.ostride;
+  const C2 *gy = reinterpret_cast<const C2 *>(p.y);
+  unsigned char *gz = reinterpret_cast<unsigned char *>(p.z);
+  const IT gw = (IT)blockIdx.x * wpb + wib, GW = (IT)gridDim.x * wpb;
+  const IT mine = nwt > gw ? (nwt - gw + GW - 1) / GW : 0;
+  for (IT j = 0; j < mine + D; j++) {
+    if (j < mine) {
+      // stage j % NS was last used by tile j - NS, whose bulk store must have finished reading it
+      if (lane == 0) bulk_wait_read<1>();
+      __syncwarp();
+      const IT wt = gw + j * GW;
+      const IT left = (IT)p.nmat - wt * 32;
+      const int nm = left < 32 ? (int)left : 32;
+      const int nc = nm * 9;
+      IT srcbase = 0;
+      if (lane < nm) {
+        const IT g = wt * 32 + lane;
+        const IT rec = g / W;
+        const int l = (int)(g % W);
+        const IT o = rec / p.nl;
+        const int mu = (int)(rec - o * p.nl);
+        const int oc = (int)((o / ostride) % p.rd);
+        const int ic = (l / p.lstride) % p.simd_d;
+        int xn = ic * p.rd + oc + p.disp;
+        if (xn >= p.Ld) xn -= p.Ld;
+        const int icn = xn / p.rd, ocn = xn - icn * p.rd;
+        const IT on = o + (IT)(ocn - oc) * ostride;
+        const int ln = l + (icn - ic) * p.lstride;
+        srcbase = ((on * p.nl + mu) * 9) * W + ln;
+      }
+      C2 *st = ring + (size_t)(j % NS) * 288;
+#pragma unroll
+      for (int jj = 0; jj < 9; jj++) {
+        const int idx = jj * 32 + lane;
+        const int q = idx / (9 * W), rem = idx - q * 9 * W;
+        const int e = rem / W, l = rem - e * W;
+        const IT sb = __shfl_sync(0xffffffffu, srcbase, q * W + l);
+        if (idx < nc) cp_async_c2(st + idx, gy + sb + e * W);
+      }
+    }
+    cp_async_commit();  // one group per iteration, empty past the last tile, so that the count below is uniform
+    if (j >= D) {
+      const IT t = j - D;  // its gather is complete once at most D younger groups are pending
+      cp_async_wait<D>();
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) {
+        const IT wt = gw + t * GW;
+        const IT left = (IT)p.nmat - wt * 32;
+        const int nm = left < 32 ? (int)left : 32;
+        const uint32_t bytes = (uint32_t)nm * 9u * CB, b16 = bytes & ~15u;
+        const C2 *st = ring + (size_t)(t % NS) * 288;
+        unsigned char *dst = gz + (size_t)wt * 288 * CB;
+        if (b16) bulk_s2g(dst, st, b16);
+        bulk_commit();
+        if (bytes != b16)
+          *reinterpret_cast<uint64_t *>(dst + b16) = *reinterpret_cast<const uint64_t *>((const unsigned char *)st + b16);
+      }
+    }
+  }
+  if (lane == 0) bulk_wait_all<0>();
+}
+
 // ---------------------------------------------------------------- streaming ceilings (A6) and z = x + y
 // dst = src as a pure TMA pipeline: one thread per CTA moves tiles global -> shared -> global with
 // 1-D bulk copies through a ring of `stages` slots; no register ever holds data.  The ceiling the
