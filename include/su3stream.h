@@ -192,6 +192,14 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *cuda_stream);
 su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host,
                         su3_field *zd, su3_field *xd, su3_field *yd, int chunks, void *cuda_stream);
 
+/* The same chunked, copy/compute-overlapped pipeline for the three ahead-of-time expressions, with operands that
+ * may already be resident: op = SU3_OP_MUL (z = x*y), SU3_OP_MUL3 (z = x*y*u), SU3_OP_MUL_ADD (z = x*y + u).  A NULL
+ * x_host / y_host / u_host means "that operand is already in its device field" (no copy); a NULL z_host leaves the
+ * result in zd only.  u_host and ud must be NULL for SU3_OP_MUL.  Otherwise as su3_mul_host. */
+typedef enum { SU3_OP_MUL = 0, SU3_OP_MUL3 = 1, SU3_OP_MUL_ADD = 2 } su3_op;
+su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
+                         su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream);
+
 /* Launch knobs (see su3_tune).  su3_tune_set(NULL) restores the defaults. */
 su3_status su3_tune_set(const su3_tune *t);
 su3_status su3_tune_get(su3_tune *out);

@@ -16,7 +16,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
-           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_cshift", "su3_mul_shift", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_tune_set",
+           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_cshift", "su3_mul_shift", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info"]
 
 
@@ -65,6 +65,7 @@ def _load():
         "su3_convert": (i32, [vp, vp, vp]),
         "su3_copy": (i32, [vp, vp, vp]),
         "su3_mul_host": (i32, [vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]),
+        "su3_eval_host": (i32, [ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]),
         "su3_tune_set": (i32, [T]),
         "su3_tune_get": (i32, [T]),
         "su3_launch_count": (i64, []),
@@ -244,6 +245,20 @@ def su3_mul_host(z_host, x_host, y_host, zd, xd, yd, chunks=0, stream=None):
         return ctypes.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
     _ck(lib.su3_mul_host(hp(z_host), hp(x_host), hp(y_host), zd.handle, xd.handle, yd.handle, int(chunks),
                          _stream(stream)))
+
+
+SU3_OP_MUL, SU3_OP_MUL3, SU3_OP_MUL_ADD = 0, 1, 2
+
+
+def su3_eval_host(op, z_host, x_host, y_host, u_host, zd, xd, yd, ud, chunks=0, stream=None):
+    """chunked H2D -> op -> D2H; a host argument of None means the operand is already resident (or, for z_host,
+    that the result stays on the device)"""
+    def hp(a):
+        if a is None:
+            return None
+        return ctypes.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+    _ck(lib.su3_eval_host(int(op), hp(z_host), hp(x_host), hp(y_host), hp(u_host), zd.handle, xd.handle, yd.handle,
+                          ud.handle if ud is not None else None, int(chunks), _stream(stream)))
 
 
 def su3_tune_set(tile_mats=0, stages=0, ctas_per_sm=0, l2_hint=0, path=0):

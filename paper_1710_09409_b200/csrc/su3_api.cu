@@ -904,11 +904,13 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   return SU3_OK;
 }
 
-su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su3_field *zd, su3_field *xd,
-                        su3_field *yd, int chunks, void *cuda_stream) {
-  if (!z_host || !x_host || !y_host) return fail(SU3_ERR_NULL, "host pointer is NULL");
-  su3_status st = check_arith(zd, xd, yd, nullptr, false);
+su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
+                         su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream) {
+  if (op != SU3_OP_MUL && op != SU3_OP_MUL3 && op != SU3_OP_MUL_ADD) return fail(SU3_ERR_INVALID, "op = %d not in {0,1,2}", op);
+  const bool has_u = op != SU3_OP_MUL;
+  su3_status st = check_arith(zd, xd, yd, ud, has_u);
   if (st != SU3_OK) return st;
+  if (!has_u && (u_host || ud)) return fail(SU3_ERR_INVALID, "SU3_OP_MUL takes no third operand");
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   cudaStream_t user = (cudaStream_t)cuda_stream;
@@ -924,7 +926,7 @@ su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su
   const int64_t nchunks = nmat ? (nmat + per - 1) / per : 0;
   std::lock_guard<std::mutex> lk(g_hp.mu);
   cudaError_t e = g_hp.ensure((size_t)(2 * nchunks + 2));
-  if (e != cudaSuccess) return cuda_fail("su3_mul_host stream/event setup", e);
+  if (e != cudaSuccess) return cuda_fail("su3_eval_host stream/event setup", e);
   cudaEvent_t ev_start = g_hp.ev[0], ev_done = g_hp.ev[1];
 #define SU3_CK(call)                                         \
   do {                                                       \
@@ -939,21 +941,28 @@ su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su
     const int64_t nm = (nmat - m0 < per) ? nmat - m0 : per;
     const size_t off = (size_t)m0 * mat_bytes, len = (size_t)nm * mat_bytes;
     cudaEvent_t ev_in = g_hp.ev[2 + 2 * c], ev_k = g_hp.ev[3 + 2 * c];
-    SU3_CK(cudaMemcpyAsync((char *)xd->ptr + off, (const char *)x_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
-    SU3_CK(cudaMemcpyAsync((char *)yd->ptr + off, (const char *)y_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
+    if (x_host) SU3_CK(cudaMemcpyAsync((char *)xd->ptr + off, (const char *)x_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
+    if (y_host) SU3_CK(cudaMemcpyAsync((char *)yd->ptr + off, (const char *)y_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
+    if (u_host) SU3_CK(cudaMemcpyAsync((char *)ud->ptr + off, (const char *)u_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
     SU3_CK(cudaEventRecord(ev_in, g_hp.h2d));
     SU3_CK(cudaStreamWaitEvent(user, ev_in, 0));
-    st = launch_stream(su3::OP_MUL, prec, W, (char *)zd->ptr + off, (const char *)xd->ptr + off,
-                       (const char *)yd->ptr + off, nullptr, nm, 3 * zd->nbytes, user);
+    st = launch_stream(op, prec, W, (char *)zd->ptr + off, (const char *)xd->ptr + off, (const char *)yd->ptr + off,
+                       has_u ? (const char *)ud->ptr + off : nullptr, nm, (has_u ? 4 : 3) * zd->nbytes, user);
     if (st != SU3_OK) return st;
     SU3_CK(cudaEventRecord(ev_k, user));
     SU3_CK(cudaStreamWaitEvent(g_hp.d2h, ev_k, 0));
-    SU3_CK(cudaMemcpyAsync((char *)z_host + off, (const char *)zd->ptr + off, len, cudaMemcpyDeviceToHost, g_hp.d2h));
+    if (z_host) SU3_CK(cudaMemcpyAsync((char *)z_host + off, (const char *)zd->ptr + off, len, cudaMemcpyDeviceToHost, g_hp.d2h));
   }
   SU3_CK(cudaEventRecord(ev_done, g_hp.d2h));
   SU3_CK(cudaStreamWaitEvent(user, ev_done, 0));
 #undef SU3_CK
   return SU3_OK;
+}
+
+su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su3_field *zd, su3_field *xd,
+                        su3_field *yd, int chunks, void *cuda_stream) {
+  if (!z_host || !x_host || !y_host) return fail(SU3_ERR_NULL, "host pointer is NULL");
+  return su3_eval_host(SU3_OP_MUL, z_host, x_host, y_host, nullptr, zd, xd, yd, nullptr, chunks, cuda_stream);
 }
 
 su3_status su3_tune_set(const su3_tune *t) {

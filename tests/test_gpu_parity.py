@@ -220,3 +220,32 @@ def test_mul_host_end_to_end():
             torch.cuda.synchronize()
             err, _ = rel_err(hz.numpy(), oracle.mul(geom_of(desc), x, y), su3.su3_desc_normalize(desc).W)
             assert err <= TOL[desc.prec]
+
+
+def test_eval_host_resident_operands_and_fused_ops():
+    desc = su3.make_desc((8, 8, 8, 10), prec=F32, layout=VE, W=8)
+    Wn = 8
+    x, y, w = (host_field(desc, 37, f) for f in (su3gen.FIELD_X, su3gen.FIELD_Y, su3gen.FIELD_W))
+    v = host_field(desc, 37, su3gen.FIELD_V, kind="gauss")
+    hx, hy, hw, hv = (torch.from_numpy(a).pin_memory() for a in (x, y, w, v))
+    hz = torch.empty_like(hx).pin_memory()
+    zd, xd, yd, ud = (su3.alloc_field(desc) for _ in range(4))
+    g = geom_of(desc)
+    # everything from the host
+    su3.su3_eval_host(su3.SU3_OP_MUL3, hz, hx, hy, hw, zd, xd, yd, ud, chunks=3)
+    torch.cuda.synchronize()
+    assert rel_err(hz.numpy(), oracle.mul3(g, x, y, w), Wn)[0] <= TOL[F32]
+    # x, y already resident (left there by the call above); only v travels; result also stays on the device
+    hz.zero_()
+    su3.su3_eval_host(su3.SU3_OP_MUL_ADD, hz, None, None, hv, zd, xd, yd, ud, chunks=0)
+    torch.cuda.synchronize()
+    ref = oracle.mul_add(g, x, y, v)
+    assert rel_err(hz.numpy(), ref, Wn)[0] <= TOL[F32]
+    assert np.array_equal(download(zd), hz.numpy())
+    su3.su3_eval_host(su3.SU3_OP_MUL, None, None, None, None, zd, xd, yd, None, chunks=2)
+    assert rel_err(download(zd), oracle.mul(g, x, y), Wn)[0] <= TOL[F32]
+    for bad in (lambda: su3.su3_eval_host(7, hz, hx, hy, None, zd, xd, yd, None),
+                lambda: su3.su3_eval_host(su3.SU3_OP_MUL, hz, hx, hy, hw, zd, xd, yd, ud)):
+        with pytest.raises(su3.Su3Error) as e:
+            bad()
+        assert e.value.status in (su3.SU3_ERR_INVALID, su3.SU3_ERR_MISMATCH)
