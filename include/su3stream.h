@@ -79,14 +79,18 @@ typedef struct {
 
 typedef struct su3_field su3_field; /* opaque: validated descriptor + device pointer */
 
-/* Launch knobs of the streaming pipeline (process-wide; 0 = library default).
- * They never change results, only speed; bench.py and the tests use them to pin
- * the launch configuration that is being measured. */
+/* Launch knobs (process-wide; 0 = library default).  They never change results, only speed; bench.py and the
+ * tests use them to pin the launch configuration that is being measured.  Meaning per kernel family:
+ *   pipeline (su3_mul/mul3/mul_add/add, su3_matvec): tile_mats, stages = ring depth, ctas_per_sm, l2_hint, path
+ *   su3_copy: tile = tile_mats x matrix bytes, stages, ctas_per_sm, l2_hint; path = 2 selects the plain LDG copy
+ *   su3_expr (interpreted programs): stages = ring depth per warp (2..), ctas_per_sm; the tile is 32 matrices
+ *   su3_cshift / su3_mul_shift: ctas_per_sm = blocks per SM of the grid; path = 2 selects the register Cshift
+ *   su3_convert: path = 2 selects the unstaged kernel for fp32 */
 typedef struct {
   int32_t tile_mats;    /* matrices per pipeline tile: 32, 64 or 128 (su3_copy: x matrix bytes) */
   int32_t stages;       /* shared-memory ring depth, 2..16                             */
   int32_t ctas_per_sm;  /* persistent CTAs per SM, 1..8                                 */
-  int32_t l2_hint;      /* 0 auto (by footprint), 1 none, 2 evict_first loads+stores   */
+  int32_t l2_hint;      /* 0 auto (= none), 1 none, 2 evict_first loads+stores         */
   int32_t path;         /* 0 auto (by footprint and layout), 1 TMA-bulk pipeline, 2 direct per-lane LDG, 3 warp-staged */
   int32_t reserved[3];
 } su3_tune;

@@ -208,9 +208,7 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
 
   su3::StreamParams p;
   p.z = z; p.x = x; p.y = y; p.u = u; p.nmat = nmat;
-  int hint = tn.l2_hint;
-  if (hint == 0) hint = (footprint_bytes > (size_t)di.l2) ? 1 : 1;  // auto: no hint (measured: DESIGN.md section 6)
-  p.hint = (hint == 2) ? 1 : 0;
+  p.hint = tn.l2_hint == 2 ? 1 : 0;  // auto = no hint: evict_first measured neutral (+-0.5 %) at every size, DESIGN.md 6.1
 
   if (warp) {
     p.tile_mats = 32; p.stages = 0;
