@@ -100,3 +100,46 @@ def test_expr_errors_launch_nothing():
         su3.su3_expr(a, "0+", [a])
     assert e.value.status == su3.SU3_ERR_INVALID
     assert su3.su3_launch_count() == n0
+
+
+def _random_program(rng, n_ops, n_operators):
+    """a random valid postfix program that uses every operand 0..n_ops-1 (and more pushes as needed)"""
+    pushes = n_operators + 1
+    leaves = list(range(n_ops)) + [int(rng.integers(0, n_ops)) for _ in range(pushes - n_ops)]
+    rng.shuffle(leaves)
+    prog, depth, li, ops_left = [], 0, 0, n_operators
+    while li < len(leaves) or ops_left:
+        can_push = li < len(leaves) and depth < 8
+        can_op = depth >= 2 and ops_left
+        if can_push and (not can_op or rng.random() < 0.55):
+            prog.append(str(leaves[li])); li += 1; depth += 1
+        else:
+            prog.append("+-*"[int(rng.integers(0, 3))]); depth -= 1; ops_left -= 1
+    return "".join(prog)
+
+
+@pytest.mark.parametrize("prec,layout,W", [(F64, SC, 1), (F32, VE, 8), (F64, VE, 4)])
+def test_expr_random_programs_fuzz(prec, layout, W):
+    """random trees (deep stacks, several live temporaries, repeated operands) against the oracle's stack machine"""
+    rng = np.random.default_rng(20251104 + W)
+    desc = su3.make_desc((4, 4, 6, 4), prec=prec, layout=layout, W=W)
+    g = geom_of(desc)
+    hosts = [host_field(desc, 71, f) for f in range(6)]          # SU(3): products keep unit scale
+    fs = [upload(desc, h) for h in hosts]
+    z = su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    seen_temps = 0
+    for _ in range(60):
+        n_ops = int(rng.integers(1, 7))
+        n_operators = int(rng.integers(max(1, n_ops - 1), 13))
+        prog = _random_program(rng, n_ops, n_operators)
+        st, fl = su3.su3_expr_cost(prog, n_ops)
+        assert st == n_ops + 1 and fl == 198 * prog.count("*") + 18 * (prog.count("+") + prog.count("-"))
+        z.tensor.fill_(0xFF)
+        su3.su3_expr(z, prog, fs[:n_ops])
+        got, ref = download(z), oracle.expr(g, prog, *hosts[:n_ops])
+        # relative to the largest entry of the result field: x - x style cancellations make per-matrix norms meaningless
+        scale = max(np.abs(ref).max(), 1.0)
+        assert np.isfinite(got).all() and np.abs(got - ref).max() / scale <= 50 * TOL[prec], prog
+        seen_temps += prog.count("*") > 2
+    assert seen_temps > 10
