@@ -249,3 +249,51 @@ def test_eval_host_resident_operands_and_fused_ops():
         with pytest.raises(su3.Su3Error) as e:
             bad()
         assert e.value.status in (su3.SU3_ERR_INVALID, su3.SU3_ERR_MISMATCH)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", [((3, 3, 3, 3), 1, SC, 1), ((5, 3, 1, 7), 1, SC, 1), ((6, 2, 10, 2), 4, VE, 8),
+                                           ((2, 2, 2, 2), 4, VE, 16), ((4, 6, 4, 8), 1, VE, 4)])
+def test_no_write_outside_the_output_field(prec, L, nl, layout, W):
+    """compute-sanitizer is not available on the GPU pool: every kernel family writes its result into a field that
+    sits between two canary bands, for ragged sizes and every path, and the bands must come back untouched"""
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    ds = scalar_desc(desc)
+    nb, nvb, G = su3.su3_field_bytes(desc), su3.su3_vec_bytes(desc), 4096
+    buf = torch.empty(nb + 2 * G, dtype=torch.uint8, device="cuda")
+
+    def guarded(kind="matrix", d=desc):
+        buf.fill_(0xA5)
+        n = nb if kind == "matrix" else nvb
+        wrap = su3.su3_field_wrap if kind == "matrix" else su3.su3_vec_wrap
+        return wrap(d, buf[G:G + n]), n
+
+    def intact(n, what):
+        torch.cuda.synchronize()
+        assert bool((buf[:G] == 0xA5).all()) and bool((buf[G + n:] == 0xA5).all()), what
+
+    x, y, w = (upload(desc, host_field(desc, 83, f)) for f in (0, 1, 2))
+    xs = upload(ds, host_field(ds, 83, 0))
+    psi = su3.alloc_vec(desc)
+    psi.tensor.zero_()
+    for path in (0, 1, 2, 3):
+        su3.su3_tune_set(path=path)
+        for name, call in [("mul", lambda z: su3.su3_mul(z, x, y)), ("mul3", lambda z: su3.su3_mul3(z, x, y, w)),
+                           ("mul_add", lambda z: su3.su3_mul_add(z, x, y, w)), ("add", lambda z: su3.su3_add(z, x, y)),
+                           ("copy", lambda z: su3.su3_copy(z, x)), ("expr", lambda z: su3.su3_expr(z, "01+01*+2-", [x, y, w])),
+                           ("cshift", lambda z: su3.su3_cshift(z, x, 3, 1)), ("cshift0", lambda z: su3.su3_cshift(z, x, 0, -1)),
+                           ("mul_shift", lambda z: su3.su3_mul_shift(z, x, y, 2, 1))]:
+            z, n = guarded()
+            call(z)
+            intact(n, (name, path))
+        if layout == VE:
+            z, n = guarded()
+            su3.su3_convert(z, xs)
+            intact(n, ("convert s->v", path))
+            z, n = guarded(d=ds)
+            su3.su3_convert(z, x)
+            intact(n, ("convert v->s", path))
+        z, n = guarded("vector")
+        su3.su3_matvec(z, x, psi)
+        intact(n, ("matvec", path))
+    su3.su3_tune_set()
