@@ -494,6 +494,25 @@ def run_next_rows(args, r):
             out["shift"].append({"dim": dim, "disp": 1, "layout": lay, "cshift_GBps": 2 * nb / (mn * 1e-3) / 1e9,
                                  "mul_shift_GBps": 3 * nb / (mn2 * 1e-3) / 1e9,
                                  "mul_shift_GFLOPps": FLOPS["mul"] * Ln ** 4 / (mn2 * 1e-3) / 1e9})
+    # BASELINE.json configs[2] and configs[3] as bench points (their parity is in tests/test_gpu_fullsize.py)
+    out["configs"] = []
+    if args.L >= 48:
+        d3s, d3v = su3.make_desc(32, n_lorentz=4), su3.make_desc(32, n_lorentz=4, layout=1, W=W64)
+        nb3 = su3.su3_field_bytes(d3s)
+        for d3, lay, (a_, b_) in ((d3s, "scalar", ("xs", "ys")), (d3v, "vector W=%d" % W64, ("xv", "yv"))):
+            fa, fb, fz = (su3.su3_field_wrap(d3, f[n_].tensor[:nb3]) for n_ in (a_, b_, "zc"))
+            mn, _, _ = time_calls(torch, lambda: su3.su3_mul(fz, fa, fb))
+            out["configs"].append({"config": "cfg3: 32^4 x 4 Lorentz fp64, mul, " + lay, "GBps": 3 * nb3 / (mn * 1e-3) / 1e9,
+                                   "GFLOPps": FLOPS["mul"] * 4 * 32 ** 4 / (mn * 1e-3) / 1e9})
+        d4 = su3.make_desc(48, prec=su3.SU3_F32, layout=1, W=W32)
+        nb4 = su3.su3_field_bytes(d4)
+        f4 = [su3.su3_field_wrap(d4, f[n_].tensor[:nb4]) for n_ in ("xv", "yv", "wv", "zc")]   # fp64 bytes read as fp32:
+        for fld in f4[:3]:                                                                      # make them finite numbers
+            fld.tensor.view(torch.float32).normal_()
+        for opn, fn in (("mul3", su3.su3_mul3), ("mul_add", su3.su3_mul_add)):
+            mn, _, _ = time_calls(torch, lambda: fn(f4[3], f4[0], f4[1], f4[2]))
+            out["configs"].append({"config": "cfg4: 48^4 fp32 vector W=%d, %s" % (W32, opn), "GBps": 4 * nb4 / (mn * 1e-3) / 1e9,
+                                   "GFLOPps": FLOPS[opn] * 48 ** 4 / (mn * 1e-3) / 1e9})
     # f4: colour vectors, y = U.psi (66 flops, 240 B fp64 / 120 B fp32 per site)
     out["matvec"] = []
     for prec, layout, W in ((8, 0, 1), (8, 1, W64), (4, 0, 1), (4, 1, W32)):
