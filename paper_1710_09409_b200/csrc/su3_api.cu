@@ -12,7 +12,7 @@
 #include <new>
 #include <vector>
 
-#include "su3_kernels.cuh"
+#include "su3_tables.h"
 
 struct su3_field {
   su3_desc d;  // normalised
@@ -24,6 +24,11 @@ struct su3_field {
 };
 
 namespace {
+
+using su3tab::NCW;
+using su3tab::expr_kernel_t;
+using su3tab::shift_kernel_t;
+using su3tab::stream_kernel_t;
 
 thread_local char g_err[512] = "";
 std::atomic<int64_t> g_launches{0};
@@ -112,61 +117,6 @@ const DevInfo &devinfo() {
 }
 
 // ---------------------------------------------------------------- kernel tables
-typedef void (*stream_kernel_t)(const su3::StreamParams);
-constexpr int NCW = 4;  // consumer warps per CTA of the pipeline kernel (tile <= 128 matrices)
-
-template <typename R, int OP> stream_kernel_t pipe_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_pipe_kernel<R, 1, OP, NCW>;
-    case 2: return su3::su3_pipe_kernel<R, 2, OP, NCW>;
-    case 4: return su3::su3_pipe_kernel<R, 4, OP, NCW>;
-    case 8: return su3::su3_pipe_kernel<R, 8, OP, NCW>;
-    case 16: return su3::su3_pipe_kernel<R, 16, OP, NCW>;
-    case 32: return su3::su3_pipe_kernel<R, 32, OP, NCW>;
-  }
-  return nullptr;
-}
-template <typename R, int OP> stream_kernel_t direct_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_direct_kernel<R, 1, OP>;
-    case 2: return su3::su3_direct_kernel<R, 2, OP>;
-    case 4: return su3::su3_direct_kernel<R, 4, OP>;
-    case 8: return su3::su3_direct_kernel<R, 8, OP>;
-    case 16: return su3::su3_direct_kernel<R, 16, OP>;
-    case 32: return su3::su3_direct_kernel<R, 32, OP>;
-  }
-  return nullptr;
-}
-template <typename R, int OP> stream_kernel_t warp_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_warp_kernel<R, 1, OP>;
-    case 2: return su3::su3_warp_kernel<R, 2, OP>;
-    case 4: return su3::su3_warp_kernel<R, 4, OP>;
-    case 8: return su3::su3_warp_kernel<R, 8, OP>;
-    case 16: return su3::su3_warp_kernel<R, 16, OP>;
-    case 32: return su3::su3_warp_kernel<R, 32, OP>;
-  }
-  return nullptr;
-}
-template <typename R> stream_kernel_t pick_warp(int op, int W) {
-  switch (op) {
-    case su3::OP_MUL: return warp_for_w<R, su3::OP_MUL>(W);
-    case su3::OP_MUL3: return warp_for_w<R, su3::OP_MUL3>(W);
-    case su3::OP_MUL_ADD: return warp_for_w<R, su3::OP_MUL_ADD>(W);
-    case su3::OP_ADD: return warp_for_w<R, su3::OP_ADD>(1);
-  }
-  return nullptr;
-}
-template <typename R> stream_kernel_t pick(int op, int W, bool direct) {
-  switch (op) {
-    case su3::OP_MUL: return direct ? direct_for_w<R, su3::OP_MUL>(W) : pipe_for_w<R, su3::OP_MUL>(W);
-    case su3::OP_MUL3: return direct ? direct_for_w<R, su3::OP_MUL3>(W) : pipe_for_w<R, su3::OP_MUL3>(W);
-    case su3::OP_MUL_ADD: return direct ? direct_for_w<R, su3::OP_MUL_ADD>(W) : pipe_for_w<R, su3::OP_MUL_ADD>(W);
-    case su3::OP_ADD: return direct ? nullptr : pipe_for_w<R, su3::OP_ADD>(1);  // element-wise: layout-agnostic
-  }
-  return nullptr;
-}
-
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and process, not once per launch
 cudaError_t allow_max_smem(const void *fn, int bytes) {
   static std::mutex mu;
@@ -202,8 +152,8 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   const bool direct = tn.path == 2 || (tn.path == 0 && op != su3::OP_ADD && W * cb >= 32 &&
                                        footprint_bytes <= (size_t)di.l2 / 5 * 3);
   const bool warp = !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
-  stream_kernel_t k = warp ? ((prec == SU3_F64) ? pick_warp<double>(op, W) : pick_warp<float>(op, W))
-                           : ((prec == SU3_F64) ? pick<double>(op, W, direct) : pick<float>(op, W, direct));
+  const int family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
+  stream_kernel_t k = prec == SU3_F64 ? su3tab::stream_f64(family, op, W) : su3tab::stream_f32(family, op, W);
   if (!k) return fail(SU3_ERR_INVALID, "no kernel for op %d prec %d W %d", op, prec, W);
 
   su3::StreamParams p;
@@ -358,48 +308,7 @@ su3_status compile_expr(const char *prog, int nops, ExprProgram *out) {
   return SU3_OK;
 }
 
-typedef void (*expr_kernel_t)(const su3::ExprParams);
-template <typename R> expr_kernel_t expr_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_expr_kernel<R, 1, NCW>;
-    case 2: return su3::su3_expr_kernel<R, 2, NCW>;
-    case 4: return su3::su3_expr_kernel<R, 4, NCW>;
-    case 8: return su3::su3_expr_kernel<R, 8, NCW>;
-    case 16: return su3::su3_expr_kernel<R, 16, NCW>;
-    case 32: return su3::su3_expr_kernel<R, 32, NCW>;
-  }
-  return nullptr;
-}
-
 // ---------------------------------------------------------------- Cshift / shifted product
-typedef void (*shift_kernel_t)(const su3::ShiftParams);
-template <typename R, int OP, typename IT> shift_kernel_t shift_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_shift_kernel<R, 1, OP, IT>;
-    case 2: return su3::su3_shift_kernel<R, 2, OP, IT>;
-    case 4: return su3::su3_shift_kernel<R, 4, OP, IT>;
-    case 8: return su3::su3_shift_kernel<R, 8, OP, IT>;
-    case 16: return su3::su3_shift_kernel<R, 16, OP, IT>;
-    case 32: return su3::su3_shift_kernel<R, 32, OP, IT>;
-  }
-  return nullptr;
-}
-template <typename R, typename IT> shift_kernel_t cshift_async_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_cshift_async_kernel<R, 1, IT>;
-    case 2: return su3::su3_cshift_async_kernel<R, 2, IT>;
-    case 4: return su3::su3_cshift_async_kernel<R, 4, IT>;
-    case 8: return su3::su3_cshift_async_kernel<R, 8, IT>;
-    case 16: return su3::su3_cshift_async_kernel<R, 16, IT>;
-    case 32: return su3::su3_cshift_async_kernel<R, 32, IT>;
-  }
-  return nullptr;
-}
-template <typename IT> shift_kernel_t shift_pick(int prec, int op, int W) {
-  if (prec == SU3_F64) return op == su3::SH_MUL ? shift_for_w<double, su3::SH_MUL, IT>(W) : shift_for_w<double, su3::SH_COPY, IT>(W);
-  return op == su3::SH_MUL ? shift_for_w<float, su3::SH_MUL, IT>(W) : shift_for_w<float, su3::SH_COPY, IT>(W);
-}
-
 su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
   if (!z || !y || (op == su3::SH_MUL && !x)) return fail(SU3_ERR_NULL, "field handle is NULL");
   if (!same_desc(z->d, y->d) || (x && !same_desc(z->d, x->d))) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
@@ -421,7 +330,7 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   p.Ld = d.L[dim]; p.simd_d = d.simd[dim]; p.rd = d.L[dim] / d.simd[dim];
   p.disp = ((disp % p.Ld) + p.Ld) % p.Ld;
   // 32-bit index arithmetic whenever every complex index (plus one tile of slack) fits 31 bits
-  shift_kernel_t k = (z->nmat + 64) * 9 < 0x7fffffffLL ? shift_pick<int>(d.prec, op, d.W) : shift_pick<long long>(d.prec, op, d.W);
+  shift_kernel_t k = su3tab::shift_kernel(d.prec, op, d.W, (z->nmat + 64) * 9 < 0x7fffffffLL);
   if (!k) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
   su3_tune tn;
   {
@@ -430,8 +339,7 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   }
   if (op == su3::SH_COPY && tn.path != 2) {  // cp.async gather + TMA store (path = 2 keeps the register version)
     const bool small = (z->nmat + 64) * 9 < 0x7fffffffLL;
-    shift_kernel_t ka = d.prec == SU3_F64 ? (small ? cshift_async_for_w<double, int>(d.W) : cshift_async_for_w<double, long long>(d.W))
-                                          : (small ? cshift_async_for_w<float, int>(d.W) : cshift_async_for_w<float, long long>(d.W));
+    shift_kernel_t ka = su3tab::cshift_async_kernel(d.prec, d.W, small);
     if (!ka) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
     const size_t smem_a = 4 * 18432;
     cudaError_t ea = allow_max_smem((const void *)ka, di.smem_optin);
@@ -459,18 +367,6 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
 }
 
 // ---------------------------------------------------------------- y = U.psi
-template <typename R> stream_kernel_t matvec_for_w(int W) {
-  switch (W) {
-    case 1: return su3::su3_matvec_kernel<R, 1, NCW>;
-    case 2: return su3::su3_matvec_kernel<R, 2, NCW>;
-    case 4: return su3::su3_matvec_kernel<R, 4, NCW>;
-    case 8: return su3::su3_matvec_kernel<R, 8, NCW>;
-    case 16: return su3::su3_matvec_kernel<R, 16, NCW>;
-    case 32: return su3::su3_matvec_kernel<R, 32, NCW>;
-  }
-  return nullptr;
-}
-
 // ---------------------------------------------------------------- su3_mul_host resources
 struct HostPipe {
   std::mutex mu;
@@ -643,7 +539,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
     tn = g_tune;
   }
   const int cb = 2 * z->d.prec;
-  expr_kernel_t k = z->d.prec == SU3_F64 ? expr_for_w<double>(z->d.W) : expr_for_w<float>(z->d.W);
+  expr_kernel_t k = su3tab::expr_kernel(z->d.prec, z->d.W);
   if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", z->d.W);
   // Every warp is a self-contained pipeline with a private ring of `sw` stages of 32 matrices per operand.  Long programs are latency-bound per tile, so the launch maximises resident warps per SM
   // under the shared-memory budget (ring depth 2, 3 if there is room for >= 8 warps anyway), at most 16.
@@ -728,7 +624,7 @@ su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, vo
     tn = g_tune;
   }
   const int cb = 2 * y->d.prec;
-  stream_kernel_t k = y->d.prec == SU3_F64 ? matvec_for_w<double>(y->d.W) : matvec_for_w<float>(y->d.W);
+  stream_kernel_t k = su3tab::matvec_kernel(y->d.prec, y->d.W);
   if (!k) return fail(SU3_ERR_INVALID, "no matvec kernel for W %d", y->d.W);
   // measured (48^4): ~110 KB in flight per SM is the sweet spot -> 2 CTAs/SM of 24.6 KB stages (fp64), 4 of 12.3 KB (fp32)
   const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (y->d.prec == SU3_F64 ? 2 : 4);
@@ -859,43 +755,10 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   }
   if (p.nrec == 0) return SU3_OK;
   const su3_tune tn_c = [] { std::lock_guard<std::mutex> lk(g_tune_mu); return g_tune; }();
-  if (v.prec == SU3_F32 && tn_c.path != 2) {  // staged through shared memory: 256-byte requests on both sides
-    cudaStream_t s = (cudaStream_t)stream;
-#define SU3_STAGED(WW, TRR)                                                                                        \
-  case WW: {                                                                                                       \
-    const long long blocks = (p.nrec + TRR - 1) / TRR;                                                             \
-    if (blocks > 0x7fffffffLL) return fail(SU3_ERR_SIZE, "su3_convert: lattice too large for one launch");         \
-    const size_t smem = sizeof(float2) * TRR * nc * (WW + 1) + sizeof(long long) * TRR;                                  \
-    if (nc == 9) su3::su3_convert_staged_kernel<float2, WW, TRR, 9><<<(unsigned)blocks, 256, smem, s>>>(p);        \
-    else su3::su3_convert_staged_kernel<float2, WW, TRR, 3><<<(unsigned)blocks, 256, smem, s>>>(p);                \
-  } break;
-    switch (v.W) {
-      SU3_STAGED(1, 64) SU3_STAGED(2, 64) SU3_STAGED(4, 64) SU3_STAGED(8, 64) SU3_STAGED(16, 32) SU3_STAGED(32, 16)
-      default: return fail(SU3_ERR_INVALID, "su3_convert: W = %d", v.W);
-    }
-#undef SU3_STAGED
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return SU3_OK;
-  }
-  constexpr int TR = 64;
-  const long long blocks = (p.nrec + TR - 1) / TR;
-  if (blocks > 0x7fffffffLL) return fail(SU3_ERR_SIZE, "su3_convert: lattice too large for one launch");
-  cudaStream_t s = (cudaStream_t)stream;
-  const unsigned grid = (unsigned)blocks;
-#define SU3_CONVERT_CASE(WW)                                                                     \
-  case WW:                                                                                       \
-    if (v.prec == SU3_F64 && nc == 9) su3::su3_convert_kernel<double2, WW, TR, 9><<<grid, 256, 0, s>>>(p);      \
-    else if (v.prec == SU3_F64) su3::su3_convert_kernel<double2, WW, TR, 3><<<grid, 256, 0, s>>>(p);            \
-    else if (nc == 9) su3::su3_convert_kernel<float2, WW, TR, 9><<<grid, 256, 0, s>>>(p);                       \
-    else su3::su3_convert_kernel<float2, WW, TR, 3><<<grid, 256, 0, s>>>(p);                                    \
-    break;
-  switch (v.W) {
-    SU3_CONVERT_CASE(1) SU3_CONVERT_CASE(2) SU3_CONVERT_CASE(4) SU3_CONVERT_CASE(8) SU3_CONVERT_CASE(16) SU3_CONVERT_CASE(32)
-    default: return fail(SU3_ERR_INVALID, "su3_convert: W = %d", v.W);
-  }
-#undef SU3_CONVERT_CASE
+  // fp32: staged through shared memory (256-byte requests on both sides); path = 2 forces the unstaged kernel
+  const char *err = nullptr;
+  if (!su3tab::launch_convert(v.prec, nc, v.W, v.prec == SU3_F32 && tn_c.path != 2, p, (cudaStream_t)stream, &err))
+    return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);

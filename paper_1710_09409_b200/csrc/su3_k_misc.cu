@@ -1,0 +1,42 @@
+// instantiations of the expression, matvec and layout-conversion kernels; see su3_tables.h
+#include "su3_tables.h"
+namespace su3tab {
+expr_kernel_t expr_kernel(int prec, int W) { return prec == 8 ? expr_for_w<double>(W) : expr_for_w<float>(W); }
+stream_kernel_t matvec_kernel(int prec, int W) { return prec == 8 ? matvec_for_w<double>(W) : matvec_for_w<float>(W); }
+
+bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertParams &p, cudaStream_t s, const char **err) {
+  if (staged) {
+#define SU3_STAGED(WW, TRR)                                                                                  \
+  case WW: {                                                                                                 \
+    const long long blocks = (p.nrec + TRR - 1) / TRR;                                                       \
+    if (blocks > 0x7fffffffLL) { *err = "lattice too large for one launch"; return false; }                  \
+    const size_t smem = sizeof(float2) * TRR * nc * (WW + 1) + sizeof(long long) * TRR;                      \
+    if (nc == 9) su3::su3_convert_staged_kernel<float2, WW, TRR, 9><<<(unsigned)blocks, 256, smem, s>>>(p);  \
+    else su3::su3_convert_staged_kernel<float2, WW, TRR, 3><<<(unsigned)blocks, 256, smem, s>>>(p);          \
+  } return true;
+    switch (W) {
+      SU3_STAGED(1, 64) SU3_STAGED(2, 64) SU3_STAGED(4, 64) SU3_STAGED(8, 64) SU3_STAGED(16, 32) SU3_STAGED(32, 16)
+    }
+#undef SU3_STAGED
+    *err = "unsupported W";
+    return false;
+  }
+  constexpr int TR = 64;
+  const long long blocks = (p.nrec + TR - 1) / TR;
+  if (blocks > 0x7fffffffLL) { *err = "lattice too large for one launch"; return false; }
+  const unsigned grid = (unsigned)blocks;
+#define SU3_CONVERT_CASE(WW)                                                                           \
+  case WW:                                                                                             \
+    if (prec == 8 && nc == 9) su3::su3_convert_kernel<double2, WW, TR, 9><<<grid, 256, 0, s>>>(p);     \
+    else if (prec == 8) su3::su3_convert_kernel<double2, WW, TR, 3><<<grid, 256, 0, s>>>(p);           \
+    else if (nc == 9) su3::su3_convert_kernel<float2, WW, TR, 9><<<grid, 256, 0, s>>>(p);              \
+    else su3::su3_convert_kernel<float2, WW, TR, 3><<<grid, 256, 0, s>>>(p);                           \
+    return true;
+  switch (W) {
+    SU3_CONVERT_CASE(1) SU3_CONVERT_CASE(2) SU3_CONVERT_CASE(4) SU3_CONVERT_CASE(8) SU3_CONVERT_CASE(16) SU3_CONVERT_CASE(32)
+  }
+#undef SU3_CONVERT_CASE
+  *err = "unsupported W";
+  return false;
+}
+}  // namespace su3tab

@@ -1,0 +1,5 @@
+// fp32 instantiations of the streaming kernels (pipeline, direct, warp-staged); see su3_tables.h
+#include "su3_tables.h"
+namespace su3tab {
+stream_kernel_t stream_f32(int family, int op, int W) { return stream_any<float>(family, op, W); }
+}  // namespace su3tab

@@ -891,7 +891,7 @@ struct CopyParams {
   int hint;
 };
 
-__global__ void __launch_bounds__(32) su3_bulk_copy_kernel(const CopyParams p) {
+static __global__ void __launch_bounds__(32) su3_bulk_copy_kernel(const CopyParams p) {
   extern __shared__ __align__(128) unsigned char smem[];
   if (threadIdx.x != 0) return;
   const int S = p.stages;
@@ -945,7 +945,7 @@ __global__ void __launch_bounds__(32) su3_bulk_copy_kernel(const CopyParams p) {
 
 // dst = src over n16 16-byte words (+ an optional 8-byte tail), 4 independent 128-bit loads
 // in flight per thread (path = 2: the plain LDG/STG copy, kept as the measured comparison).
-__global__ void __launch_bounds__(256) su3_copy_kernel(uint4 *__restrict__ dst, const uint4 *__restrict__ src,
+static __global__ void __launch_bounds__(256) su3_copy_kernel(uint4 *__restrict__ dst, const uint4 *__restrict__ src,
                                                        size_t n16, int tail8) {
   const size_t bd = blockDim.x;
   const size_t stride = (size_t)gridDim.x * bd * 4;
