@@ -677,22 +677,20 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *s
   return SU3_OK;
 }
 
-su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
-  if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
-  if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds");
+static su3_status launch_copy(void *dst_ptr, const void *src_ptr, size_t nbytes, int prec, void *stream) {
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
-  if (dst->nbytes == 0) return SU3_OK;
+  if (nbytes == 0) return SU3_OK;
   su3_tune tn;
   {
     std::lock_guard<std::mutex> lk(g_tune_mu);
     tn = g_tune;
   }
   if (tn.path != 2) {  // TMA bulk pipeline: global -> shared -> global, one issuing thread per CTA
-    const int mat_bytes = 18 * dst->d.prec;
+    const int mat_bytes = 18 * prec;
     const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 3;
     unsigned tile = tn.tile_mats > 0 ? (unsigned)tn.tile_mats * mat_bytes : 18432u;  // multiple of 16
-    const size_t n16 = dst->nbytes & ~(size_t)15;
+    const size_t n16 = nbytes & ~(size_t)15;
     while (tile > 2304 && (n16 + tile - 1) / tile < (size_t)2 * di.sms * ctas) tile >>= 1;
     int stages = tn.stages > 0 ? tn.stages : 2;
     const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
@@ -702,22 +700,28 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
     cudaError_t e = allow_max_smem((const void *)su3::su3_bulk_copy_kernel, di.smem_optin);
     if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
     su3::CopyParams p;
-    p.dst = dst->ptr; p.src = src->ptr; p.nbytes = dst->nbytes; p.tile_bytes = tile; p.stages = stages;
+    p.dst = dst_ptr; p.src = src_ptr; p.nbytes = nbytes; p.tile_bytes = tile; p.stages = stages;
     p.hint = tn.l2_hint == 2;
     size_t ntiles = (n16 + tile - 1) / tile;
     if (ntiles < 1) ntiles = 1;
     const size_t cap = (size_t)di.sms * ctas;
     su3::su3_bulk_copy_kernel<<<(unsigned)(ntiles < cap ? ntiles : cap), 32, smem, (cudaStream_t)stream>>>(p);
   } else {
-    const size_t n16 = dst->nbytes / 16;
-    const int tail8 = (dst->nbytes % 16) ? 1 : 0;
+    const size_t n16 = nbytes / 16;
+    const int tail8 = (nbytes % 16) ? 1 : 0;
     const unsigned grid = flat_grid(n16, 1024, 8);
-    su3::su3_copy_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((uint4 *)dst->ptr, (const uint4 *)src->ptr, n16, tail8);
+    su3::su3_copy_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((uint4 *)dst_ptr, (const uint4 *)src_ptr, n16, tail8);
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_copy launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return SU3_OK;
+}
+
+su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
+  if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds");
+  return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);
 }
 
 su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
@@ -728,6 +732,8 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   if (dst->ptr == src->ptr) return fail(SU3_ERR_MISMATCH, "su3_convert: dst and src must not alias");
   if (dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_convert: matrix and vector fields cannot be mixed");
   const int nc = dst->ncomp;
+  if (dst->d.W == 1 && src->d.W == 1)  // the W = 1 vector layout is byte-identical to the scalar layout
+    return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   const su3_desc &v = (dst->d.layout == SU3_VECTOR) ? dst->d : src->d;

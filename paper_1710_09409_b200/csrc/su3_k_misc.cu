@@ -15,7 +15,7 @@ bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertPara
     else su3::su3_convert_staged_kernel<float2, WW, TRR, 3><<<(unsigned)blocks, 256, smem, s>>>(p);          \
   } return true;
     switch (W) {
-      SU3_STAGED(1, 64) SU3_STAGED(2, 64) SU3_STAGED(4, 64) SU3_STAGED(8, 64) SU3_STAGED(16, 32) SU3_STAGED(32, 16)
+      SU3_STAGED(1, 256) SU3_STAGED(2, 128) SU3_STAGED(4, 64) SU3_STAGED(8, 32) SU3_STAGED(16, 16) SU3_STAGED(32, 8)  // 18 KB tiles
     }
 #undef SU3_STAGED
     *err = "unsupported W";
