@@ -183,12 +183,21 @@ def run_ours(args, rank, world, local_rank):
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    ngpu = torch.cuda.device_count()
+    dev = torch.device("cuda", local_rank % ngpu)
+    torch.cuda.set_device(dev)
     dist = None
+    coll_dev = dev
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+        if ngpu >= world:
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            # fewer GPUs than ranks (a functional check of the N > 1 path only): ranks share GPUs, plumbing over gloo.
+            # No kernel of one rank ever waits for another rank, so sharing a GPU cannot deadlock.
+            log("[rank %d] %d GPU(s) for %d ranks: sharing devices, gloo plumbing -- NOT a scaling measurement" % (rank, ngpu, world))
+            dist.init_process_group("gloo")
+            coll_dev = torch.device("cpu")
 
     def barrier():
         if dist is not None:
@@ -253,7 +262,7 @@ def run_ours(args, rank, world, local_rank):
             events[len(rows)].record()
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps, per-launch events inside
-    clocks = ClockSampler(local_rank)   # sampled from here on: warm-up and timed steps are both under load
+    clocks = ClockSampler(dev.index)   # sampled from here on: warm-up and timed steps are both under load
     t_warm = time.perf_counter()
     nwarm = 0
     while nwarm < max(args.warmup, 3) or time.perf_counter() - t_warm < 0.6:
@@ -277,7 +286,7 @@ def run_ours(args, rank, world, local_rank):
     total_ms = evs[0][0].elapsed_time(evs[K - 1][len(rows)])
     row_ms = [float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)])) for i in range(len(rows))]
     # whole-job value: bytes of all ranks / max-over-ranks device time (independent shards, no collective)
-    rate, total_ms, _ = shard.job_throughput(K * step_bytes, total_ms, dist, dev)
+    rate, total_ms, _ = shard.job_throughput(K * step_bytes, total_ms, dist, coll_dev)
     ms_per_step = total_ms / K
     value = rate / 1e9
 
@@ -287,7 +296,7 @@ def run_ours(args, rank, world, local_rank):
         "vector_result_equals_scalar_result_bitwise": bool(torch.equal(f["zb"].tensor, f["zs"].tensor)),
         "copy_bitwise": bool(torch.equal(f["zc"].tensor, f["zs"].tensor)),
     }
-    return dict(torch=torch, su3=su3, dist=dist, dev=dev, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
+    return dict(torch=torch, su3=su3, dist=dist, dev=coll_dev, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
                 nmat=nmat, step_bytes=step_bytes, step_flops=step_flops, ms_per_step=ms_per_step, value=value,
                 launches=launches, clk=clk, checks=checks, info=info, t_wall=t_wall, barrier=barrier, step=step,
                 hbytes=hbytes)
@@ -574,6 +583,11 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    # torchrun exports OMP_NUM_THREADS=1; the host-side generator and the oracle (gcc/OpenMP libraries loaded later)
+    # should still use the box's cores: all of them for the reference arm (rank 0 alone works), a fair share otherwise
+    if world > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+        ncpu = os.cpu_count() or 1
+        os.environ["OMP_NUM_THREADS"] = str(ncpu if args.impl == "reference" else max(1, ncpu // world))
     if args.impl == "reference":
         run_reference(args, rank)
         return
