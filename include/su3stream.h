@@ -146,6 +146,12 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *c
 su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *operands, int n_operands,
                     void *cuda_stream);
 
+/* The register-machine listing the host compiler produces for `program` (what the interpreter kernel executes),
+ * one instruction per line: "<op> <a> <b> [spill tK]" with op in {mul, add, sub, copy}, sources oK = operand K,
+ * tK = temporary K, acc = accumulator; "spill tK" = the accumulator is parked in temporary K first.  Written
+ * NUL-terminated into buf (SU3_ERR_SIZE if it does not fit).  Host-only; for debugging and for the tests. */
+su3_status su3_expr_disasm(const char *program, int n_operands, char *buf, size_t buf_len);
+
 /* Accounting of a program by reading S9: field streams (n_operands + 1) and flops per matrix (198 per '*',
  * 18 per '+' or '-').  Validates the program like su3_expr.  Host-only. */
 su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix);

@@ -16,7 +16,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
-           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_cshift", "su3_mul_shift", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
+           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_cshift", "su3_mul_shift", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info"]
 
 
@@ -61,6 +61,7 @@ def _load():
         "su3_cshift": (i32, [vp, vp, ctypes.c_int, ctypes.c_int, vp]),
         "su3_mul_shift": (i32, [vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]),
         "su3_expr": (i32, [vp, ctypes.c_char_p, ctypes.POINTER(vp), ctypes.c_int, vp]),
+        "su3_expr_disasm": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.c_char_p, sz]),
         "su3_expr_cost": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.POINTER(i32), ctypes.POINTER(i32)]),
         "su3_convert": (i32, [vp, vp, vp]),
         "su3_copy": (i32, [vp, vp, vp]),
@@ -189,6 +190,17 @@ def su3_expr(z, program, operands, stream=None):
     """z = postfix `program` over `operands` (digits push operands[k]; '+', '-', '*'), one pass."""
     arr = (ctypes.c_void_p * len(operands))(*[o.handle.value for o in operands])
     _ck(lib.su3_expr(z.handle, program.encode(), arr, len(operands), _stream(stream)))
+
+
+def su3_expr_disasm(program, n_operands):
+    """the compiled register-machine listing, one (op, a, b, spill-or-None) tuple per instruction"""
+    buf = ctypes.create_string_buffer(2048)
+    _ck(lib.su3_expr_disasm(program.encode(), int(n_operands), buf, len(buf)))
+    out = []
+    for line in buf.value.decode().splitlines():
+        t = line.split()
+        out.append((t[0], t[1], t[2], t[4] if len(t) > 3 else None))
+    return out
 
 
 def su3_expr_cost(program, n_operands):

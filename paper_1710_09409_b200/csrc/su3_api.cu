@@ -490,6 +490,34 @@ su3_status su3_mul_add(su3_field *z, const su3_field *x, const su3_field *y, con
   return arith(su3::OP_MUL_ADD, z, x, y, v, s);
 }
 
+su3_status su3_expr_disasm(const char *program, int n_operands, char *buf, size_t buf_len) {
+  if (!buf) return fail(SU3_ERR_NULL, "buf is NULL");
+  ExprProgram pr;
+  su3_status st = compile_expr(program, n_operands, &pr);
+  if (st != SU3_OK) return st;
+  static const char *names[] = {"mul", "add", "sub", "copy"};
+  size_t used = 0;
+  auto src = [](unsigned char v, char *out) {
+    if (v == su3::EX_SRC_ACC) snprintf(out, 8, "acc");
+    else if (v >= su3::EX_TEMP0) snprintf(out, 8, "t%d", v - su3::EX_TEMP0);
+    else snprintf(out, 8, "o%d", v);
+  };
+  for (int i = 0; i < pr.nins; i++) {
+    char a[8], b[8] = "-", line[64];
+    src(pr.ins[i].a, a);
+    if (pr.ins[i].op != su3::EX_COPY) src(pr.ins[i].b, b);
+    int n = snprintf(line, sizeof line, "%s %s %s", names[pr.ins[i].op], a, b);
+    if (pr.ins[i].spill != su3::EX_NONE) n += snprintf(line + n, sizeof line - n, " spill t%d", pr.ins[i].spill - su3::EX_TEMP0);
+    n += snprintf(line + n, sizeof line - n, "\n");
+    if (used + n + 1 > buf_len) return fail(SU3_ERR_SIZE, "listing needs more than %zu bytes", buf_len);
+    memcpy(buf + used, line, n);
+    used += n;
+  }
+  if (buf_len == 0) return fail(SU3_ERR_SIZE, "empty buffer");
+  buf[used] = 0;
+  return SU3_OK;
+}
+
 su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix) {
   ExprProgram pr;
   su3_status st = compile_expr(program, n_operands, &pr);

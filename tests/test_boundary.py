@@ -155,3 +155,60 @@ def test_colour_vector_boundary_host_side():
     with pytest.raises(su3.Su3Error) as e:
         su3.su3_vec_index(d, 0, 0, 3, 0)
     assert e.value.status == su3.SU3_ERR_INVALID
+
+
+def _run_listing(listing, mats):
+    """execute the compiled register machine on one site with numpy (what the interpreter kernel does per thread)"""
+    import numpy as np
+    acc, temps = None, {}
+
+    def get(s):
+        return acc if s == "acc" else (temps[s] if s[0] == "t" else mats[int(s[1:])])
+    for op, a, b, spill in listing:
+        if spill is not None:
+            temps[spill] = acc
+        A = get(a)
+        B = get(b) if op != "copy" else None
+        acc = {"mul": lambda: A @ B, "add": lambda: A + B, "sub": lambda: A - B, "copy": lambda: A}[op]()
+    return np.array(acc)
+
+
+def _postfix(prog, mats):
+    st = []
+    for t in prog:
+        if t.isdigit():
+            st.append(mats[int(t)])
+        else:
+            b, a = st.pop(), st.pop()
+            st.append(a @ b if t == "*" else (a + b if t == "+" else a - b))
+    return st[0]
+
+
+def test_expr_compiler_listing_evaluates_like_the_postfix_program():
+    """host-only pin of the postfix -> register-machine compiler: known listings, and 300 random programs whose
+    listing, executed with numpy on random integer matrices, equals direct postfix evaluation exactly"""
+    import numpy as np
+    assert su3.su3_expr_disasm("01*2*", 3) == [("mul", "o0", "o1", None), ("mul", "acc", "o2", None)]
+    assert su3.su3_expr_disasm("01+01*+", 2) == [("add", "o0", "o1", None), ("mul", "o0", "o1", "t0"), ("add", "t0", "acc", None)]
+    assert su3.su3_expr_disasm("0", 1) == [("copy", "o0", "-", None)]
+    assert su3.su3_expr_disasm("012**", 3) == [("mul", "o1", "o2", None), ("mul", "o0", "acc", None)]
+    rng = np.random.default_rng(7)
+    mats = [rng.integers(-3, 4, (3, 3)).astype(np.int64).astype(object) for _ in range(8)]   # exact Python integers
+    deepest = 0
+    for _ in range(300):
+        n_ops = int(rng.integers(1, 9))
+        n_operators = int(rng.integers(max(1, n_ops - 1), 16))
+        leaves = list(range(n_ops)) + [int(rng.integers(0, n_ops)) for _ in range(n_operators + 1 - n_ops)]
+        rng.shuffle(leaves)
+        prog, depth, li, left = [], 0, 0, n_operators
+        while li < len(leaves) or left:
+            if li < len(leaves) and depth < 8 and (depth < 2 or not left or rng.random() < 0.6):
+                prog.append(str(leaves[li])); li += 1; depth += 1
+            else:
+                prog.append("+-*"[int(rng.integers(0, 3))]); depth -= 1; left -= 1
+        prog = "".join(prog)
+        listing = su3.su3_expr_disasm(prog, n_ops)
+        assert len(listing) == n_operators
+        deepest = max(deepest, len({sp for *_, sp in listing if sp}))
+        assert (_run_listing(listing, mats) == _postfix(prog, mats)).all(), prog
+    assert deepest >= 3  # programs with several live temporaries were among them
