@@ -350,6 +350,34 @@ int orc_convert_vec(const orc_geom *gd, const orc_geom *gs, int prec, void *dst,
   return 0;
 }
 
+/* ---- real scalar fields, the paper's own example of the expression engine (Listing 2):
+ *   Lattice<double> v1, v2, v3;  v1 = 1.0;  v2 = 2.0;  v3 = v1+v2;  v3 = v1+v2+v1*v2;
+ * One real per (site, mu); '+', '-', '*' act element-wise, so no layout map is involved: the field is just n
+ * reals.  Same postfix convention and the same validity rules as orc_expr; fp64 result. */
+int orc_expr_real(int64_t n, int prec, int nops, const void *const *ops, const char *prog, double *z) {
+  int depth = 0;
+  for (const char *t = prog; *t; t++) {
+    if (*t >= '0' && *t <= '7') { if (*t - '0' >= nops) return 2; if (++depth > 8) return 3; }
+    else if (*t == '+' || *t == '-' || *t == '*') { if (depth < 2) return 4; depth--; }
+    else return 1;
+  }
+  if (depth != 1) return 5;
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; i++) {
+    double st[8];
+    int sp = 0;
+    for (const char *t = prog; *t; t++) {
+      if (*t >= '0' && *t <= '7') st[sp++] = rd(ops[*t - '0'], prec, i);
+      else {
+        double b = st[--sp], a = st[--sp];
+        st[sp++] = *t == '+' ? a + b : (*t == '-' ? a - b : a * b);
+      }
+    }
+    z[i] = st[0];
+  }
+  return 0;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -51,6 +51,8 @@ def _load():
         lib.orc_matvec.restype = None
         lib.orc_convert_vec.argtypes = [P, P, I, V, V]
         lib.orc_convert_vec.restype = I
+        lib.orc_expr_real.argtypes = [I64, I, I, ctypes.POINTER(V), ctypes.c_char_p, V]
+        lib.orc_expr_real.restype = I
         lib.orc_convert.argtypes = [P, P, I, V, V]
         lib.orc_convert.restype = I
         lib.orc_num_threads.restype = I
@@ -194,6 +196,18 @@ def convert_vec(g_dst, g_src, src):
     if _load().orc_convert_vec(ctypes.byref(g_dst.c), ctypes.byref(g_src.c), src.dtype.itemsize, dst.ctypes.data, src.ctypes.data):
         raise ValueError("geometry mismatch")
     return dst
+
+
+def expr_real(prog, *ops):
+    """element-wise postfix expression over real scalar fields (flat fp32/fp64 arrays of equal length); fp64 result"""
+    n = ops[0].size
+    assert all(o.flags.c_contiguous and o.size == n and o.dtype == ops[0].dtype for o in ops)
+    z = np.empty(n, dtype=np.float64)
+    arr = (ctypes.c_void_p * len(ops))(*[o.ctypes.data for o in ops])
+    rc = _load().orc_expr_real(n, ops[0].dtype.itemsize, len(ops), arr, prog.encode(), z.ctypes.data)
+    if rc:
+        raise ValueError("malformed expression %r (orc_expr_real -> %d)" % (prog, rc))
+    return z
 
 
 def convert(g_dst, g_src, src):

@@ -439,3 +439,37 @@ def test_index_vec_is_a_bijection_and_matches_the_matrix_map():
     assert seen == set(range(g.nmat * 6))
     gs = oracle.Geom((4, 2, 2, 4), nl=4)
     assert oracle.index_vec(gs, 5, 3, 2, 1) == ((5 * 4 + 3) * 3 + 2) * 2 + 1
+
+
+# ---------------------------------------------------------------- real scalar fields: the paper's Listing 2
+def load_listing2():
+    import os
+    from helpers import GOLDEN
+    rows = []
+    with open(os.path.join(GOLDEN, "listing2_example.txt")) as f:
+        for line in f:
+            t = line.split("#")[0].split()
+            if t:
+                rows.append((t[0], float(t[1]), float(t[2]), float(t[3])))
+    return rows
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_expr_real_reproduces_the_papers_listing2(dtype):
+    n = 8 ** 4
+    for prog, a, b, want in load_listing2():
+        v1, v2 = np.full(n, a, dtype=dtype), np.full(n, b, dtype=dtype)
+        assert np.array_equal(oracle.expr_real(prog, v1, v2), np.full(n, want))
+
+
+def test_expr_real_against_numpy_and_rejects_malformed():
+    rng = np.random.default_rng(3)
+    a, b, c = (rng.standard_normal(1001) for _ in range(3))
+    assert np.array_equal(oracle.expr_real("01+01*+", a, b), (a + b) + a * b)
+    assert np.array_equal(oracle.expr_real("01*2-0+", a, b, c), (a * b - c) + a)
+    assert np.array_equal(oracle.expr_real("012-*", a, b, c), a * (b - c))
+    a32 = a.astype(np.float32)
+    assert np.array_equal(oracle.expr_real("00*", a32), a32.astype(np.float64) ** 2)   # promoted exactly, kept in fp64
+    for bad in ["", "0+", "00", "01*", "0a*"]:
+        with pytest.raises(ValueError):
+            oracle.expr_real(bad, a)
