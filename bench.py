@@ -522,6 +522,22 @@ def run_next_rows(args, r):
             mn, _, _ = time_calls(torch, lambda: fn(f4[3], f4[0], f4[1], f4[2]))
             out["configs"].append({"config": "cfg4: 48^4 fp32 vector W=%d, %s" % (W32, opn), "GBps": 4 * nb4 / (mn * 1e-3) / 1e9,
                                    "GFLOPps": FLOPS[opn] * 48 ** 4 / (mn * 1e-3) / 1e9})
+    # the paper's Listing 2 on real scalar fields: v3 = v1+v2 and v3 = v1+v2+v1*v2 (3 streams of 8 / 4 B per element)
+    out["listing2"] = []
+    for prec in (8, 4):
+        dr = su3.make_desc(Ln, n_lorentz=4, prec=prec)
+        nr = su3.su3_real_bytes(dr)
+        reps = max(1, (1 << 29) // nr)                       # batch enough copies of the field to stream >= 0.5 GB each
+        dbig = su3.make_desc((Ln, Ln, Ln, Ln * reps), n_lorentz=4, prec=prec)
+        nbig = su3.su3_real_bytes(dbig)
+        v1, v2, v3 = (su3.su3_real_wrap(dbig, f[n_].tensor[:nbig]) for n_ in ("xs", "ys", "zc"))
+        su3.su3_fill(v1, 1.0); su3.su3_fill(v2, 2.0)
+        for prog, flops in (("01+", 1), ("01+01*+", 3)):
+            mn, _, _ = time_calls(torch, lambda: su3.su3_expr(v3, prog, [v1, v2]))
+            ok = bool((v3.tensor.view(torch.float64 if prec == 8 else torch.float32) == (3.0 if prog == "01+" else 5.0)).all())
+            out["listing2"].append({"program": prog, "prec": "f64" if prec == 8 else "f32", "reals": nbig // prec,
+                                    "GBps": 3 * nbig / (mn * 1e-3) / 1e9, "GFLOPps": flops * (nbig // prec) / (mn * 1e-3) / 1e9,
+                                    "value_is_the_papers": ok})
     # f4: colour vectors, y = U.psi (66 flops, 240 B fp64 / 120 B fp32 per site)
     out["matvec"] = []
     for prec, layout, W in ((8, 0, 1), (8, 1, W64), (4, 0, 1), (4, 1, W32)):

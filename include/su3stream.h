@@ -182,6 +182,16 @@ su3_status su3_vec_index(const su3_desc *desc, int64_t site, int mu, int i, int 
  * colour-matrix field, psi and y colour-vector fields, identical descriptors.  y may be the same field as psi. */
 su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, void *cuda_stream);
 
+/* Real scalar fields, the operands of the paper's own example of the expression engine (Listing 2:
+ * `Lattice<double> v1, v2, v3; v1 = 1.0; v2 = 2.0; v3 = v1+v2+v1*v2;`): one real per (site, mu),
+ * su3_real_bytes = volume * n_lorentz * prec.  Element-wise operations only, so the layout of the descriptor
+ * does not matter.  A handle made by su3_real_wrap goes to su3_fill, su3_expr (all operands and z of real kind:
+ * '+', '-', '*' act element-wise) and su3_field_free/desc/ptr; every other call returns SU3_ERR_MISMATCH for it. */
+su3_status su3_real_bytes(const su3_desc *desc, size_t *nbytes);
+su3_status su3_real_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out);
+/* field = value at every (site, mu) (Listing 2: `v1 = 1.0;`).  Real scalar fields only. */
+su3_status su3_fill(su3_field *z, double value, void *cuda_stream);
+
 /* Layout conversion scalar <-> vector: a pure, bit-exact permutation of complex numbers,
  * vec[o][mu][e][l] = sca[site(o,l)][mu][e] (extract/merge).  Exactly one of
  * dst/src must be SU3_SCALAR and the other SU3_VECTOR; L, n_lorentz, prec must agree

@@ -16,7 +16,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
-           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_cshift", "su3_mul_shift", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
+           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info"]
 
 
@@ -54,6 +54,9 @@ def _load():
         "su3_mul3": (i32, [vp, vp, vp, vp, vp]),
         "su3_mul_add": (i32, [vp, vp, vp, vp, vp]),
         "su3_add": (i32, [vp, vp, vp, vp]),
+        "su3_real_bytes": (i32, [D, ctypes.POINTER(sz)]),
+        "su3_real_wrap": (i32, [D, vp, sz, ctypes.POINTER(vp)]),
+        "su3_fill": (i32, [vp, ctypes.c_double, vp]),
         "su3_vec_bytes": (i32, [D, ctypes.POINTER(sz)]),
         "su3_vec_wrap": (i32, [D, vp, sz, ctypes.POINTER(vp)]),
         "su3_vec_index": (i32, [D, i64, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(i64)]),
@@ -128,12 +131,12 @@ class Field:
         self.tensor = tensor  # keeps the memory alive as long as the handle
         self.kind = kind
         h = ctypes.c_void_p()
-        wrap = lib.su3_field_wrap if kind == "matrix" else lib.su3_vec_wrap
+        wrap = {"matrix": lib.su3_field_wrap, "vector": lib.su3_vec_wrap, "real": lib.su3_real_wrap}[kind]
         _ck(wrap(ctypes.byref(desc), ctypes.c_void_p(tensor.data_ptr()),
                  tensor.numel() * tensor.element_size(), ctypes.byref(h)))
         self.handle = h
         self.desc = su3_field_desc(self)
-        self.nbytes = su3_field_bytes(self.desc) if kind == "matrix" else su3_vec_bytes(self.desc)
+        self.nbytes = {"matrix": su3_field_bytes, "vector": su3_vec_bytes, "real": su3_real_bytes}[kind](self.desc)
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None
@@ -216,6 +219,25 @@ def su3_cshift(z, x, dim, disp, stream=None):
 
 def su3_mul_shift(z, x, y, dim, disp, stream=None):
     _ck(lib.su3_mul_shift(z.handle, x.handle, y.handle, int(dim), int(disp), _stream(stream)))
+
+
+def su3_real_bytes(desc):
+    n = ctypes.c_size_t()
+    _ck(lib.su3_real_bytes(ctypes.byref(desc), ctypes.byref(n)))
+    return n.value
+
+
+def su3_real_wrap(desc, tensor):
+    return Field(desc, tensor, kind="real")
+
+
+def alloc_real(desc, device="cuda"):
+    import torch
+    return Field(desc, torch.empty(su3_real_bytes(desc), dtype=torch.uint8, device=device), kind="real")
+
+
+def su3_fill(z, value, stream=None):
+    _ck(lib.su3_fill(z.handle, float(value), _stream(stream)))
 
 
 def su3_vec_bytes(desc):

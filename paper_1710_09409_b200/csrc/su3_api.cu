@@ -20,7 +20,7 @@ struct su3_field {
   size_t nbytes;
   int64_t volume;
   int64_t nmat;
-  int ncomp;  // complex numbers per (site, mu): 9 = colour matrix, 3 = colour vector
+  int ncomp;  // complex numbers per (site, mu): 9 = colour matrix, 3 = colour vector; 0 = real scalar field (1 real)
 };
 
 namespace {
@@ -411,7 +411,7 @@ static su3_status wrap_kind(const su3_desc *desc, void *dev_ptr, size_t nbytes, 
   if (st != SU3_OK) return st;
   if (!dev_ptr) return fail(SU3_ERR_NULL, "device pointer is NULL");
   if ((uintptr_t)dev_ptr & 15) return fail(SU3_ERR_ALIGN, "device pointer %p is not 16-byte aligned", dev_ptr);
-  const size_t need = (size_t)volume_of(d) * d.n_lorentz * 2 * ncomp * d.prec;
+  const size_t need = (size_t)volume_of(d) * d.n_lorentz * (ncomp ? 2 * ncomp : 1) * d.prec;  // ncomp = 0: one REAL per (site, mu)
   if (nbytes < need) return fail(SU3_ERR_SIZE, "buffer of %zu bytes is smaller than the %zu the field needs", nbytes, need);
   su3_field *f = new (std::nothrow) su3_field;
   if (!f) return fail(SU3_ERR_SIZE, "out of host memory");
@@ -427,6 +427,34 @@ su3_status su3_field_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su
 
 su3_status su3_vec_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
   return wrap_kind(desc, dev_ptr, nbytes, out, 3);
+}
+
+su3_status su3_real_wrap(const su3_desc *desc, void *dev_ptr, size_t nbytes, su3_field **out) {
+  return wrap_kind(desc, dev_ptr, nbytes, out, 0);
+}
+
+su3_status su3_real_bytes(const su3_desc *desc, size_t *nbytes) {
+  if (!nbytes) return fail(SU3_ERR_NULL, "nbytes is NULL");
+  su3_desc d;
+  su3_status st = normalize(desc, &d);
+  if (st != SU3_OK) return st;
+  *nbytes = (size_t)volume_of(d) * d.n_lorentz * d.prec;
+  return SU3_OK;
+}
+
+su3_status su3_fill(su3_field *z, double value, void *cuda_stream) {
+  if (!z) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (z->ncomp != 0) return fail(SU3_ERR_MISMATCH, "su3_fill takes a real scalar field");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (z->nmat == 0) return SU3_OK;
+  const unsigned grid = flat_grid((size_t)z->nmat, 256, 8);
+  if (z->d.prec == SU3_F64) su3::su3_real_fill_kernel<double><<<grid, 256, 0, (cudaStream_t)cuda_stream>>>((double *)z->ptr, z->nmat, value);
+  else su3::su3_real_fill_kernel<float><<<grid, 256, 0, (cudaStream_t)cuda_stream>>>((float *)z->ptr, z->nmat, (float)value);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_fill launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
 }
 
 su3_status su3_vec_bytes(const su3_desc *desc, size_t *nbytes) {
@@ -533,14 +561,40 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   ExprProgram pr;
   su3_status st = compile_expr(program, n_operands, &pr);
   if (st != SU3_OK) return st;
+  if (z->ncomp != 9 && z->ncomp != 0) return fail(SU3_ERR_MISMATCH, "su3_expr takes colour-matrix fields or real scalar fields");
   for (int k = 0; k < n_operands; k++) {
     if (!operands[k]) return fail(SU3_ERR_NULL, "operand %d is NULL", k);
-    if (!same_desc(z->d, operands[k]->d) || operands[k]->ncomp != 9 || z->ncomp != 9)
-      return fail(SU3_ERR_MISMATCH, "operand %d: descriptor differs from z (or not a colour-matrix field)", k);
+    if (!same_desc(z->d, operands[k]->d) || operands[k]->ncomp != z->ncomp)
+      return fail(SU3_ERR_MISMATCH, "operand %d: descriptor or field kind differs from z", k);
   }
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (z->nmat == 0) return SU3_OK;
+  const bool real = z->ncomp == 0;
+  // Real scalar fields (the paper's Listing 2) are element-wise, so n reals = n / 18 records of 18 reals for the
+  // matrix machinery below (W = 1; '*' becomes the element-wise EX_EMUL) plus a tail of n % 18 reals.
+  const int64_t nrec = real ? z->nmat / 18 : z->nmat;
+  const int W_eff = real ? 1 : z->d.W;
+  if (real) {
+    for (int i = 0; i < pr.nins; i++)
+      if (pr.ins[i].op == su3::EX_MUL) pr.ins[i].op = su3::EX_EMUL;
+    const int64_t ntail = z->nmat - nrec * 18;
+    if (ntail) {
+      su3::ExprParams pt;
+      memset(&pt, 0, sizeof pt);
+      const size_t off = (size_t)nrec * 18 * z->d.prec;
+      pt.z = (char *)z->ptr + off;
+      for (int i = 0; i < n_operands; i++) pt.ops[i] = (const char *)operands[i]->ptr + off;
+      pt.nmat = ntail; pt.nops = n_operands; pt.nins = pr.nins; pt.ntemp = pr.ntemp;
+      for (int i = 0; i < pr.nins; i++) pt.ins[i] = pr.ins[i];
+      if (z->d.prec == SU3_F64) su3::su3_real_expr_kernel<double><<<1, 32, 0, (cudaStream_t)cuda_stream>>>(pt);
+      else su3::su3_real_expr_kernel<float><<<1, 32, 0, (cudaStream_t)cuda_stream>>>(pt);
+      cudaError_t er = cudaGetLastError();
+      if (er != cudaSuccess) return cuda_fail("su3_expr (real tail) launch", er);
+      g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    if (nrec == 0) return SU3_OK;
+  }
   {
     // the fixed menu: programs that ARE one of the ahead-of-time kernels run on them (same FMA chain, so the
     // result is bit-identical either way; IEEE addition is commutative, so v + x*y is x*y + v)
@@ -548,7 +602,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
     const bool first_on_operands = in[0].a < su3::EX_TEMP0 && in[0].b < su3::EX_TEMP0;
     int op = -1;
     const su3_field *fx = nullptr, *fy = nullptr, *fu = nullptr;
-    if (pr.nins >= 1 && first_on_operands && in[0].op != su3::EX_SUB && in[0].op != su3::EX_COPY) {
+    if (pr.nins >= 1 && first_on_operands && (in[0].op == su3::EX_MUL || in[0].op == su3::EX_ADD) && (!real || pr.nins == 1)) {
       fx = operands[in[0].a]; fy = operands[in[0].b];
       if (pr.nins == 1) op = in[0].op == su3::EX_MUL ? su3::OP_MUL : su3::OP_ADD;
       else if (pr.nins == 2 && in[0].op == su3::EX_MUL && in[1].spill == su3::EX_NONE) {
@@ -558,7 +612,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
       }
     }
     if (op >= 0)
-      return launch_stream(op, z->d.prec, op == su3::OP_ADD ? 1 : z->d.W, z->ptr, fx->ptr, fy->ptr, fu ? fu->ptr : nullptr, z->nmat,
+      return launch_stream(op, z->d.prec, op == su3::OP_ADD ? 1 : W_eff, z->ptr, fx->ptr, fy->ptr, fu ? fu->ptr : nullptr, nrec,
                            z->nbytes * (fu ? 4 : 3), (cudaStream_t)cuda_stream);
   }
   su3_tune tn;
@@ -567,8 +621,8 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
     tn = g_tune;
   }
   const int cb = 2 * z->d.prec;
-  expr_kernel_t k = su3tab::expr_kernel(z->d.prec, z->d.W);
-  if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", z->d.W);
+  expr_kernel_t k = su3tab::expr_kernel(z->d.prec, W_eff);
+  if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", W_eff);
   // Every warp is a self-contained pipeline with a private ring of `sw` stages of 32 matrices per operand.  Long programs are latency-bound per tile, so the launch maximises resident warps per SM
   // under the shared-memory budget (ring depth 2, 3 if there is room for >= 8 warps anyway), at most 16.
   const int mps = 32;
@@ -598,9 +652,9 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   memset(&p, 0, sizeof p);
   p.z = z->ptr;
   for (int i = 0; i < n_operands; i++) p.ops[i] = operands[i]->ptr;
-  p.nmat = z->nmat; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.ncw = ncw;
+  p.nmat = nrec; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.ncw = ncw;
   for (int i = 0; i < pr.nins; i++) p.ins[i] = pr.ins[i];
-  const int64_t ntiles = (z->nmat + tm - 1) / tm, blocks_needed = (ntiles + ncw - 1) / ncw, max_grid = (int64_t)di.sms * ctas;
+  const int64_t ntiles = (nrec + tm - 1) / tm, blocks_needed = (ntiles + ncw - 1) / ncw, max_grid = (int64_t)di.sms * ctas;
   k<<<(unsigned)(blocks_needed < max_grid ? blocks_needed : max_grid), NCW * 32, smem, (cudaStream_t)cuda_stream>>>(p);
   e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_expr launch", e);
@@ -748,7 +802,8 @@ static su3_status launch_copy(void *dst_ptr, const void *src_ptr, size_t nbytes,
 
 su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
   if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
-  if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds");
+  if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp || dst->ncomp == 0)
+    return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds (matrix or vector)");
   return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);
 }
 
@@ -758,7 +813,7 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   if (dst->d.layout == src->d.layout)
     return fail(SU3_ERR_MISMATCH, "su3_convert: exactly one of dst/src must be SU3_SCALAR and the other SU3_VECTOR");
   if (dst->ptr == src->ptr) return fail(SU3_ERR_MISMATCH, "su3_convert: dst and src must not alias");
-  if (dst->ncomp != src->ncomp) return fail(SU3_ERR_MISMATCH, "su3_convert: matrix and vector fields cannot be mixed");
+  if (dst->ncomp != src->ncomp || dst->ncomp == 0) return fail(SU3_ERR_MISMATCH, "su3_convert: matrix and vector fields cannot be mixed; real scalar fields have no layout");
   const int nc = dst->ncomp;
   if (dst->d.W == 1 && src->d.W == 1)  // the W = 1 vector layout is byte-identical to the scalar layout
     return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);

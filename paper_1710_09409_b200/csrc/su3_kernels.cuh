@@ -362,7 +362,8 @@ __global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
 // accumulator.  The program is uniform over the grid, so the interpreter's branches never diverge.
 // Same pipeline as su3_pipe_kernel (TMA bulk in, TMA bulk out), same mat33_mul, hence bit-identical
 // to su3_mul / su3_mul3 / su3_mul_add on their three programs.
-enum { EX_MUL = 0, EX_ADD = 1, EX_SUB = 2, EX_COPY = 3, EX_SRC_ACC = 255, EX_NONE = 255, EX_TEMP0 = 8 };
+enum { EX_MUL = 0, EX_ADD = 1, EX_SUB = 2, EX_COPY = 3, EX_EMUL = 4,  // EMUL: element-wise product of the reals (real scalar fields)
+       EX_SRC_ACC = 255, EX_NONE = 255, EX_TEMP0 = 8 };
 struct ExprIns {
   unsigned char op, a, b, spill;  // sources: 0..7 operand slot, 8..15 temporary, 255 accumulator
 };
@@ -480,6 +481,12 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
             acc[e].x = add_rn(a[e].x, -b[e].x);
             acc[e].y = add_rn(a[e].y, -b[e].y);
           }
+        } else if (in.op == EX_EMUL) {
+#pragma unroll
+          for (int e = 0; e < 9; e++) {
+            acc[e].x = mul_rn(a[e].x, b[e].x);
+            acc[e].y = mul_rn(a[e].y, b[e].y);
+          }
         } else {
 #pragma unroll
           for (int e = 0; e < 9; e++) acc[e] = a[e];
@@ -504,6 +511,37 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
     __syncwarp();
   }
   if (lane == 0) bulk_wait_all<0>();
+}
+
+// ---------------------------------------------------------------- real scalar fields (Listing 2 of the paper)
+// `Lattice<double> v3 = v1+v2+v1*v2`: one real per (site, mu), element-wise, hence layout-agnostic.
+// A real field of n reals is evaluated as n / 18 records of 18 reals by the matrix machinery (su3_pipe_kernel's OP_ADD
+// for `a+b`, su3_expr_kernel with EX_EMUL for '*' otherwise: TMA in, TMA out); this plain kernel takes the n % 18 tail.
+template <typename R>
+__global__ void __launch_bounds__(32) su3_real_expr_kernel(const ExprParams p) {
+  for (long long i = threadIdx.x; i < p.nmat; i += blockDim.x) {  // one block: this is the tail of < 18 reals
+    R acc = 0, tmp[8];
+#pragma unroll 1
+    for (int k = 0; k < p.nins; k++) {
+      const ExprIns in = p.ins[k];
+      if (in.spill != EX_NONE) tmp[in.spill - EX_TEMP0] = acc;
+      auto fetch = [&](unsigned char srcid) -> R {
+        if (srcid == EX_SRC_ACC) return acc;
+        if (srcid >= EX_TEMP0) return tmp[srcid - EX_TEMP0];
+        return reinterpret_cast<const R *>(p.ops[srcid])[i];
+      };
+      const R a = fetch(in.a);
+      const R b = in.op != EX_COPY ? fetch(in.b) : R(0);
+      acc = (in.op == EX_MUL || in.op == EX_EMUL) ? mul_rn(a, b) : in.op == EX_ADD ? add_rn(a, b) : in.op == EX_SUB ? add_rn(a, -b) : a;
+    }
+    reinterpret_cast<R *>(p.z)[i] = acc;
+  }
+}
+
+// field = value (Listing 2: `v1 = 1.0;`)
+template <typename R> __global__ void __launch_bounds__(256) su3_real_fill_kernel(R *z, long long n, R value) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) z[i] = value;
 }
 
 // ---------------------------------------------------------------- y = U.psi on colour vectors (f4)
