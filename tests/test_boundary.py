@@ -212,3 +212,38 @@ def test_expr_compiler_listing_evaluates_like_the_postfix_program():
         deepest = max(deepest, len({sp for *_, sp in listing if sp}))
         assert (_run_listing(listing, mats) == _postfix(prog, mats)).all(), prog
     assert deepest >= 3  # programs with several live temporaries were among them
+
+
+def test_library_and_oracle_index_maps_agree_on_random_geometries():
+    """two independent implementations of readings S1-S6 (su3_index / su3_vec_index in the library, orc_index /
+    orc_index_vec in the oracle) must give the same offsets for random admissible geometries and custom splits"""
+    import numpy as np
+    import oracle
+    rng = np.random.default_rng(11)
+    checked = 0
+    while checked < 60:
+        W = int(2 ** rng.integers(0, 6))
+        simd, w = [1, 1, 1, 1], W
+        while w > 1:                       # random split of W over the dimensions
+            simd[int(rng.integers(0, 4))] *= 2
+            w //= 2
+        L = [int(s * rng.integers(1, 4)) for s in simd]
+        nl = int(rng.choice([1, 4]))
+        layout = su3.SU3_VECTOR if (W > 1 or rng.random() < 0.5) else su3.SU3_SCALAR
+        if layout == su3.SU3_SCALAR:
+            W, simd = 1, [1, 1, 1, 1]
+        d = su3.make_desc(L, n_lorentz=nl, layout=layout, W=W, simd=simd)
+        g = oracle.Geom(L, nl=nl, layout=layout, W=W, simd=simd)
+        V = int(np.prod(L))
+        seen = set()
+        for site in rng.integers(0, V, 12):
+            mu, i, j, c = int(rng.integers(0, nl)), int(rng.integers(0, 3)), int(rng.integers(0, 3)), int(rng.integers(0, 2))
+            off = su3.su3_index(d, int(site), mu, i, j, c)
+            assert off == oracle.index(g, int(site), mu, i, j, c)
+            assert su3.su3_vec_index(d, int(site), mu, i, c) == oracle.index_vec(g, int(site), mu, i, c)
+            assert 0 <= off < V * nl * 18
+            seen.add(off)
+        checked += 1
+    # default split (simd all zero) agrees too
+    for W in (2, 4, 8, 16, 32):
+        assert tuple(su3.su3_desc_normalize(su3.make_desc(32, layout=su3.SU3_VECTOR, W=W)).simd) == oracle.default_simd(W)
