@@ -79,3 +79,38 @@ def test_cshift_full_size_32x4_lorentz_properties():
         assert not torch.equal(b.tensor, a.tensor)
         su3.su3_cshift(c, a, dim, 32)
         assert torch.equal(c.tensor, a.tensor)
+
+
+def test_random_geometries_and_splits_fuzz():
+    """random extents, vector lengths, custom virtual-node splits, Lorentz index and precision: layout permutation
+    and Cshift bit-exact against the oracle, products within tolerance"""
+    from gpu_util import scalar_desc
+    rng = np.random.default_rng(77)
+    for it in range(40):
+        W = int(2 ** rng.integers(0, 6))
+        simd, w = [1, 1, 1, 1], W
+        while w > 1:
+            simd[int(rng.integers(0, 4))] *= 2
+            w //= 2
+        L = tuple(int(s * rng.integers(1, 4)) for s in simd)
+        nl = int(rng.choice([1, 4]))
+        prec = int(rng.choice([F64, F32]))
+        desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=VE, W=W, simd=simd)
+        g, ds = geom_of(desc), scalar_desc(desc)
+        xs = host_field(ds, 90 + it, 0)
+        x, y = host_field(desc, 90 + it, 0), host_field(desc, 90 + it, 1)
+        fs, fx, fy, fz = upload(ds, xs), su3.alloc_field(desc), upload(desc, y), su3.alloc_field(desc)
+        su3.su3_convert(fx, fs)
+        assert np.array_equal(download(fx), x), (L, W, simd)
+        back = su3.alloc_field(ds)
+        su3.su3_convert(back, fx)
+        assert np.array_equal(download(back), xs), (L, W, simd)
+        dim, disp = int(rng.integers(0, 4)), int(rng.integers(-5, 6))
+        su3.su3_cshift(fz, fx, dim, disp)
+        assert np.array_equal(download(fz), oracle.cshift(g, x, dim, disp)), (L, W, simd, dim, disp)
+        su3.su3_mul_shift(fz, fx, fy, dim, disp)
+        err, _ = rel_err(download(fz), oracle.mul_shift(g, x, y, dim, disp), W)
+        assert err <= TOL[prec], (L, W, simd, dim, disp, err)
+        su3.su3_mul(fz, fx, fy)
+        err, _ = rel_err(download(fz), oracle.mul(g, x, y), W)
+        assert err <= TOL[prec], (L, W, simd, err)
