@@ -141,8 +141,9 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *c
  * product).  Examples: "01*" = su3_mul, "01*2*" = su3_mul3, "01*2+" = su3_mul_add (bit-identical to them),
  * "01+01*+" = v1+v2+v1*v2.  At most 32 tokens, 16 operators, stack depth 8; every operand 0..n_operands-1
  * must be used; exactly one value must remain (SU3_ERR_INVALID otherwise).  All fields must have identical
- * descriptors (SU3_ERR_MISMATCH); z may be the same field as any operand.  Every distinct operand adds one
- * read stream: bytes = (n_operands + 1) * field bytes. */
+ * descriptors and be of one kind -- all colour-matrix fields, or all real scalar fields (su3_real_wrap; '*' is then
+ * the element-wise product) -- else SU3_ERR_MISMATCH; z may be the same field as any operand.  Every distinct
+ * operand adds one read stream: bytes = (n_operands + 1) * field bytes. */
 su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *operands, int n_operands,
                     void *cuda_stream);
 
