@@ -247,3 +247,17 @@ def test_library_and_oracle_index_maps_agree_on_random_geometries():
     # default split (simd all zero) agrees too
     for W in (2, 4, 8, 16, 32):
         assert tuple(su3.su3_desc_normalize(su3.make_desc(32, layout=su3.SU3_VECTOR, W=W)).simd) == oracle.default_simd(W)
+
+
+def test_expression_front_end_builds_postfix_programs():
+    """the Lattice front end (Listing 3 style `z = x*y`) only builds the tree: check the programs it emits"""
+    from paper_1710_09409_b200.lattice import Lattice, postfix
+    x, y, w, v = (Lattice(None) for _ in range(4))
+    assert postfix(x * y) == ("01*", [x, y])
+    assert postfix(x * y * w) == ("01*2*", [x, y, w])                 # left-associative, as C++ parses it (P:106)
+    assert postfix(x * y + v) == ("01*2+", [x, y, v])
+    assert postfix(x + y + x * y) == ("01+01*+", [x, y])             # Listing 2: v1+v2+v1*v2, fields deduplicated
+    assert postfix(x * (y - w) - v * x)[0] == "012-*30*-"
+    assert postfix(x) == ("0", [x])
+    with pytest.raises(TypeError):
+        x + 1.0

@@ -143,3 +143,25 @@ def test_expr_random_programs_fuzz(prec, layout, W):
         assert np.isfinite(got).all() and np.abs(got - ref).max() / scale <= 50 * TOL[prec], prog
         seen_temps += prog.count("*") > 2
     assert seen_temps > 10
+
+
+def test_lattice_front_end_assign():
+    from paper_1710_09409_b200.lattice import Lattice
+    desc = su3.make_desc((4, 4, 4, 6), prec=F32, layout=VE, W=8)
+    hosts = [host_field(desc, 97, f) for f in range(3)]
+    x, y, w = (Lattice(upload(desc, h)) for h in hosts)
+    z = Lattice(su3.alloc_field(desc))
+    z.assign(x * y)
+    ref = su3.alloc_field(desc)
+    su3.su3_mul(ref, x.field, y.field)
+    assert np.array_equal(download(z.field), download(ref))
+    z.assign(x + y + x * y - w * x)
+    err, _ = rel_err(download(z.field), oracle.expr(geom_of(desc), "01+01*+20*-", *hosts), 8)
+    assert err <= 4 * TOL[F32]
+    # real scalar fields: the paper's Listing 2, written the paper's way
+    v1, v2, v3 = (Lattice(su3.alloc_real(desc)) for _ in range(3))
+    su3.su3_fill(v1.field, 1.0)
+    su3.su3_fill(v2.field, 2.0)
+    v3.assign(v1 + v2 + v1 * v2)
+    torch.cuda.synchronize()
+    assert bool((v3.field.tensor.view(torch.float32) == 5.0).all())
