@@ -844,9 +844,9 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   }
   if (p.nrec == 0) return SU3_OK;
   const su3_tune tn_c = [] { std::lock_guard<std::mutex> lk(g_tune_mu); return g_tune; }();
-  // fp32: staged through shared memory (256-byte requests on both sides); path = 2 forces the unstaged kernel
+  // fp32 (and fp64 vector -> scalar with W >= 8): staged through shared memory; path = 2 forces the unstaged kernel
   const char *err = nullptr;
-  if (!su3tab::launch_convert(v.prec, nc, v.W, v.prec == SU3_F32 && tn_c.path != 2, p, (cudaStream_t)stream, &err))
+  if (!su3tab::launch_convert(v.prec, nc, v.W, tn_c.path != 2 && (v.prec == SU3_F32 || (v.W >= 8 && !p.to_vector)), p, (cudaStream_t)stream, &err))
     return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);

@@ -11,7 +11,13 @@ bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertPara
     const long long blocks = (p.nrec + TRR - 1) / TRR;                                                       \
     if (blocks > 0x7fffffffLL) { *err = "lattice too large for one launch"; return false; }                  \
     const size_t smem = sizeof(float2) * TRR * nc * (WW + 1) + sizeof(long long) * TRR;                      \
-    if (nc == 9) su3::su3_convert_staged_kernel<float2, WW, TRR, 9><<<(unsigned)blocks, 256, smem, s>>>(p);  \
+    if (prec == 8) {                                                                                         \
+      constexpr int TRD = TRR / 2 > 0 ? TRR / 2 : 1;                                                         \
+      const long long blocksd = (p.nrec + TRD - 1) / TRD;                                                    \
+      const size_t smemd = sizeof(double2) * TRD * nc * (WW + 1) + sizeof(long long) * TRD;                  \
+      if (nc == 9) su3::su3_convert_staged_kernel<double2, WW, TRD, 9><<<(unsigned)blocksd, 256, smemd, s>>>(p); \
+      else su3::su3_convert_staged_kernel<double2, WW, TRD, 3><<<(unsigned)blocksd, 256, smemd, s>>>(p);     \
+    } else if (nc == 9) su3::su3_convert_staged_kernel<float2, WW, TRR, 9><<<(unsigned)blocks, 256, smem, s>>>(p);  \
     else su3::su3_convert_staged_kernel<float2, WW, TRR, 3><<<(unsigned)blocks, 256, smem, s>>>(p);          \
   } return true;
     switch (W) {
