@@ -26,6 +26,8 @@
  *     undefined.
  *   - Handles are immutable after wrap; calls are thread-safe (su3_tune_set is a
  *     process-wide knob and is the one exception: do not race it with launches).
+ *   - One process drives one GPU (the device that is current at the first call): device facts and per-kernel
+ *     attributes are cached per process.
  *   - There is no CPU fallback anywhere: without a CUDA device the arithmetic
  *     calls return SU3_ERR_CUDA.
  *
