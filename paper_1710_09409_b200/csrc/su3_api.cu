@@ -149,8 +149,9 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
   // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
   // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
-  const bool direct = tn.path == 2 || (tn.path == 0 && op != su3::OP_ADD && W * cb >= 32 &&
-                                       footprint_bytes <= (size_t)di.l2 * 2);  // measured cross-over with the pipeline: ~2 x L2
+  const bool direct = op != su3::OP_ADD &&  // OP_ADD has no direct kernel (su3_add's path = 2 is its own plain kernel)
+                      (tn.path == 2 || (tn.path == 0 && W * cb >= 32 &&
+                                        footprint_bytes <= (size_t)di.l2 * 2));  // measured cross-over with the pipeline: ~2 x L2
   const bool warp = !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
   const int family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
   stream_kernel_t k = prec == SU3_F64 ? su3tab::stream_f64(family, op, W) : su3tab::stream_f32(family, op, W);

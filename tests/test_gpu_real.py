@@ -53,6 +53,12 @@ def test_real_expressions_against_the_oracle(prec):
         got = down(z).astype(np.float64)
         tol = 1e-14 if prec == F64 else 1e-5
         assert np.isfinite(got).all() and np.abs(got - ref).max() <= tol * max(1.0, np.abs(ref).max()), prog
+    # the fixed-menu program `a+b` under every path knob
+    for path in (0, 1, 2, 3):
+        su3.su3_tune_set(path=path)
+        su3.su3_expr(z, "01+", fs[:2])
+        assert np.array_equal(down(z), hosts[0] + hosts[1]), path
+    su3.su3_tune_set()
     # z may be an operand
     su3.su3_expr(fs[0], "01+", fs[:2])
     assert np.array_equal(down(fs[0]), hosts[0] + hosts[1])
