@@ -298,7 +298,7 @@ def run_ours(args, rank, world, local_rank):
     }
     return dict(torch=torch, su3=su3, dist=dist, dev=coll_dev, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
                 nmat=nmat, step_bytes=step_bytes, step_flops=step_flops, ms_per_step=ms_per_step, value=value,
-                launches=launches, clk=clk, checks=checks, info=info, t_wall=t_wall, barrier=barrier, step=step,
+                launches=launches, clk=clk, checks=checks, nwarm=nwarm, info=info, t_wall=t_wall, barrier=barrier, step=step,
                 hbytes=hbytes)
 
 
@@ -656,7 +656,7 @@ def main():
     if rank != 0:
         return
     line = {
-        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "warmup_steps_run": r["nwarm"],
         "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "BASELINE.json configs[4] top point: %d^4 lattice per GPU (%d matrices, %.3f GB per field), "
