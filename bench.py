@@ -40,6 +40,7 @@ METRIC = "su3xsu3_stream_GBps"
 UNIT = "GB/s"
 FLOPS = {"mul": 198, "mul3": 396, "mul_add": 216, "convert": 0, "copy": 0, "add": 18}
 STREAMS = {"mul": 3, "mul3": 4, "mul_add": 4, "convert": 2, "copy": 2, "add": 3}
+E2E_CHUNKS = int(os.environ.get("SU3_E2E_CHUNKS", "16"))  # chunks of the host pipelines in the e2e leg
 W64, W32 = 4, 8  # vector lengths of the configs: fp64 W=4, fp32 W=8 (64-byte element vectors)
 
 
@@ -349,7 +350,7 @@ def run_e2e(args, r, world):
         main = torch.cuda.current_stream()
         start = torch.cuda.Event(); start.record(main)
         # A1: x, y in and z out, chunked and overlapped inside the library; x, y stay resident for A2-A4
-        su3.su3_mul_host(hz[0], hx, hy, f["zs"], f["xs"], f["ys"], chunks=8)
+        su3.su3_mul_host(hz[0], hx, hy, f["zs"], f["xs"], f["ys"], chunks=E2E_CHUNKS)
         # w, v follow x, y on the H2D engine while the A1 result is already flowing back
         h2d_s.wait_event(start)
         with torch.cuda.stream(h2d_s):
@@ -372,7 +373,7 @@ def run_e2e(args, r, world):
         su3.su3_mul3(f["z3"], f["xv"], f["yv"], f["wv"])                              # A3
         result_to_host(f["z3"])
         # A4 chunked through the library: v arrives chunk by chunk behind w, every chunk of x*y + v leaves at once
-        su3.su3_eval_host(su3.SU3_OP_MUL_ADD, hz[2], None, None, hv, f["z4"], f["xs"], f["ys"], f["vs"], chunks=8)
+        su3.su3_eval_host(su3.SU3_OP_MUL_ADD, hz[2], None, None, hv, f["z4"], f["xs"], f["ys"], f["vs"], chunks=E2E_CHUNKS)
         done = torch.cuda.Event(); done.record(d2h_s)
         main.wait_event(done)
 
