@@ -67,3 +67,15 @@ def rel_err(z, zref, W):
     with np.errstate(divide="ignore", invalid="ignore"):
         r = np.where(num == 0, 0.0, num / den)
     return float(r.max()) if r.size else 0.0, float(d.max()) if d.size else 0.0
+
+
+def rel_err_chunked(z, zref, W, chunk_records=1 << 20):
+    """rel_err over a whole large field, evaluated in slices of `chunk_records` records so that the temporaries
+    stay small next to the field (64^4 fp64 = 2.4 GB per array)."""
+    step = chunk_records * 18 * W
+    worst, worst_abs = 0.0, 0.0
+    assert z.size == zref.size and z.size % (18 * W) == 0
+    for a in range(0, z.size, step):
+        e, d = rel_err(z[a:a + step], zref[a:a + step], W)
+        worst, worst_abs = max(worst, e), max(worst_abs, d)
+    return worst, worst_abs
