@@ -61,7 +61,6 @@ def parse_args():
     ap.add_argument("--profile-pass", action="store_true",
                     help="launch every kernel variant of the library once at 48^4 (no timing): the command ncu wraps "
                          "for profiles/*_all_kernels.md")
-    ap.add_argument("--cpu-L", type=int, default=32, help="lattice extent of the oracle's bounded sample")
     return ap.parse_args()
 
 
@@ -75,60 +74,165 @@ def measured_peak():
 
 
 # ---------------------------------------------------------------------------- the oracle legs
-def oracle_step(L, reps, threads=None):
-    """Time the oracle, as it stands, on `reps` passes of one step (rows A1-A6; A6 is a memcpy) of an L^4
-    fp64 lattice.  Returns (seconds per pass [reps], bytes a pass moves by S9's accounting, threads used)."""
-    import oracle
-    import su3gen
-    if threads:
-        oracle.set_num_threads(threads)
-    seed = su3gen.config_seed(5)
-    gs, gv = oracle.Geom(L), oracle.Geom(L, layout=oracle.su3_oracle.VECTOR, W=W64)
-    n = gs.nmat
-    xs, ys, ws = (su3gen.su3_field(seed, f, n).view(np.float64).reshape(-1) for f in (0, 1, 2))
-    vs = su3gen.gaussian_field(seed, 3, n).view(np.float64).reshape(-1)
-    times = []
-    for _ in range(reps):
+class OracleStep:
+    """One step (rows A1-A6; A6 is a memcpy) by the oracle, as it stands, on an L^4 fp64 lattice.  Inputs come from
+    su3gen (or from the caller: flat fp64 arrays in logical order); every output buffer is allocated once and
+    first-touched by an untimed pass, so the timed passes contain the oracle's loops and nothing else."""
+
+    def __init__(self, L, inputs=None, threads=None):
+        import oracle
+        import su3gen
+        self.oracle = oracle
+        if threads:
+            oracle.set_num_threads(threads)
+        self.gs, self.gv = oracle.Geom(L), oracle.Geom(L, layout=oracle.su3_oracle.VECTOR, W=W64)
+        n = self.gs.nmat
+        self.n = n
+        if inputs is None:
+            seed = su3gen.config_seed(5)
+            inputs = [su3gen.su3_field(seed, f, n).view(np.float64).reshape(-1) for f in (0, 1, 2)]
+            inputs.append(su3gen.gaussian_field(seed, 3, n).view(np.float64).reshape(-1))
+        self.xs, self.ys, self.ws, self.vs = inputs
+        self.out = {k: np.empty(n * 18, dtype=np.float64) for k in ("xv", "yv", "wv", "zs", "zv", "z3", "z4", "zb", "zc")}
+        self.bytes = 24 * n * 144          # S9's accounting: 24 field streams
+        self.threads = oracle.num_threads()
+        self.run()                         # first touch of the outputs with the loops' own OpenMP schedule
+
+    def run(self):
+        o, b, gs, gv = self.oracle, self.out, self.gs, self.gv
         t0 = time.perf_counter()
-        xv, yv, wv = (oracle.convert(gv, gs, a) for a in (xs, ys, ws))
-        zs = oracle.mul(gs, xs, ys)
-        zv = oracle.mul(gv, xv, yv)
-        z3 = oracle.mul3(gv, xv, yv, wv)
-        z4 = oracle.mul_add(gs, xs, ys, vs)
-        zb = oracle.convert(gs, gv, zv)
-        zc = zs.copy()
-        times.append(time.perf_counter() - t0)
-    assert np.array_equal(zb, zs) and zc.size == zs.size and z3.size == z4.size
-    return times, 24 * n * 144, oracle.num_threads()
+        o.convert(gv, gs, self.xs, out=b["xv"]); o.convert(gv, gs, self.ys, out=b["yv"]); o.convert(gv, gs, self.ws, out=b["wv"])
+        o.mul(gs, self.xs, self.ys, out=b["zs"])
+        o.mul(gv, b["xv"], b["yv"], out=b["zv"])
+        o.mul3(gv, b["xv"], b["yv"], b["wv"], out=b["z3"])
+        o.mul_add(gs, self.xs, self.ys, self.vs, out=b["z4"])
+        o.convert(gs, gv, b["zv"], out=b["zb"])
+        np.copyto(b["zc"], b["zs"])
+        return time.perf_counter() - t0
+
+    def check(self):
+        assert np.array_equal(self.out["zb"], self.out["zs"]) and np.array_equal(self.out["zc"], self.out["zs"])
+
+
+REF_BUDGET_S = 240.0   # --impl reference: the whole run (W + K passes) should end within a few minutes
 
 
 def run_reference(args, rank):
-    """--impl reference: the oracle on the host cores, same metric/config; every step is one pass over a
-    bounded sample (a smaller lattice of the same sweep) so that W+K passes end within a few minutes."""
+    """--impl reference: the oracle on the host cores, same metric/config.  Every step is one pass of rows A1-A6 at the
+    WORKLOAD's own L whenever (W + K) passes fit the time budget (64^4: a few seconds per pass); otherwise a smaller
+    point of the same sweep serves as the bounded sample, and `same_config` says so."""
     if rank != 0:
         return
-    L = min(args.cpu_L, args.L)
-    if args.warmup + args.steps > 30:
-        L = min(L, 24)
-    times, nbytes, threads = oracle_step(L, args.warmup + args.steps)
+    L = args.L
+    st = OracleStep(L)
+    t1 = st.run()
+    total = args.warmup + args.steps
+    while L > 16 and total * t1 > REF_BUDGET_S:
+        L = {64: 48, 48: 32, 32: 24, 24: 16}.get(L, 16)
+        del st
+        st = OracleStep(L)
+        t1 = st.run()
+    times = [st.run() for _ in range(total)]
+    st.check()
     timed = times[args.warmup:]
     sec = sum(timed) / len(timed)
-    val = nbytes / sec / 1e9
-    sample = "every step = rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep; workload %d^4)" % (L, args.L)
+    val = st.bytes / sec / 1e9
+    same = L == args.L
+    sample = ("every step = one pass of rows A1-A6 on the workload's own %d^4 fp64 lattice" % L if same else
+              "every step = rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep; workload %d^4)" % (L, args.L))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "cfg5 volume sweep top: %d^4 fp64, rows A1-A6" % args.L, "sample_L": L},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "config": {"workload": "BASELINE.json configs[4] top point: %d^4 lattice, fp64 complex, scalar + vector(W=%d) layouts, "
+                               "rows A1-A6 per step" % (args.L, W64), "L": args.L, "sample_L": L, "same_config": same},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": st.threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }), flush=True)
+
+
+def run_cpu_baseline(args, host):
+    """cpu_baseline leg (rank 0, N = 1): the oracle on the box's host cores.  `value` = one step (rows A1-A6) at the
+    workload's own L, all cores, best of 2 after a first-touch pass; beside it `z = x*y` (and the fused expressions of
+    config 4) per BASELINE.json config, best of 3, with the bytes the oracle really moves (fp32 configs: fp32 in, fp64
+    out = 288 B per matrix for mul), the one-thread figure, and a host STREAM triad."""
+    import oracle
+    VEC = oracle.su3_oracle.VECTOR
+    L = args.L
+    flat = [host[k].numpy().view(np.float64).reshape(-1) for k in ("x", "y", "w", "v")]
+    st = OracleStep(L, inputs=flat)
+    t = min(st.run(), st.run())
+    st.check()
+    cpu = {"value": st.bytes / t / 1e9, "unit": UNIT, "cores": st.threads, "kind": "oracle",
+           "sample": "one step = rows A1-A6 on the workload's own %d^4 fp64 lattice, all cores, best of 2 passes after a "
+                     "first-touch pass" % L, "ms_per_step": t * 1e3}
+    del st
+
+    def best_of(fn, reps=3):
+        fn()
+        return min(_timeit(fn) for _ in range(reps))
+
+    def _timeit(fn):
+        t0 = time.perf_counter()
+        fn()
+        return time.perf_counter() - t0
+
+    per = []
+
+    def mul_point(name, Lc, nl, prec, layout, W, ops=("mul",)):
+        g = oracle.Geom(Lc, nl=nl, layout=layout, W=W)
+        gs = oracle.Geom(Lc, nl=nl)
+        n = g.nmat
+        if n * 18 > flat[0].size:
+            return
+        dt = np.float64 if prec == 8 else np.float32
+        used = {0, 1} | ({2} if "mul3" in ops else set()) | ({3} if "mul_add" in ops else set())
+        # a prefix of the resident fields: timing is data-independent
+        ins = [np.ascontiguousarray(a[:n * 18], dtype=dt) if k in used else None for k, a in enumerate(flat)]
+        if layout == VEC:
+            ins = [oracle.convert(g, gs, a) if a is not None else None for a in ins]
+        out = np.zeros(n * 18, dtype=np.float64)
+        for op in ops:
+            fn = {"mul": lambda: oracle.mul(g, ins[0], ins[1], out=out),
+                  "mul3": lambda: oracle.mul3(g, ins[0], ins[1], ins[2], out=out),
+                  "mul_add": lambda: oracle.mul_add(g, ins[0], ins[1], ins[3], out=out)}[op]
+            sec = best_of(fn)
+            nin = 2 if op == "mul" else 3
+            moved = n * (nin * 18 * prec + 144)                  # inputs in storage precision, fp64 result
+            per.append({"config": name, "op": op, "GBps": moved / sec / 1e9, "GFLOPps": FLOPS[op] * n / sec / 1e9,
+                        "bytes_per_matrix": nin * 18 * prec + 144, "ms": sec * 1e3})
+
+    mul_point("cfg1: 8^4 fp64 scalar", 8, 1, 8, 0, 1)
+    mul_point("cfg2: 16^4 fp64 scalar", 16, 1, 8, 0, 1)
+    mul_point("cfg2: 16^4 fp64 vector W=%d" % W64, 16, 1, 8, VEC, W64)
+    mul_point("cfg3: 32^4 x 4 Lorentz fp64 scalar", 32, 4, 8, 0, 1)
+    mul_point("cfg3: 32^4 x 4 Lorentz fp64 vector W=%d" % W64, 32, 4, 8, VEC, W64)
+    mul_point("cfg4: 48^4 fp32 vector W=%d" % W32, 48, 1, 4, VEC, W32, ops=("mul3", "mul_add"))
+    mul_point("cfg5: 48^4 fp64 scalar", 48, 1, 8, 0, 1)
+    mul_point("cfg5: %d^4 fp64 scalar" % L, L, 1, 8, 0, 1)
+    mul_point("cfg5: %d^4 fp32 vector W=%d" % (L, W32), L, 1, 4, VEC, W32)
+    cpu["per_config"] = per
+    cpu["stream_triad_GBps"] = oracle.stream_triad(1 << 27)
+    nthreads = oracle.num_threads()
+    oracle.set_num_threads(1)
+    try:
+        L1 = min(L, 32)
+        g1 = oracle.Geom(L1)
+        n1 = g1.nmat
+        out1 = np.zeros(n1 * 18, dtype=np.float64)
+        sec = best_of(lambda: oracle.mul(g1, flat[0][:n1 * 18], flat[1][:n1 * 18], out=out1))
+        cpu["one_thread"] = {"op": "mul", "sample": "z = x*y on a %d^4 fp64 lattice, 1 thread, best of 3" % L1,
+                             "GBps": 3 * n1 * 144 / sec / 1e9, "GFLOPps": FLOPS["mul"] * n1 / sec / 1e9,
+                             "stream_triad_GBps": oracle.stream_triad(1 << 25)}
+    finally:
+        oracle.set_num_threads(nthreads)
+    return cpu
 
 
 # ---------------------------------------------------------------------------- clocks during the timed region
 CLOCK_Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
            "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-           "clocks_event_reasons.sw_power_cap")
+           "clocks_event_reasons.sw_power_cap,clocks.mem,clocks.max.mem,name")
 
 
 class ClockSampler:
@@ -153,7 +257,7 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, smax, reasons, power = [], [], set(), []
+        sm, smax, reasons, power, mem, memmax, name = [], [], set(), [], [], [], None
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f:
             c = [t.strip() for t in line.split(",")]
@@ -163,6 +267,11 @@ class ClockSampler:
                 sm.append(float(c[1])); smax.append(float(c[2])); power.append(float(c[3]))
             except ValueError:
                 continue
+            if len(c) >= 12:
+                try:
+                    mem.append(float(c[9])); memmax.append(float(c[10])); name = c[11]
+                except ValueError:
+                    pass
             for nm, v in zip(names, c[5:9]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
@@ -171,7 +280,8 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(smax), "power_w_max": max(power),
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "mem_mhz": float(np.median(mem)) if mem else None, "mem_max_mhz": max(memmax) if memmax else None,
+                "gpu_name": name, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 # ---------------------------------------------------------------------------- our arm
@@ -297,13 +407,14 @@ def run_ours(args, rank, world, local_rank):
         "vector_result_equals_scalar_result_bitwise": bool(torch.equal(f["zb"].tensor, f["zs"].tensor)),
         "copy_bitwise": bool(torch.equal(f["zc"].tensor, f["zs"].tensor)),
     }
-    return dict(torch=torch, su3=su3, dist=dist, dev=coll_dev, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
+    gpu_name, _ = su3.su3_device_name()
+    return dict(torch=torch, su3=su3, dist=dist, dev=coll_dev, gpu_name=gpu_name, f=f, host=host, hz=hz, rows=rows, row_ms=row_ms, B=B,
                 nmat=nmat, step_bytes=step_bytes, step_flops=step_flops, ms_per_step=ms_per_step, value=value,
                 launches=launches, clk=clk, checks=checks, nwarm=nwarm, info=info, t_wall=t_wall, barrier=barrier, step=step,
                 hbytes=hbytes)
 
 
-def time_calls(torch, fn, target_ms=2.0, batches=5, warm=3, graph_below_us=0.0):
+def time_calls(torch, fn, target_ms=2.0, batches=10, warm=3, graph_below_us=0.0):
     """SURVEY 8(d) protocol: warm-up calls, then `batches` batches of Nloop back-to-back calls between two
     CUDA events on the current stream; returns (min, median) ms per call and how the calls were issued.
     Calls shorter than `graph_below_us` are launch-bound from Python: their Nloop calls are captured once
@@ -389,27 +500,81 @@ def run_e2e(args, r, world):
     from paper_1710_09409_b200 import shard
     rate, ms, _ = shard.job_throughput(r["step_bytes"], a.elapsed_time(b) / n, r["dist"], r["dev"])
     ok = bool(torch.equal(hz[0], f["zs"].tensor.cpu())) and bool(torch.equal(hz[2], f["z4"].tensor.cpu()))
-    return {"value": rate / 1e9, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
+    # and the host results against the ORACLE on sampled matrices (A1: z = x*y, A4: z = x*y + v)
+    import oracle
+    nmat = r["nmat"]
+    pick = np.unique(np.concatenate([np.random.default_rng(5).integers(0, nmat, 4000), [0, 1, nmat - 2, nmat - 1]]))
+    small = oracle.Geom((len(pick), 1, 1, 1))
+    sx, sy, sv = (host[k].numpy().reshape(nmat, 9)[pick].view(np.float64).reshape(-1) for k in ("x", "y", "v"))
+    errs = []
+    for hzk, ref in ((hz[0], oracle.mul(small, sx, sy)), (hz[2], oracle.mul_add(small, sx, sy, sv))):
+        got = hzk.numpy().view(np.float64).reshape(nmat, 18)[pick]
+        ref = ref.reshape(-1, 18)
+        errs.append(float((np.abs(got - ref).max(axis=1) / np.abs(ref).max(axis=1)).max()))
+    return {"value": rate / 1e9, "host_result_vs_oracle_sampled": {"matrices": int(len(pick)), "max_rel_err_A1": errs[0],
+                                                                      "max_rel_err_A4": errs[1], "ok": bool(max(errs) <= 1e-12)}, "unit": UNIT, "h2d_bytes_per_step": 4 * B,
             "d2h_bytes_per_step": 4 * B, "ms_per_step": ms, "steps": n,
             "api": "su3_mul_host (A1), su3_eval_host (A4, x and y resident) + pinned async copies on side streams around su3_convert/su3_mul/su3_mul3/su3_copy",
             "host_result_matches_device": ok}
 
 
+class Ceilings:
+    """Same-run streaming ceilings at ANY field size (the paper draws its STREAM line across the whole footprint
+    axis, Fig. 3): the library's own TMA copy kernel, cudaMemcpyAsync D2D (torch copy_) and the
+    2-read-1-write add, timed with the sweep's own protocol on prefixes of resident fields; cached per size."""
+
+    def __init__(self, torch, su3, a, b, c, l2):
+        self.torch, self.su3, self.a, self.b, self.c, self.l2 = torch, su3, a, b, c, l2
+        self.cache = {}
+
+    def at(self, L, prec, nl=1):
+        key = (L, prec, nl)
+        if key in self.cache:
+            return self.cache[key]
+        torch, su3 = self.torch, self.su3
+        d = su3.make_desc(L, n_lorentz=nl, prec=prec)
+        nb = su3.su3_field_bytes(d)
+        fa, fb, fc = (su3.su3_field_wrap(d, t.tensor[:nb]) for t in (self.a, self.b, self.c))
+        out = {"L": L, "prec": "f64" if prec == 8 else "f32", "field_MB": nb / 1e6}
+        mn, _, how = time_calls(torch, lambda: su3.su3_copy(fc, fa), graph_below_us=60.0)
+        out["su3_copy"] = 2 * nb / (mn * 1e-3) / 1e9
+        mn, _, _ = time_calls(torch, lambda: fc.tensor.copy_(fa.tensor), graph_below_us=60.0)
+        out["memcpy_d2d"] = 2 * nb / (mn * 1e-3) / 1e9
+        mn, _, _ = time_calls(torch, lambda: su3.su3_add(fc, fa, fb), graph_below_us=60.0)
+        out["su3_add_2r1w"] = 3 * nb / (mn * 1e-3) / 1e9
+        out["best_copy"] = max(out["su3_copy"], out["memcpy_d2d"])
+        out["issued"] = how
+        if 3 * nb <= 2 * self.l2:
+            # cold protocol (S18) for the copy as well: rotate through (dst, src) pairs that together exceed 2 x L2
+            nb_al = (nb + 255) // 256 * 256
+            npair = int(min(self.a.tensor.numel() // nb_al, 2 * self.l2 // (2 * nb) + 2))
+            if npair * 2 * nb > 2 * self.l2:
+                pairs = [(su3.su3_field_wrap(d, self.c.tensor[k * nb_al:k * nb_al + nb]),
+                          su3.su3_field_wrap(d, self.a.tensor[k * nb_al:k * nb_al + nb])) for k in range(npair)]
+                ctr = [0]
+
+                def rot():
+                    dst, src = pairs[ctr[0] % npair]
+                    ctr[0] += 1
+                    su3.su3_copy(dst, src)
+                cmn, _, _ = time_calls(torch, rot, target_ms=4.0, warm=npair, graph_below_us=60.0)
+                out["su3_copy_cold"] = 2 * nb / (cmn * 1e-3) / 1e9
+        self.cache[key] = out
+        return out
+
+
 def run_ceilings_and_sweep(args, r):
-    """Same-run ceilings (A6: own copy kernel, cudaMemcpyAsync D2D, the 2-read-1-write add) at the workload
-    size, then the volume sweep of BASELINE.json configs[4]: z = x*y for L = 8..64, fp64/fp32, scalar/vector,
-    warm protocol (Listing 3: same operands every call).  Operands are prefixes of the resident fields."""
+    """Same-run ceilings (A6) at the workload size and at EVERY sweep size, then the volume sweep of BASELINE.json
+    configs[4]: z = x*y for L = 8..64, fp64/fp32, scalar/vector, warm protocol (Listing 3: same operands every call)
+    and, below 2 x L2, cold protocol (rotating operands).  Operands are prefixes of the resident fields."""
     torch, su3, f, B = r["torch"], r["su3"], r["f"], r["B"]
     l2 = r["info"]["l2_bytes"]
-    out = {}
-    mn, md, _ = time_calls(torch, lambda: su3.su3_copy(f["zc"], f["zs"]))
-    out["su3_copy"] = 2 * B / (mn * 1e-3) / 1e9
-    mn, md, _ = time_calls(torch, lambda: f["zc"].tensor.copy_(f["zs"].tensor))
-    out["memcpy_d2d"] = 2 * B / (mn * 1e-3) / 1e9
-    mn, md, _ = time_calls(torch, lambda: su3.su3_add(f["zc"], f["xs"], f["ys"]))
-    out["su3_add_2r1w"] = 3 * B / (mn * 1e-3) / 1e9
-    ceiling = max(out["su3_copy"], out["memcpy_d2d"])
-    out["bar_denominator"] = ceiling
+    ceil = Ceilings(torch, su3, f["zs"], f["xs"], f["zc"], l2)
+    r["ceil"] = ceil
+    top = ceil.at(args.L, 8)
+    out = {"su3_copy": top["su3_copy"], "memcpy_d2d": top["memcpy_d2d"], "su3_add_2r1w": top["su3_add_2r1w"],
+           "bar_denominator": top["best_copy"]}
+    ceiling = top["best_copy"]
     if args.no_sweep:
         return out, []
     # fp32 copies of x, y in both layouts (input preparation only: rounding fp64 -> fp32, S16)
@@ -424,28 +589,43 @@ def run_ceilings_and_sweep(args, r):
            (4, 0): (fx32s, fy32s, f["zc"]), (4, 1): (fx32v, fy32v, f["zc"])}
     # f1 (Fig. 4): vector-length sweep at a fixed HBM-bound volume, fp32 complex.
     # The paper's GPUs plateaued only at W = 16 because block = one vector; here bandwidth is flat in W.
-    wsweep = []
-    Lw = min(args.L, 48)
-    for Wv in (1, 2, 4, 8, 16, 32):
-        dsw = su3.make_desc(Lw, prec=su3.SU3_F32)
-        dw = su3.make_desc(Lw, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=Wv)
-        nbw = su3.su3_field_bytes(dw)
-        xs_w = su3.su3_field_wrap(dsw, x32[:nbw // 4].view(torch.uint8))
-        ys_w = su3.su3_field_wrap(dsw, y32[:nbw // 4].view(torch.uint8))
-        xw, yw, zw = su3.alloc_field(dw), su3.alloc_field(dw), su3.alloc_field(dw)
-        su3.su3_convert(xw, xs_w); su3.su3_convert(yw, ys_w)
-        mn, md, _ = time_calls(torch, lambda: su3.su3_mul(zw, xw, yw))
-        wsweep.append({"W": Wv, "L": Lw, "prec": "f32", "simd": list(su3.su3_desc_normalize(dw).simd),
-                       "us_min": mn * 1e3, "GBps": 3 * nbw / (mn * 1e-3) / 1e9,
-                       "GFLOPps": FLOPS["mul"] * Lw ** 4 / (mn * 1e-3) / 1e9,
-                       "frac_of_copy": 3 * nbw / (mn * 1e-3) / 1e9 / ceiling})
-        del xw, yw, zw
+    # A5 in fp32 rides along: the scalar <-> vector permutation is timed for every W, both directions.
+    wsweep, conv32 = [], []
+    for Lw in sorted({min(args.L, 48), args.L}):
+        cw = ceil.at(Lw, 4)
+        for Wv in (1, 2, 4, 8, 16, 32):
+            dsw = su3.make_desc(Lw, prec=su3.SU3_F32)
+            dw = su3.make_desc(Lw, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=Wv)
+            nbw = su3.su3_field_bytes(dw)
+            xs_w = su3.su3_field_wrap(dsw, x32[:nbw // 4].view(torch.uint8))
+            ys_w = su3.su3_field_wrap(dsw, y32[:nbw // 4].view(torch.uint8))
+            xw, yw, zw = su3.alloc_field(dw), su3.alloc_field(dw), su3.alloc_field(dw)
+            back = su3.su3_field_wrap(dsw, f["zc"].tensor[:nbw])
+            su3.su3_convert(xw, xs_w); su3.su3_convert(yw, ys_w)
+            if Wv >= 2:
+                t_sv, _, _ = time_calls(torch, lambda: su3.su3_convert(xw, xs_w))
+                t_vs, _, _ = time_calls(torch, lambda: su3.su3_convert(back, xw))
+                ok = bool(torch.equal(back.tensor, xs_w.tensor))
+                conv32.append({"L": Lw, "W": Wv, "prec": "f32", "scalar_to_vector_GBps": 2 * nbw / (t_sv * 1e-3) / 1e9,
+                               "vector_to_scalar_GBps": 2 * nbw / (t_vs * 1e-3) / 1e9,
+                               "frac_of_copy": [2 * nbw / (t * 1e-3) / 1e9 / cw["best_copy"] for t in (t_sv, t_vs)],
+                               "round_trip_bit_exact": ok})
+            if Lw == min(args.L, 48):
+                mn, md, _ = time_calls(torch, lambda: su3.su3_mul(zw, xw, yw))
+                wsweep.append({"W": Wv, "L": Lw, "prec": "f32", "simd": list(su3.su3_desc_normalize(dw).simd),
+                               "us_min": mn * 1e3, "GBps": 3 * nbw / (mn * 1e-3) / 1e9,
+                               "GFLOPps": FLOPS["mul"] * Lw ** 4 / (mn * 1e-3) / 1e9,
+                               "frac_of_copy": 3 * nbw / (mn * 1e-3) / 1e9 / cw["best_copy"]})
+            del xw, yw, zw
     out["wsweep"] = wsweep
-    sweep = []
+    out["convert_f32"] = conv32
+    sweep, by_size = [], []
     for Ls in (8, 12, 16, 24, 32, 48, 64):
         if Ls > args.L:
             continue
         for prec in (8, 4):
+            c = ceil.at(Ls, prec)
+            by_size.append(c)
             for layout in (0, 1):
                 W = 1 if layout == 0 else (W64 if prec == 8 else W32)
                 d = su3.make_desc(Ls, prec=prec, layout=layout, W=W)
@@ -476,7 +656,10 @@ def run_ceilings_and_sweep(args, r):
                 sweep.append({"L": Ls, "prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector",
                               "W": W, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3, "issued": how,
                               "GBps": gbs, "GFLOPps": FLOPS["mul"] * Ls ** 4 / (mn * 1e-3) / 1e9, "regime": regime, "cold_GBps": cold,
-                              "frac_of_copy": gbs / ceiling if regime == "HBM-bound" else None})
+                              # against the SAME-SIZE ceilings of this run (warm: best of su3_copy / D2D; and the 2r1w add)
+                              "frac_of_copy": gbs / c["best_copy"], "frac_of_add_2r1w": gbs / c["su3_add_2r1w"],
+                              "cold_frac_of_copy": cold / c["su3_copy_cold"] if cold and c.get("su3_copy_cold") else None})
+    out["by_size"] = by_size
     return out, sweep
 
 
@@ -485,7 +668,8 @@ def run_next_rows(args, r):
     same protocol: f2 the one-pass expression evaluator, f3 Cshift and the shifted product."""
     torch, su3, f = r["torch"], r["su3"], r["f"]
     Ln = min(args.L, 48)
-    out = {"L": Ln, "prec": "f64", "expr": [], "shift": []}
+    c64, c32 = r["ceil"].at(Ln, 8)["best_copy"], r["ceil"].at(Ln, 4)["best_copy"]
+    out = {"L": Ln, "prec": "f64", "copy_ceiling_GBps": {"f64": c64, "f32": c32}, "expr": [], "shift": []}
     for layout, W, names in ((0, 1, ("xs", "ys", "ws", "vs")), (1, W64, ("xv", "yv", "wv", "z3"))):
         d = su3.make_desc(Ln, layout=layout, W=W)
         nb = su3.su3_field_bytes(d)
@@ -497,12 +681,15 @@ def run_next_rows(args, r):
             st, fl = su3.su3_expr_cost(prog, n)
             mn, _, _ = time_calls(torch, lambda: su3.su3_expr(z, prog, ops[:n]))
             out["expr"].append({"program": prog, "layout": lay, "streams": st, "flops_per_matrix": fl,
-                                "GBps": st * nb / (mn * 1e-3) / 1e9, "GFLOPps": fl * Ln ** 4 / (mn * 1e-3) / 1e9})
+                                "GBps": st * nb / (mn * 1e-3) / 1e9, "GFLOPps": fl * Ln ** 4 / (mn * 1e-3) / 1e9,
+                                "frac_of_copy": st * nb / (mn * 1e-3) / 1e9 / c64})
         for dim in range(4):
             mn, _, _ = time_calls(torch, lambda: su3.su3_cshift(z, ops[1], dim, 1))
             mn2, _, _ = time_calls(torch, lambda: su3.su3_mul_shift(z, ops[0], ops[1], dim, 1))
             out["shift"].append({"dim": dim, "disp": 1, "layout": lay, "cshift_GBps": 2 * nb / (mn * 1e-3) / 1e9,
                                  "mul_shift_GBps": 3 * nb / (mn2 * 1e-3) / 1e9,
+                                 "cshift_frac_of_copy": 2 * nb / (mn * 1e-3) / 1e9 / c64,
+                                 "mul_shift_frac_of_copy": 3 * nb / (mn2 * 1e-3) / 1e9 / c64,
                                  "mul_shift_GFLOPps": FLOPS["mul"] * Ln ** 4 / (mn2 * 1e-3) / 1e9})
     # BASELINE.json configs[2] and configs[3] as bench points (their parity is in tests/test_gpu_fullsize.py)
     out["configs"] = []
@@ -538,6 +725,7 @@ def run_next_rows(args, r):
             ok = bool((v3.tensor.view(torch.float64 if prec == 8 else torch.float32) == (3.0 if prog == "01+" else 5.0)).all())
             out["listing2"].append({"program": prog, "prec": "f64" if prec == 8 else "f32", "reals": nbig // prec,
                                     "GBps": 3 * nbig / (mn * 1e-3) / 1e9, "GFLOPps": flops * (nbig // prec) / (mn * 1e-3) / 1e9,
+                                    "frac_of_copy": 3 * nbig / (mn * 1e-3) / 1e9 / (c64 if prec == 8 else c32),
                                     "value_is_the_papers": ok})
     # f4: colour vectors, y = U.psi (66 flops, 240 B fp64 / 120 B fp32 per site)
     out["matvec"] = []
@@ -549,8 +737,24 @@ def run_next_rows(args, r):
         mn, _, _ = time_calls(torch, lambda: su3.su3_matvec(yv, U, psi))
         nb = su3.su3_field_bytes(d) + 2 * nv
         out["matvec"].append({"prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector W=%d" % W,
-                              "GBps": nb / (mn * 1e-3) / 1e9, "GFLOPps": 66 * Ln ** 4 / (mn * 1e-3) / 1e9})
+                              "GBps": nb / (mn * 1e-3) / 1e9, "GFLOPps": 66 * Ln ** 4 / (mn * 1e-3) / 1e9,
+                              "frac_of_copy": nb / (mn * 1e-3) / 1e9 / (c64 if prec == 8 else c32)})
     return out
+
+
+def ncu_traffic(L):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel: NOT measured in this run (no
+    number is ever taken under a profiler here) but read from the committed ncu --set full summary, whose own header
+    names the command, the lattice and the commit it was captured at.  None if there is no capture for this L."""
+    import glob
+    import re
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_pipe_kernel_full.md")), reverse=True):
+        text = open(path).read()
+        m = re.search(r"traffic_bytes_per_launch\s*=\s*(\d+)\s*\(L\s*=\s*(\d+),\s*captured at commit ([0-9a-f]+), ([^)]*)\)", text)
+        if m and int(m.group(2)) == L:
+            return int(m.group(1)), "%s: ncu --set full capture at commit %s (%s); not re-measured in this run" % (
+                os.path.relpath(path, ROOT), m.group(3), m.group(4))
+    return None, "no committed ncu --set full capture for L = %d" % L
 
 
 def profile_pass(args):
@@ -632,32 +836,33 @@ def main():
                     "frac_of_measured_peak": gbs / peak,
                     "frac_of_copy": gbs / ceilings["bar_denominator"] if ceilings else None})
     a1 = ops[3]
-    # nominal pin-rate peak from device properties: memory clock x 2 (DDR) x bus width / 8
-    pin_rate = r["info"]["mem_clock_khz"] * 1e3 * 2 * r["info"]["bus_width_bits"] / 8 / 1e9
+    # Nominal pin-rate peaks, both stated: nvidia-smi's clocks.max.mem (3996 MHz on B200, the figure ncu's
+    # dram__throughput is relative to) and the CUDA attribute cudaDevAttrMemoryClockRate (3746 MHz on the same
+    # chip); peak = clock x 2 (DDR) x bus width / 8.  `pin_rate_peak` is the nvidia-smi one.
+    bus = r["info"]["bus_width_bits"]
+    pin_attr = r["info"]["mem_clock_khz"] * 1e3 * 2 * bus / 8 / 1e9
+    mem_max = r["clk"].get("mem_max_mhz")
+    pin_rate = mem_max * 1e6 * 2 * bus / 8 / 1e9 if mem_max else pin_attr
+    traffic, traffic_src = ncu_traffic(args.L)
     roofline = {"bound": "hbm", "kernel": "su3_pipe_kernel<double,W=1,OP_MUL> (row A1, z=x*y fp64 scalar)",
                 "achieved": a1["GBps"], "peak": peak, "unit": "GB/s", "frac": a1["GBps"] / peak, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": 3 * B, "avg_launch_ms": a1["ms"],
                 "frac_of_same_run_copy": a1["frac_of_copy"], "pin_rate_peak": pin_rate, "frac_of_pin_rate_peak": a1["GBps"] / pin_rate,
-                # dram__bytes_read.sum + dram__bytes_write.sum of this launch at 64^4, from the one ncu --set full
-                # capture summarised in profiles/r01_pipe_kernel_full.md (4.831918 + 2.385510 GB)
-                "traffic": 7217428000 if args.L == 64 else None,
-                "traffic_source": "profiles/r01_pipe_kernel_full.md (ncu --set full, per launch)"}
+                "pin_rate_peak_source": "nvidia-smi clocks.max.mem %s MHz x 2 x %d bit / 8" % (mem_max, bus) if mem_max
+                                        else "cudaDevAttrMemoryClockRate x 2 x bus / 8",
+                "pin_rate_peak_cuda_attr": pin_attr,
+                "pin_rate_peak_cuda_attr_source": "cudaDevAttrMemoryClockRate %.0f MHz x 2 x %d bit / 8" % (r["info"]["mem_clock_khz"] / 1e3, bus),
+                "traffic": traffic, "traffic_source": traffic_src}
     cpu = None
     if rank == 0 and not args.no_cpu:
-        Lc = min(args.cpu_L, args.L)
-        times, nbytes, threads = oracle_step(Lc, 3)
-        cpu = {"value": nbytes / min(times) / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": "rows A1-A6 on a %d^4 fp64 lattice (a smaller point of the same sweep), best of 3 passes" % Lc}
-        t1, nb1, _ = oracle_step(min(Lc, 24), 1, threads=1)
-        cpu["one_thread_value"] = nb1 / min(t1) / 1e9
-        cpu["one_thread_sample"] = "the same rows on a %d^4 lattice, 1 thread, 1 pass" % min(Lc, 24)
+        cpu = run_cpu_baseline(args, r["host"])
     if r["dist"] is not None:
         r["dist"].barrier()
         r["dist"].destroy_process_group()
     if rank != 0:
         return
     line = {
-        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "warmup_steps_run": r["nwarm"],
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "gpu": r["gpu_name"], "steps": args.steps, "warmup": args.warmup, "warmup_steps_run": r["nwarm"],
         "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "BASELINE.json configs[4] top point: %d^4 lattice per GPU (%d matrices, %.3f GB per field), "
@@ -667,7 +872,8 @@ def main():
                    "parallelism": "independent x3 slabs, no collective" if world > 1 else "single GPU"},
         "GFLOPps": world * r["step_flops"] / (r["ms_per_step"] * 1e-3) / 1e9,
         "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
-        "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k != "wsweep"},
+        "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k not in ("wsweep", "by_size", "convert_f32")},
+        "ceilings_by_size": ceilings.get("by_size"), "convert_f32": ceilings.get("convert_f32"),
         "wsweep": ceilings.get("wsweep"), "next_rows": next_rows, "sweep": sweep, "checks": r["checks"],
         "wall_s_timed_region": r["t_wall"],
         # the paper's own numbers for z = x*y, as context only (other hardware, fp32, volumes unstated)

@@ -24,10 +24,12 @@
  *     NULL = legacy default stream) and return without synchronising.
  *   - `z` may be the SAME field as any input.  Partially overlapping fields are
  *     undefined.
- *   - Handles are immutable after wrap; calls are thread-safe (su3_tune_set is a
- *     process-wide knob and is the one exception: do not race it with launches).
- *   - One process drives one GPU (the device that is current at the first call): device facts and per-kernel
- *     attributes are cached per process.
+ *   - Handles are immutable after wrap; every call is thread-safe.  The only state besides handles is per
+ *     thread (the last-error string and the launch knobs of su3_tune_set) or keyed by device ordinal (cached
+ *     device facts and per-kernel attributes) or by (device, caller stream) (su3_eval_host's copy streams).
+ *   - A call launches on the device that is CURRENT on the calling thread; su3_field_wrap records which device
+ *     owns the memory (when the runtime can tell) and a call whose fields live elsewhere returns
+ *     SU3_ERR_MISMATCH instead of launching.  One process may drive several GPUs.
  *   - There is no CPU fallback anywhere: without a CUDA device the arithmetic
  *     calls return SU3_ERR_CUDA.
  *
@@ -81,8 +83,8 @@ typedef struct {
 
 typedef struct su3_field su3_field; /* opaque: validated descriptor + device pointer */
 
-/* Launch knobs (process-wide; 0 = library default).  They never change results, only speed; bench.py and the
- * tests use them to pin the launch configuration that is being measured.  Meaning per kernel family:
+/* Launch knobs of the CALLING THREAD (0 = library default).  They never change results, only speed; bench.py and
+ * the tests use them to pin the launch configuration that is being measured.  Meaning per kernel family:
  *   pipeline (su3_mul/mul3/mul_add/add, su3_matvec): tile_mats, stages = ring depth, ctas_per_sm, l2_hint, path
  *   su3_copy: tile = tile_mats x matrix bytes, stages, ctas_per_sm, l2_hint; path = 2 selects the plain LDG copy
  *   su3_expr (interpreted programs): stages = ring depth per warp (2..), ctas_per_sm; the tile is 32 matrices
@@ -211,7 +213,8 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *cuda_stream);
  * of x and y, the product kernel per chunk, and the device->host copy of z, overlapped on
  * internal copy streams, then makes cuda_stream wait for all of it.  Does not synchronise
  * the host; pinned host memory is needed for the copies to be asynchronous.  `chunks` <= 0
- * picks a default. */
+ * picks a default; more than 64 chunks -> SU3_ERR_INVALID.  The internal copy streams and events are
+ * kept per (device, cuda_stream): threads driving different streams do not serialise on each other. */
 su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host,
                         su3_field *zd, su3_field *xd, su3_field *yd, int chunks, void *cuda_stream);
 
@@ -223,7 +226,13 @@ typedef enum { SU3_OP_MUL = 0, SU3_OP_MUL3 = 1, SU3_OP_MUL_ADD = 2 } su3_op;
 su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
                          su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream);
 
-/* Launch knobs (see su3_tune).  su3_tune_set(NULL) restores the defaults. */
+/* Destroys the copy streams and events that su3_mul_host / su3_eval_host created (after waiting for their own
+ * copies).  Optional teardown; must not run concurrently with those two calls.  At most 64 distinct
+ * (device, stream) pairs may hold such resources at a time (SU3_ERR_SIZE beyond that). */
+su3_status su3_host_release(void);
+
+/* Launch knobs of the calling thread (see su3_tune; thread-local, so concurrent threads never race on them).
+ * su3_tune_set(NULL) restores the defaults. */
 su3_status su3_tune_set(const su3_tune *t);
 su3_status su3_tune_get(su3_tune *out);
 
@@ -233,6 +242,9 @@ int64_t su3_launch_count(void);
 /* Device facts the harness prints next to its numbers: SM count, L2 bytes, memory clock
  * (kHz), bus width (bits), of the current CUDA device.  SU3_ERR_CUDA without a device. */
 su3_status su3_device_info(int32_t *sm_count, int64_t *l2_bytes, int32_t *mem_clock_khz, int32_t *bus_width_bits);
+
+/* Name (NUL-terminated, truncated to buf_len) and ordinal of the current CUDA device. */
+su3_status su3_device_name(char *buf, size_t buf_len, int32_t *ordinal);
 
 #ifdef __cplusplus
 }

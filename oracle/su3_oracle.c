@@ -378,6 +378,33 @@ int orc_expr_real(int64_t n, int prec, int nops, const void *const *ops, const c
   return 0;
 }
 
+/* Host STREAM triad a[i] = b[i] + s*c[i] (the line the paper draws next to its curves), best of `reps`
+ * passes over n doubles, returned in GB/s counting 24 bytes per element.  A measurement aid of bench.py's
+ * cpu_baseline leg: it is NOT part of the method and nothing above uses it. */
+#include <stdlib.h>
+#include <time.h>
+double orc_stream_triad(int64_t n, int reps) {
+  double *a = malloc(sizeof(double) * (size_t)n), *b = malloc(sizeof(double) * (size_t)n), *c = malloc(sizeof(double) * (size_t)n);
+  double best = 0.0;
+  if (a && b && c && n > 0) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; i++) { a[i] = 0.0; b[i] = 1.0; c[i] = 2.0; } /* first touch */
+    for (int r = 0; r < reps; r++) {
+      struct timespec t0, t1;
+      clock_gettime(CLOCK_MONOTONIC, &t0);
+#pragma omp parallel for schedule(static)
+      for (int64_t i = 0; i < n; i++) a[i] = b[i] + 3.0 * c[i];
+      clock_gettime(CLOCK_MONOTONIC, &t1);
+      const double s = (double)(t1.tv_sec - t0.tv_sec) + 1e-9 * (double)(t1.tv_nsec - t0.tv_nsec);
+      const double gbs = 24.0 * (double)n / s / 1e9;
+      if (gbs > best) best = gbs;
+    }
+    if (a[n / 2] != 7.0) best = -1.0;
+  }
+  free(a); free(b); free(c);
+  return best;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -113,31 +113,35 @@ def _prec(a, g):
     raise TypeError(a.dtype)
 
 
-def _out(g):
-    return np.empty(g.nreals, dtype=np.float64)
+def _out(g, out=None):
+    """result buffer: a fresh fp64 array, or the caller's (bench.py times the oracle with first-touched outputs)"""
+    if out is None:
+        return np.empty(g.nreals, dtype=np.float64)
+    assert out.dtype == np.float64 and out.flags.c_contiguous and out.size == g.nreals
+    return out
 
 
-def mul(g, x, y):
+def mul(g, x, y, out=None):
     """z = x*y; x, y flat real arrays (fp32 or fp64) in layout g; returns fp64, layout g."""
     p = _prec(x, g)
     assert _prec(y, g) == p
-    z = _out(g)
+    z = _out(g, out)
     _load().orc_mul(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, z.ctypes.data)
     return z
 
 
-def mul3(g, x, y, w):
+def mul3(g, x, y, w, out=None):
     p = _prec(x, g)
     assert _prec(y, g) == p and _prec(w, g) == p
-    z = _out(g)
+    z = _out(g, out)
     _load().orc_mul3(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, w.ctypes.data, z.ctypes.data)
     return z
 
 
-def mul_add(g, x, y, v):
+def mul_add(g, x, y, v, out=None):
     p = _prec(x, g)
     assert _prec(y, g) == p and _prec(v, g) == p
-    z = _out(g)
+    z = _out(g, out)
     _load().orc_mul_add(ctypes.byref(g.c), p, x.ctypes.data, y.ctypes.data, v.ctypes.data, z.ctypes.data)
     return z
 
@@ -210,14 +214,25 @@ def expr_real(prog, *ops):
     return z
 
 
-def convert(g_dst, g_src, src):
+def convert(g_dst, g_src, src, out=None):
     """Bit-exact permutation of the reals of `src` (layout g_src) into layout g_dst."""
     p = _prec(src, g_src)
-    dst = np.empty_like(src)
+    dst = np.empty_like(src) if out is None else out
+    assert dst.dtype == src.dtype and dst.size == src.size and dst.flags.c_contiguous
     rc = _load().orc_convert(ctypes.byref(g_dst.c), ctypes.byref(g_src.c), p, dst.ctypes.data, src.ctypes.data)
     if rc:
         raise ValueError("geometry mismatch (orc_convert -> %d)" % rc)
     return dst
+
+
+def stream_triad(n, reps=3):
+    """host STREAM triad a = b + s*c over n doubles, best of `reps`, in GB/s (24 B per element; arrays first-touched
+    by the same OpenMP schedule).  A measurement aid for bench.py's cpu_baseline leg (the paper draws the STREAM
+    triad next to its curves); not part of the method."""
+    lib = _load()
+    lib.orc_stream_triad.argtypes = [ctypes.c_int64, ctypes.c_int]
+    lib.orc_stream_triad.restype = ctypes.c_double
+    return float(lib.orc_stream_triad(int(n), int(reps)))
 
 
 def num_threads():

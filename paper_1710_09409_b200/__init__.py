@@ -17,7 +17,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
            "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
-           "su3_tune_get", "su3_launch_count", "su3_device_info"]
+           "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release"]
 
 
 class su3_desc(ctypes.Structure):
@@ -74,6 +74,8 @@ def _load():
         "su3_tune_get": (i32, [T]),
         "su3_launch_count": (i64, []),
         "su3_device_info": (i32, [ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), ctypes.POINTER(i32)]),
+        "su3_device_name": (i32, [ctypes.c_char_p, sz, ctypes.POINTER(i32)]),
+        "su3_host_release": (i32, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -314,3 +316,14 @@ def su3_device_info():
     sm, l2, mk, bw = ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32()
     _ck(lib.su3_device_info(ctypes.byref(sm), ctypes.byref(l2), ctypes.byref(mk), ctypes.byref(bw)))
     return dict(sm_count=sm.value, l2_bytes=l2.value, mem_clock_khz=mk.value, bus_width_bits=bw.value)
+
+
+def su3_device_name():
+    """(name, ordinal) of the current CUDA device"""
+    buf, o = ctypes.create_string_buffer(128), ctypes.c_int32()
+    _ck(lib.su3_device_name(buf, len(buf), ctypes.byref(o)))
+    return buf.value.decode(), o.value
+
+
+def su3_host_release():
+    _ck(lib.su3_host_release())

@@ -8,6 +8,10 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <initializer_list>
+#include <map>
+#include <memory>
+#include <utility>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -20,7 +24,8 @@ struct su3_field {
   size_t nbytes;
   int64_t volume;
   int64_t nmat;
-  int ncomp;  // complex numbers per (site, mu): 9 = colour matrix, 3 = colour vector; 0 = real scalar field (1 real)
+  int ncomp;   // complex numbers per (site, mu): 9 = colour matrix, 3 = colour vector; 0 = real scalar field (1 real)
+  int device;  // ordinal of the device that owns ptr, -1 if the runtime could not tell at wrap time
 };
 
 namespace {
@@ -32,8 +37,8 @@ using su3tab::stream_kernel_t;
 
 thread_local char g_err[512] = "";
 std::atomic<int64_t> g_launches{0};
-std::mutex g_tune_mu;
-su3_tune g_tune = {0, 0, 0, 0, 0, {0, 0, 0}};
+// launch knobs of the CALLING THREAD (su3_tune_set): no process-wide state, so threads never race on them
+thread_local su3_tune g_tune = {0, 0, 0, 0, 0, {0, 0, 0}};
 
 su3_status fail(su3_status st, const char *fmt, ...) {
   va_list ap;
@@ -85,52 +90,78 @@ bool same_desc(const su3_desc &a, const su3_desc &b) {
   return same_lattice(a, b) && a.layout == b.layout && a.W == b.W && !memcmp(a.simd, b.simd, sizeof a.simd);
 }
 
-// ---------------------------------------------------------------- device facts (cached per process)
+// ---------------------------------------------------------------- device facts (cached per device ordinal)
+constexpr int MAX_DEVICES = 64;
 struct DevInfo {
   bool ok = false;
-  int sms = 0, smem_optin = 0, mem_khz = 0, bus_bits = 0;
+  int dev = -1, sms = 0, smem_optin = 0, mem_khz = 0, bus_bits = 0;
   long long l2 = 0;
+  char name[256] = "";
   char err[256] = "";
 };
+// Facts of the device that is CURRENT on the calling thread, looked up per call (cudaGetDevice is a thread-local read)
+// and cached per ordinal, so one process may drive several GPUs.  A failed query is not cached.
 const DevInfo &devinfo() {
-  static DevInfo di;
-  static std::once_flag once;
-  std::call_once(once, [] {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
+  static DevInfo table[MAX_DEVICES];
+  static std::mutex mu;
+  thread_local DevInfo bad;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess && (dev < 0 || dev >= MAX_DEVICES)) e = cudaErrorInvalidDevice;
+  if (e == cudaSuccess) {
+    std::lock_guard<std::mutex> lk(mu);
+    DevInfo &di = table[dev];
+    if (di.ok) return di;
     cudaDeviceProp pr;
-    if (e == cudaSuccess) e = cudaGetDeviceProperties(&pr, dev);
-    if (e != cudaSuccess) {
-      snprintf(di.err, sizeof di.err, "no usable CUDA device: %s", cudaGetErrorString(e));
-      (void)cudaGetLastError();
-      return;
+    e = cudaGetDeviceProperties(&pr, dev);
+    if (e == cudaSuccess) {
+      di.dev = dev;
+      di.sms = pr.multiProcessorCount;
+      di.smem_optin = (int)pr.sharedMemPerBlockOptin;
+      di.l2 = pr.l2CacheSize;
+      snprintf(di.name, sizeof di.name, "%s", pr.name);
+      int v = 0;
+      if (cudaDeviceGetAttribute(&v, cudaDevAttrMemoryClockRate, dev) == cudaSuccess) di.mem_khz = v;
+      if (cudaDeviceGetAttribute(&v, cudaDevAttrGlobalMemoryBusWidth, dev) == cudaSuccess) di.bus_bits = v;
+      di.ok = true;
+      return di;
     }
-    di.sms = pr.multiProcessorCount;
-    di.smem_optin = (int)pr.sharedMemPerBlockOptin;
-    di.l2 = pr.l2CacheSize;
-    int v = 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMemoryClockRate, dev) == cudaSuccess) di.mem_khz = v;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrGlobalMemoryBusWidth, dev) == cudaSuccess) di.bus_bits = v;
-    di.ok = true;
-  });
-  return di;
+  }
+  bad = DevInfo();
+  snprintf(bad.err, sizeof bad.err, "no usable CUDA device: %s", cudaGetErrorString(e));
+  (void)cudaGetLastError();
+  return bad;
 }
 
 // ---------------------------------------------------------------- kernel tables
-// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and process, not once per launch
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-DEVICE setting: once per (device, kernel), not per launch
 cudaError_t allow_max_smem(const void *fn, int bytes) {
   static std::mutex mu;
-  static std::vector<const void *> done;
+  static std::vector<std::pair<int, const void *>> done;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
   std::lock_guard<std::mutex> lk(mu);
-  for (const void *d : done)
-    if (d == fn) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) done.push_back(fn);
+  for (const auto &d : done)
+    if (d.first == dev && d.second == fn) return cudaSuccess;
+  e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) done.push_back({dev, fn});
   return e;
 }
 
 su3_status cuda_fail(const char *what, cudaError_t e) {
   return fail(SU3_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+// Every field of a call must live on the device that is current on the calling thread (the launch goes there).
+su3_status on_current_device(std::initializer_list<const su3_field *> fs) {
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  for (const su3_field *f : fs)
+    if (f && f->device >= 0 && f->device != di.dev)
+      return fail(SU3_ERR_MISMATCH, "field memory is on device %d but device %d is current on this thread (cudaSetDevice first)",
+                  f->device, di.dev);
+  return SU3_OK;
 }
 
 // Launch one arithmetic expression over `nmat` matrices starting at the given pointers.
@@ -139,11 +170,7 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (nmat == 0) return SU3_OK;
-  su3_tune tn;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    tn = g_tune;
-  }
+  const su3_tune tn = g_tune;
   const int nin = (op == su3::OP_MUL || op == su3::OP_ADD) ? 2 : 3;
   const int cb = 2 * prec;
   // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
@@ -233,6 +260,7 @@ su3_status check_arith(const su3_field *z, const su3_field *x, const su3_field *
 su3_status arith(int op, su3_field *z, const su3_field *x, const su3_field *y, const su3_field *u, void *stream) {
   su3_status st = check_arith(z, x, y, u, op != su3::OP_MUL);
   if (st != SU3_OK) return st;
+  if ((st = on_current_device({z, x, y, u})) != SU3_OK) return st;
   const size_t fp = z->nbytes * (op == su3::OP_MUL ? 3 : 4);
   return launch_stream(op, z->d.prec, z->d.W, z->ptr, x->ptr, y->ptr, u ? u->ptr : nullptr, z->nmat, fp,
                        (cudaStream_t)stream);
@@ -316,8 +344,8 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   if (z->ncomp != 9 || y->ncomp != 9 || (x && x->ncomp != 9)) return fail(SU3_ERR_MISMATCH, "colour-matrix fields expected");
   if (dim < 0 || dim > 3) return fail(SU3_ERR_INVALID, "dim = %d outside 0..3", dim);
   if (z->ptr == y->ptr) return fail(SU3_ERR_MISMATCH, "the output must not be the shifted operand's field");
+  if (su3_status sd = on_current_device({z, x, y})) return sd;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (z->nmat == 0) return SU3_OK;
   const su3_desc &d = z->d;
   su3::ShiftParams p;
@@ -333,11 +361,7 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   // 32-bit index arithmetic whenever every complex index (plus one tile of slack) fits 31 bits
   shift_kernel_t k = su3tab::shift_kernel(d.prec, op, d.W, (z->nmat + 64) * 9 < 0x7fffffffLL);
   if (!k) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
-  su3_tune tn;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    tn = g_tune;
-  }
+  const su3_tune tn = g_tune;
   if (op == su3::SH_COPY && tn.path != 2) {  // cp.async gather + TMA store (path = 2 keeps the register version)
     const bool small = (z->nmat + 64) * 9 < 0x7fffffffLL;
     shift_kernel_t ka = su3tab::cshift_async_kernel(d.prec, d.W, small);
@@ -367,8 +391,11 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   return SU3_OK;
 }
 
-// ---------------------------------------------------------------- y = U.psi
-// ---------------------------------------------------------------- su3_mul_host resources
+// ---------------------------------------------------------------- su3_mul_host / su3_eval_host resources
+// One set of copy streams and events per (device, caller stream): two host threads that drive different streams never
+// share anything and never serialise on each other; callers of the SAME stream are ordered by that stream anyway.
+constexpr int MAX_HOST_CHUNKS = 64;
+constexpr size_t MAX_HOST_PIPES = 64;
 struct HostPipe {
   std::mutex mu;
   cudaStream_t h2d = nullptr, d2h = nullptr;
@@ -384,8 +411,27 @@ struct HostPipe {
     }
     return e;
   }
+  void destroy() {  // waits for the pipe's own copies, then frees its streams and events
+    if (h2d) { cudaStreamSynchronize(h2d); cudaStreamDestroy(h2d); h2d = nullptr; }
+    if (d2h) { cudaStreamSynchronize(d2h); cudaStreamDestroy(d2h); d2h = nullptr; }
+    for (cudaEvent_t v : ev) cudaEventDestroy(v);
+    ev.clear();
+    (void)cudaGetLastError();
+  }
 };
-HostPipe g_hp;
+std::mutex g_hp_mu;  // guards the map only, never held across CUDA calls of a pipeline
+std::map<std::pair<int, cudaStream_t>, std::unique_ptr<HostPipe>> g_hp;
+
+HostPipe *host_pipe(int dev, cudaStream_t user) {
+  std::lock_guard<std::mutex> lk(g_hp_mu);
+  auto key = std::make_pair(dev, user);
+  auto it = g_hp.find(key);
+  if (it != g_hp.end()) return it->second.get();
+  if (g_hp.size() >= MAX_HOST_PIPES) return nullptr;
+  HostPipe *hp = new (std::nothrow) HostPipe;
+  if (hp) g_hp[key].reset(hp);
+  return hp;
+}
 
 }  // namespace
 
@@ -418,6 +464,11 @@ static su3_status wrap_kind(const su3_desc *desc, void *dev_ptr, size_t nbytes, 
   if (!f) return fail(SU3_ERR_SIZE, "out of host memory");
   f->d = d; f->ptr = dev_ptr; f->nbytes = need; f->volume = volume_of(d); f->nmat = f->volume * d.n_lorentz;
   f->ncomp = ncomp;
+  f->device = -1;  // which device owns the memory (asked once, here; never dereferenced)
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, dev_ptr) == cudaSuccess && (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged))
+    f->device = at.device;
+  (void)cudaGetLastError();
   *out = f;
   return SU3_OK;
 }
@@ -446,8 +497,8 @@ su3_status su3_real_bytes(const su3_desc *desc, size_t *nbytes) {
 su3_status su3_fill(su3_field *z, double value, void *cuda_stream) {
   if (!z) return fail(SU3_ERR_NULL, "field handle is NULL");
   if (z->ncomp != 0) return fail(SU3_ERR_MISMATCH, "su3_fill takes a real scalar field");
+  if (su3_status sd = on_current_device({z})) return sd;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (z->nmat == 0) return SU3_OK;
   const unsigned grid = flat_grid((size_t)z->nmat, 256, 8);
   if (z->d.prec == SU3_F64) su3::su3_real_fill_kernel<double><<<grid, 256, 0, (cudaStream_t)cuda_stream>>>((double *)z->ptr, z->nmat, value);
@@ -568,8 +619,10 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
     if (!same_desc(z->d, operands[k]->d) || operands[k]->ncomp != z->ncomp)
       return fail(SU3_ERR_MISMATCH, "operand %d: descriptor or field kind differs from z", k);
   }
+  if (su3_status sd = on_current_device({z})) return sd;
+  for (int k = 0; k < n_operands; k++)
+    if (su3_status sd = on_current_device({operands[k]})) return sd;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (z->nmat == 0) return SU3_OK;
   const bool real = z->ncomp == 0;
   // Real scalar fields (the paper's Listing 2) are element-wise, so n reals = n / 18 records of 18 reals for the
@@ -616,11 +669,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
       return launch_stream(op, z->d.prec, op == su3::OP_ADD ? 1 : W_eff, z->ptr, fx->ptr, fy->ptr, fu ? fu->ptr : nullptr, nrec,
                            z->nbytes * (fu ? 4 : 3), (cudaStream_t)cuda_stream);
   }
-  su3_tune tn;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    tn = g_tune;
-  }
+  const su3_tune tn = g_tune;
   const int cb = 2 * z->d.prec;
   expr_kernel_t k = su3tab::expr_kernel(z->d.prec, W_eff);
   if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", W_eff);
@@ -698,14 +747,10 @@ su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, vo
   if (U->ncomp != 9 || psi->ncomp != 3 || y->ncomp != 3)
     return fail(SU3_ERR_MISMATCH, "su3_matvec takes y, psi colour-vector fields and U a colour-matrix field");
   if (!same_desc(y->d, U->d) || !same_desc(y->d, psi->d)) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
+  if (su3_status sd = on_current_device({y, U, psi})) return sd;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (y->nmat == 0) return SU3_OK;
-  su3_tune tn;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    tn = g_tune;
-  }
+  const su3_tune tn = g_tune;
   const int cb = 2 * y->d.prec;
   stream_kernel_t k = su3tab::matvec_kernel(y->d.prec, y->d.W);
   if (!k) return fail(SU3_ERR_INVALID, "no matvec kernel for W %d", y->d.W);
@@ -737,13 +782,9 @@ su3_status su3_matvec(su3_field *y, const su3_field *U, const su3_field *psi, vo
 su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *stream) {
   su3_status st = check_arith(z, x, y, nullptr, false);
   if (st != SU3_OK) return st;
+  if ((st = on_current_device({z, x, y})) != SU3_OK) return st;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
-  int path;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    path = g_tune.path;
-  }
+  const int path = g_tune.path;
   if (path != 2)  // element-wise, hence layout-agnostic: the W = 1 pipeline over 9-complex records
     return launch_stream(su3::OP_ADD, z->d.prec, 1, z->ptr, x->ptr, y->ptr, nullptr, z->nmat, 3 * z->nbytes,
                          (cudaStream_t)stream);
@@ -764,11 +805,7 @@ static su3_status launch_copy(void *dst_ptr, const void *src_ptr, size_t nbytes,
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (nbytes == 0) return SU3_OK;
-  su3_tune tn;
-  {
-    std::lock_guard<std::mutex> lk(g_tune_mu);
-    tn = g_tune;
-  }
+  const su3_tune tn = g_tune;
   if (tn.path != 2) {  // TMA bulk pipeline: global -> shared -> global, one issuing thread per CTA
     const int mat_bytes = 18 * prec;
     const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 3;
@@ -805,6 +842,7 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *stream) {
   if (!dst || !src) return fail(SU3_ERR_NULL, "field handle is NULL");
   if (!same_desc(dst->d, src->d) || dst->ncomp != src->ncomp || dst->ncomp == 0)
     return fail(SU3_ERR_MISMATCH, "su3_copy needs identical descriptors and field kinds (matrix or vector)");
+  if (su3_status sd = on_current_device({dst, src})) return sd;
   return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);
 }
 
@@ -816,6 +854,7 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   if (dst->ptr == src->ptr) return fail(SU3_ERR_MISMATCH, "su3_convert: dst and src must not alias");
   if (dst->ncomp != src->ncomp || dst->ncomp == 0) return fail(SU3_ERR_MISMATCH, "su3_convert: matrix and vector fields cannot be mixed; real scalar fields have no layout");
   const int nc = dst->ncomp;
+  if (su3_status sd = on_current_device({dst, src})) return sd;
   if (dst->d.W == 1 && src->d.W == 1)  // the W = 1 vector layout is byte-identical to the scalar layout
     return launch_copy(dst->ptr, src->ptr, dst->nbytes, dst->d.prec, stream);
   const DevInfo &di = devinfo();
@@ -844,7 +883,7 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
     p.lane_off[l] = off * v.n_lorentz * nc;
   }
   if (p.nrec == 0) return SU3_OK;
-  const su3_tune tn_c = [] { std::lock_guard<std::mutex> lk(g_tune_mu); return g_tune; }();
+  const su3_tune tn_c = g_tune;
   // fp32 (and fp64 vector -> scalar with W >= 8): staged through shared memory; path = 2 forces the unstaged kernel
   const char *err = nullptr;
   if (!su3tab::launch_convert(v.prec, nc, v.W, tn_c.path != 2 && (v.prec == SU3_F32 || (v.W >= 8 && !p.to_vector)), p, (cudaStream_t)stream, &err))
@@ -862,19 +901,23 @@ su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y
   su3_status st = check_arith(zd, xd, yd, ud, has_u);
   if (st != SU3_OK) return st;
   if (!has_u && (u_host || ud)) return fail(SU3_ERR_INVALID, "SU3_OP_MUL takes no third operand");
+  if ((st = on_current_device({zd, xd, yd, ud})) != SU3_OK) return st;
   const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   cudaStream_t user = (cudaStream_t)cuda_stream;
   const int W = zd->d.W, prec = zd->d.prec;
   const int64_t nmat = zd->nmat;
   const size_t mat_bytes = (size_t)18 * prec;
   // chunk boundaries: multiples of 2*W matrices keep every chunk 16-byte aligned and lane-complete
   const int64_t gran = 2 * (int64_t)W;
+  if (chunks > MAX_HOST_CHUNKS) return fail(SU3_ERR_INVALID, "chunks = %d exceeds %d", chunks, MAX_HOST_CHUNKS);
   if (chunks <= 0) chunks = 8;
   int64_t per = (nmat + chunks - 1) / chunks;
   per = (per + gran - 1) / gran * gran;
   if (per < gran) per = gran;
   const int64_t nchunks = nmat ? (nmat + per - 1) / per : 0;
+  HostPipe *hp = host_pipe(di.dev, user);
+  if (!hp) return fail(SU3_ERR_SIZE, "more than %zu distinct (device, stream) pairs hold host pipelines; call su3_host_release()", MAX_HOST_PIPES);
+  HostPipe &g_hp = *hp;  // this (device, stream)'s resources
   std::lock_guard<std::mutex> lk(g_hp.mu);
   cudaError_t e = g_hp.ensure((size_t)(2 * nchunks + 2));
   if (e != cudaSuccess) return cuda_fail("su3_eval_host stream/event setup", e);
@@ -916,6 +959,24 @@ su3_status su3_mul_host(void *z_host, const void *x_host, const void *y_host, su
   return su3_eval_host(SU3_OP_MUL, z_host, x_host, y_host, nullptr, zd, xd, yd, nullptr, chunks, cuda_stream);
 }
 
+su3_status su3_host_release(void) {
+  std::map<std::pair<int, cudaStream_t>, std::unique_ptr<HostPipe>> old;
+  {
+    std::lock_guard<std::mutex> lk(g_hp_mu);
+    old.swap(g_hp);
+  }
+  int cur = 0;
+  const bool have = cudaGetDevice(&cur) == cudaSuccess;
+  for (auto &kv : old) {
+    std::lock_guard<std::mutex> lk(kv.second->mu);
+    if (have) cudaSetDevice(kv.first.first);
+    kv.second->destroy();
+  }
+  if (have) cudaSetDevice(cur);
+  (void)cudaGetLastError();
+  return SU3_OK;
+}
+
 su3_status su3_tune_set(const su3_tune *t) {
   su3_tune v = {0, 0, 0, 0, 0, {0, 0, 0}};
   if (t) v = *t;
@@ -925,19 +986,26 @@ su3_status su3_tune_set(const su3_tune *t) {
   if (v.ctas_per_sm < 0 || v.ctas_per_sm > 8) return fail(SU3_ERR_INVALID, "ctas_per_sm = %d outside 0..8", v.ctas_per_sm);
   if (v.l2_hint < 0 || v.l2_hint > 2) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..2", v.l2_hint);
   if (v.path < 0 || v.path > 3) return fail(SU3_ERR_INVALID, "path = %d outside 0..3", v.path);
-  std::lock_guard<std::mutex> lk(g_tune_mu);
   g_tune = v;
   return SU3_OK;
 }
 
 su3_status su3_tune_get(su3_tune *out) {
   if (!out) return fail(SU3_ERR_NULL, "out is NULL");
-  std::lock_guard<std::mutex> lk(g_tune_mu);
   *out = g_tune;
   return SU3_OK;
 }
 
 int64_t su3_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+su3_status su3_device_name(char *buf, size_t buf_len, int32_t *ordinal) {
+  if (!buf || buf_len == 0) return fail(SU3_ERR_NULL, "buf is NULL or empty");
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  snprintf(buf, buf_len, "%s", di.name);
+  if (ordinal) *ordinal = di.dev;
+  return SU3_OK;
+}
 
 su3_status su3_device_info(int32_t *sm_count, int64_t *l2_bytes, int32_t *mem_clock_khz, int32_t *bus_width_bits) {
   const DevInfo &di = devinfo();

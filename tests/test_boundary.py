@@ -261,3 +261,56 @@ def test_expression_front_end_builds_postfix_programs():
     assert postfix(x) == ("0", [x])
     with pytest.raises(TypeError):
         x + 1.0
+
+
+def test_tune_is_per_thread_and_argument_checks_do_not_race():
+    """no global state except thread-local data.  Two threads set different launch knobs and hammer the
+    argument checks of the launching calls; each must always read back ITS knobs and ITS error string."""
+    import threading
+    d = su3.make_desc(2)
+    need = su3.su3_field_bytes(d)
+    d32 = su3.make_desc(2, prec=su3.SU3_F32)
+    errors = []
+
+    def worker(k):
+        try:
+            su3.su3_tune_set(tile_mats=(32, 64, 128)[k % 3], stages=2 + k, ctas_per_sm=1 + k, path=1 + k % 3)
+            mine = su3.su3_tune_get()
+            h, h2 = ctypes.c_void_p(), ctypes.c_void_p()
+            assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000 * (k + 1)), need, ctypes.byref(h)) == su3.SU3_OK
+            assert su3.lib.su3_field_wrap(ctypes.byref(d32), ctypes.c_void_p(0x100000), need, ctypes.byref(h2)) == su3.SU3_OK
+            for it in range(400):
+                if k % 2:
+                    assert su3.lib.su3_mul(h, h, h2, None) == su3.SU3_ERR_MISMATCH
+                    assert "descriptors differ" in su3.su3_last_error()
+                else:
+                    assert su3.lib.su3_cshift(h, h2, 9, 1, None) in (su3.SU3_ERR_MISMATCH, su3.SU3_ERR_INVALID)
+                    assert su3.lib.su3_mul(h, None, h, None) == su3.SU3_ERR_NULL
+                    assert "NULL" in su3.su3_last_error()
+                assert su3.su3_tune_get() == mine
+            su3.lib.su3_field_free(h)
+            su3.lib.su3_field_free(h2)
+        except BaseException as e:   # noqa: BLE001 - reported below
+            errors.append((k, repr(e)))
+
+    su3.su3_tune_set()
+    ts = [threading.Thread(target=worker, args=(k,)) for k in range(6)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errors, errors
+    assert su3.su3_tune_get()["tile_mats"] == 0    # the main thread's knobs were never touched
+
+
+def test_eval_host_rejects_absurd_chunk_counts_before_any_cuda_work():
+    d = su3.make_desc(2)
+    h = ctypes.c_void_p()
+    su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), su3.su3_field_bytes(d), ctypes.byref(h))
+    import torch
+    if torch.cuda.is_available():
+        assert su3.lib.su3_eval_host(0, None, None, None, None, h, h, h, None, 1 << 20, None) == su3.SU3_ERR_INVALID
+    else:
+        assert su3.lib.su3_eval_host(0, None, None, None, None, h, h, h, None, 1 << 20, None) in (su3.SU3_ERR_INVALID, su3.SU3_ERR_CUDA)
+    assert su3.lib.su3_host_release() == su3.SU3_OK
+    su3.lib.su3_field_free(h)

@@ -297,3 +297,44 @@ def test_no_write_outside_the_output_field(prec, L, nl, layout, W):
         su3.su3_matvec(z, x, psi)
         intact(n, ("matvec", path))
     su3.su3_tune_set()
+
+
+def test_eval_host_from_two_threads_on_two_streams():
+    """su3_eval_host keeps its copy streams and events per (device, caller stream): two host threads, each on its own
+    stream, run chunked end-to-end products concurrently and both match the oracle; thread-local tune knobs differ."""
+    import threading
+    descs = [su3.make_desc((8, 8, 8, 12)), su3.make_desc((8, 8, 8, 12), prec=F32, layout=VE, W=8)]
+    data, results, errors = [], [None, None], []
+    for k, desc in enumerate(descs):
+        x, y = host_field(desc, 91 + k, su3gen.FIELD_X), host_field(desc, 91 + k, su3gen.FIELD_Y)
+        hx, hy = torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()
+        data.append((desc, x, y, hx, hy, torch.empty_like(hx).pin_memory(), [su3.alloc_field(desc) for _ in range(3)]))
+    torch.cuda.synchronize()
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            desc, x, y, hx, hy, hz, (zd, xd, yd) = data[k]
+            su3.su3_tune_set(path=1, tile_mats=32 if k else 64, stages=2 + k)
+            s = torch.cuda.Stream()
+            for it in range(25):
+                su3.su3_eval_host(su3.SU3_OP_MUL, hz, hx, hy, None, zd, xd, yd, None, chunks=3 + it % 5, stream=s.cuda_stream)
+            s.synchronize()
+            results[k] = hz.numpy().copy()
+        except BaseException as e:   # noqa: BLE001
+            errors.append((k, repr(e)))
+
+    ts = [threading.Thread(target=worker, args=(k,)) for k in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errors, errors
+    for k, (desc, x, y, *_rest) in enumerate(data):
+        err, _ = rel_err(results[k], oracle.mul(geom_of(desc), x, y), su3.su3_desc_normalize(desc).W)
+        assert err <= TOL[desc.prec], (k, err)
+    assert su3.su3_tune_get()["path"] == 0          # the workers' knobs were thread-local
+    su3.su3_host_release()
+    with pytest.raises(su3.Su3Error) as e:
+        su3.su3_eval_host(su3.SU3_OP_MUL, None, None, None, None, data[0][6][0], data[0][6][1], data[0][6][2], None, chunks=65)
+    assert e.value.status == su3.SU3_ERR_INVALID
