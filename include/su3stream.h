@@ -87,16 +87,21 @@ typedef struct su3_field su3_field; /* opaque: validated descriptor + device poi
  * the tests use them to pin the launch configuration that is being measured.  Meaning per kernel family:
  *   pipeline (su3_mul/mul3/mul_add/add, su3_matvec): tile_mats, stages = ring depth, ctas_per_sm, l2_hint, path
  *   su3_copy: tile = tile_mats x matrix bytes, stages, ctas_per_sm, l2_hint; path = 2 selects the plain LDG copy
- *   su3_expr (interpreted programs): stages = ring depth per warp (2..), ctas_per_sm; the tile is 32 matrices
- *   su3_cshift / su3_mul_shift: ctas_per_sm = blocks per SM of the grid; path = 2 selects the register Cshift
- *   su3_convert: path = 2 selects the unstaged kernel for fp32 */
+ *   su3_expr: programs on the ahead-of-time menu run on the pipeline (knobs as above); path = 3 forces the interpreter,
+ *             whose knobs are stages = ring depth per warp (2..) and ctas_per_sm; its tile is 32 matrices
+ *   su3_cshift / su3_mul_shift: default = the pipeline with a shifted operand (knobs as above); path = 2 the register
+ *             kernels, path = 3 the cp.async-gather Cshift; for those ctas_per_sm = blocks per SM of the grid
+ *   su3_convert: default = TMA bulk copies on both sides (tile_mats = 128: 36 KB tiles instead of 18 KB);
+ *                path = 3 the per-thread kernel staged through shared memory, path = 2 the unstaged kernel */
 typedef struct {
   int32_t tile_mats;    /* matrices per pipeline tile: 32, 64 or 128 (su3_copy: x matrix bytes) */
   int32_t stages;       /* shared-memory ring depth, 2..16                             */
   int32_t ctas_per_sm;  /* persistent CTAs per SM, 1..8                                 */
-  int32_t l2_hint;      /* 0 auto (= none), 1 none, 2 evict_first loads+stores         */
+  int32_t l2_hint;      /* 0 auto, 1 none, 2 evict_first loads+stores, 3 keep the first l2_pin_mb MB of every
+                           operand in L2 across calls (evict_last), stream the rest (evict_first)     */
   int32_t path;         /* 0 auto (by footprint and layout), 1 TMA-bulk pipeline, 2 direct per-lane LDG, 3 warp-staged */
-  int32_t reserved[3];
+  int32_t l2_pin_mb;    /* see l2_hint = 3                                                */
+  int32_t reserved[2];
 } su3_tune;
 
 /* Never NULL; thread-local; valid until the next failing call on this thread. */
@@ -156,6 +161,12 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
  * tK = temporary K, acc = accumulator; "spill tK" = the accumulator is parked in temporary K first.  Written
  * NUL-terminated into buf (SU3_ERR_SIZE if it does not fit).  Host-only; for debugging and for the tests. */
 su3_status su3_expr_disasm(const char *program, int n_operands, char *buf, size_t buf_len);
+
+/* Which kernel su3_expr would run for `program`: "menu <row> <row's postfix> <operand of slot 0> <slot 1> ..." when the
+ * compiled program is one of the ahead-of-time rows of the pipeline kernel (up to a renaming of the operands and the
+ * order of the sources of '+'), else "interpreter".  real_fields != 0: the operands are real scalar fields ('*' is
+ * element-wise).  Both routes give bit-identical results.  Host-only; for the tests and for bench.py's report. */
+su3_status su3_expr_plan(const char *program, int n_operands, int real_fields, char *buf, size_t buf_len);
 
 /* Accounting of a program by reading S9: field streams (n_operands + 1) and flops per matrix (198 per '*',
  * 18 per '+' or '-').  Validates the program like su3_expr.  Host-only. */

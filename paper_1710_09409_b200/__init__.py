@@ -16,7 +16,7 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
-           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
+           "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_expr_plan", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release"]
 
 
@@ -27,7 +27,8 @@ class su3_desc(ctypes.Structure):
 
 class su3_tune(ctypes.Structure):
     _fields_ = [("tile_mats", ctypes.c_int32), ("stages", ctypes.c_int32), ("ctas_per_sm", ctypes.c_int32),
-                ("l2_hint", ctypes.c_int32), ("path", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
+                ("l2_hint", ctypes.c_int32), ("path", ctypes.c_int32), ("l2_pin_mb", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 2)]
 
 
 class Su3Error(RuntimeError):
@@ -65,6 +66,7 @@ def _load():
         "su3_mul_shift": (i32, [vp, vp, vp, ctypes.c_int, ctypes.c_int, vp]),
         "su3_expr": (i32, [vp, ctypes.c_char_p, ctypes.POINTER(vp), ctypes.c_int, vp]),
         "su3_expr_disasm": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.c_char_p, sz]),
+        "su3_expr_plan": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.c_int, ctypes.c_char_p, sz]),
         "su3_expr_cost": (i32, [ctypes.c_char_p, ctypes.c_int, ctypes.POINTER(i32), ctypes.POINTER(i32)]),
         "su3_convert": (i32, [vp, vp, vp]),
         "su3_copy": (i32, [vp, vp, vp]),
@@ -208,6 +210,14 @@ def su3_expr_disasm(program, n_operands):
     return out
 
 
+def su3_expr_plan(program, n_operands, real_fields=False):
+    """"interpreter", or ("menu", row, row's postfix, [operand held by each slot]) for the ahead-of-time kernels"""
+    buf = ctypes.create_string_buffer(256)
+    _ck(lib.su3_expr_plan(program.encode(), int(n_operands), int(bool(real_fields)), buf, len(buf)))
+    t = buf.value.decode().split()
+    return "interpreter" if t[0] == "interpreter" else ("menu", int(t[1]), t[2], [int(v) for v in t[3:]])
+
+
 def su3_expr_cost(program, n_operands):
     """(field streams, flops per matrix) of a program by reading S9"""
     st, fl = ctypes.c_int32(), ctypes.c_int32()
@@ -297,15 +307,16 @@ def su3_eval_host(op, z_host, x_host, y_host, u_host, zd, xd, yd, ud, chunks=0, 
                           ud.handle if ud is not None else None, int(chunks), _stream(stream)))
 
 
-def su3_tune_set(tile_mats=0, stages=0, ctas_per_sm=0, l2_hint=0, path=0):
-    t = su3_tune(int(tile_mats), int(stages), int(ctas_per_sm), int(l2_hint), int(path))
+def su3_tune_set(tile_mats=0, stages=0, ctas_per_sm=0, l2_hint=0, path=0, l2_pin_mb=0):
+    t = su3_tune(int(tile_mats), int(stages), int(ctas_per_sm), int(l2_hint), int(path), int(l2_pin_mb))
     _ck(lib.su3_tune_set(ctypes.byref(t)))
 
 
 def su3_tune_get():
     t = su3_tune()
     _ck(lib.su3_tune_get(ctypes.byref(t)))
-    return dict(tile_mats=t.tile_mats, stages=t.stages, ctas_per_sm=t.ctas_per_sm, l2_hint=t.l2_hint, path=t.path)
+    return dict(tile_mats=t.tile_mats, stages=t.stages, ctas_per_sm=t.ctas_per_sm, l2_hint=t.l2_hint, path=t.path,
+                l2_pin_mb=t.l2_pin_mb)
 
 
 def su3_launch_count():

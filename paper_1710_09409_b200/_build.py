@@ -6,7 +6,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-UNITS = ["su3_api", "su3_k_stream_f64", "su3_k_stream_f32", "su3_k_shift", "su3_k_misc"]
+UNITS = ["su3_api", "su3_k_stream_f64", "su3_k_stream_f32", "su3_k_menu_f64", "su3_k_menu_f32", "su3_k_shiftpipe",
+         "su3_k_shift", "su3_k_misc"]
 SOURCES = [os.path.join(CSRC, u + ".cu") for u in UNITS]
 DEPS = SOURCES + [os.path.join(CSRC, "su3_kernels.cuh"), os.path.join(CSRC, "su3_tables.h"),
                   os.path.join(os.path.dirname(HERE), "include", "su3stream.h")]

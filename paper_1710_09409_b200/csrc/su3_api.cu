@@ -38,7 +38,7 @@ using su3tab::stream_kernel_t;
 thread_local char g_err[512] = "";
 std::atomic<int64_t> g_launches{0};
 // launch knobs of the CALLING THREAD (su3_tune_set): no process-wide state, so threads never race on them
-thread_local su3_tune g_tune = {0, 0, 0, 0, 0, {0, 0, 0}};
+thread_local su3_tune g_tune = {0, 0, 0, 0, 0, 0, {0, 0}};
 
 su3_status fail(su3_status st, const char *fmt, ...) {
   va_list ap;
@@ -164,29 +164,37 @@ su3_status on_current_device(std::initializer_list<const su3_field *> fs) {
   return SU3_OK;
 }
 
-// Launch one arithmetic expression over `nmat` matrices starting at the given pointers.
-su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const void *y, const void *u, int64_t nmat,
-                         size_t footprint_bytes, cudaStream_t stream) {
+// Launch one ahead-of-time program (su3_kernels.cuh: menu_prog(op)) over `nmat` matrices starting at the given
+// pointers; `sh` != NULL: the last operand is read at the shifted site (pipeline only).
+su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in, int64_t nmat,
+                         size_t footprint_bytes, cudaStream_t stream, const su3::ShiftInfo *sh = nullptr) {
   const DevInfo &di = devinfo();
   if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
   if (nmat == 0) return SU3_OK;
   const su3_tune tn = g_tune;
-  const int nin = (op == su3::OP_MUL || op == su3::OP_ADD) ? 2 : 3;
+  const int nin = su3::menu_prog(op).nin;
+  const int nslot = (sh && nin == 1) ? 2 : nin;
   const int cb = 2 * prec;
+  const bool base_op = op <= su3::OP_ADD && !sh;  // the direct and warp-staged kernels exist for su3_mul/mul3/mul_add(/add) only
   // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
   // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
   // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
-  const bool direct = op != su3::OP_ADD &&  // OP_ADD has no direct kernel (su3_add's path = 2 is its own plain kernel)
+  const bool direct = base_op && op != su3::OP_ADD &&  // OP_ADD has no direct kernel (su3_add's path = 2 is its own plain kernel)
                       (tn.path == 2 || (tn.path == 0 && W * cb >= 32 &&
                                         footprint_bytes <= (size_t)di.l2 * 2));  // measured cross-over with the pipeline: ~2 x L2
-  const bool warp = !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
+  const bool warp = base_op && !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
   const int family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
-  stream_kernel_t k = prec == SU3_F64 ? su3tab::stream_f64(family, op, W) : su3tab::stream_f32(family, op, W);
+  stream_kernel_t k = nullptr;
+  if (sh) k = su3tab::shift_pipe_kernel(prec, op, W);
+  else if (op <= su3::OP_ADD) k = prec == SU3_F64 ? su3tab::stream_f64(family, op, W) : su3tab::stream_f32(family, op, W);
+  else k = prec == SU3_F64 ? su3tab::menu_f64(op, W) : su3tab::menu_f32(op, W);
   if (!k) return fail(SU3_ERR_INVALID, "no kernel for op %d prec %d W %d", op, prec, W);
 
   su3::StreamParams p;
-  p.z = z; p.x = x; p.y = y; p.u = u; p.nmat = nmat;
-  p.hint = tn.l2_hint == 2 ? 1 : 0;  // auto = no hint: evict_first measured neutral (+-0.5 %) at every size, DESIGN.md 6.1
+  memset(&p, 0, sizeof p);
+  p.z = z; p.x = in[0]; p.y = nin > 1 ? in[1] : nullptr; p.u = nin > 2 ? in[2] : nullptr; p.v = nin > 3 ? in[3] : nullptr;
+  p.nmat = nmat;
+  if (sh) p.sh = *sh;
 
   if (warp) {
     p.tile_mats = 32; p.stages = 0;
@@ -218,7 +226,7 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
       while (tm > 32 && (nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
     }
     if (tm != 32 && tm != 64 && tm != 128) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128}", tm);
-    const size_t stage_bytes = (size_t)nin * tm * 9 * cb;
+    const size_t stage_bytes = (size_t)nslot * tm * 9 * cb + (sh ? 16 : 0);
     // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
     size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
     // auto CTAs/SM: a big tile may leave room for fewer resident CTAs than the default
@@ -233,11 +241,15 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *x, const 
       while (stages > 2 && stages * stage_bytes + 256 > budget) stages--;
     }
     if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);
-    const size_t smem = stages * stage_bytes + 2 * stages * sizeof(uint64_t);
+    const size_t smem = stages * stage_bytes + 3 * stages * sizeof(uint64_t);
     if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "pipeline needs %zu B of shared memory, device allows %d", smem, di.smem_optin);
     cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
     if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
     p.tile_mats = tm; p.stages = stages;
+    // L2 policy (l2_hint): 0/1 none (evict_first measured neutral at every HBM-bound size), 2 evict_first
+    // everywhere, 3 keep the first l2_pin_mb MB of every operand in L2 (evict_last) and stream the rest (evict_first)
+    p.hint = tn.l2_hint == 2 ? 1 : (tn.l2_hint == 3 ? 2 : 0);
+    if (p.hint == 2) p.pin_tiles = (int64_t)((size_t)tn.l2_pin_mb * 1000000 / ((size_t)tm * 9 * cb));
     const int64_t ntiles = (nmat + tm - 1) / tm;
     const unsigned grid = (unsigned)(ntiles < max_grid ? ntiles : max_grid);
     k<<<grid, (NCW + 1) * 32, smem, stream>>>(p);
@@ -262,8 +274,8 @@ su3_status arith(int op, su3_field *z, const su3_field *x, const su3_field *y, c
   if (st != SU3_OK) return st;
   if ((st = on_current_device({z, x, y, u})) != SU3_OK) return st;
   const size_t fp = z->nbytes * (op == su3::OP_MUL ? 3 : 4);
-  return launch_stream(op, z->d.prec, z->d.W, z->ptr, x->ptr, y->ptr, u ? u->ptr : nullptr, z->nmat, fp,
-                       (cudaStream_t)stream);
+  const void *in[4] = {x->ptr, y->ptr, u ? u->ptr : nullptr, nullptr};
+  return launch_stream(op, z->d.prec, z->d.W, z->ptr, in, z->nmat, fp, (cudaStream_t)stream);
 }
 
 unsigned flat_grid(size_t n_items, size_t per_block, int blocks_per_sm) {
@@ -337,6 +349,46 @@ su3_status compile_expr(const char *prog, int nops, ExprProgram *out) {
   return SU3_OK;
 }
 
+// Does the compiled program equal row `op` of the ahead-of-time menu, up to a renaming of the operands and the order
+// of the two sources of a commutative element-wise instruction?  map[k] = user operand held by menu slot k.
+bool match_menu_from(const ExprProgram &pr, const su3::MenuProg &mp, int i, int map[4]) {
+  if (i == pr.nins) return true;
+  const su3::ExprIns u = pr.ins[i], m = mp.ins[i];
+  if (u.op != m.op || u.spill != m.spill) return false;
+  const int tries = (u.op == su3::EX_ADD || u.op == su3::EX_EMUL) ? 2 : 1;   // IEEE + and * are commutative bit for bit
+  for (int t = 0; t < tries; t++) {
+    const unsigned char ua = t ? u.b : u.a, ub = t ? u.a : u.b;
+    int saved[4] = {map[0], map[1], map[2], map[3]};
+    auto bind = [&](unsigned char us, unsigned char ms) {
+      if (ms >= su3::EX_TEMP0) return us == ms;          // temporaries and the accumulator must agree literally
+      if (us >= su3::EX_TEMP0) return false;
+      if (map[ms] < 0) {
+        for (int k = 0; k < 4; k++)
+          if (map[k] == us) return false;                // injective: one slot per distinct field
+        map[ms] = us;
+        return true;
+      }
+      return map[ms] == us;
+    };
+    if (bind(ua, m.a) && (u.op == su3::EX_COPY || bind(ub, m.b)) && match_menu_from(pr, mp, i + 1, map)) return true;
+    for (int k = 0; k < 4; k++) map[k] = saved[k];
+  }
+  return false;
+}
+int match_menu(const ExprProgram &pr, int nops, bool real, int map[4]) {
+  for (int op = 0; op < su3::OP_COPY; op++) {
+    const su3::MenuProg mp = su3::menu_prog(op);
+    if (mp.nin != nops || mp.nins != pr.nins) continue;
+    if (real && !su3tab::menu_elementwise(op)) continue;
+    if (!real && (op == su3::OP_EMUL || op == su3::OP_SUM_EPROD)) continue;
+    map[0] = map[1] = map[2] = map[3] = -1;
+    if (match_menu_from(pr, mp, 0, map)) return op;
+  }
+  return -1;
+}
+const char *const kMenuPostfix[su3::OP_COUNT] = {"01*", "01*2*", "01*2+", "01+", "01+01*+", "01*23*+", "01*23*-", "01*2-",
+                                                 "01+2+", "01+2+3+", "01-", "01*", "01+01*+", "0"};
+
 // ---------------------------------------------------------------- Cshift / shifted product
 su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
   if (!z || !y || (op == su3::SH_MUL && !x)) return fail(SU3_ERR_NULL, "field handle is NULL");
@@ -362,6 +414,19 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   shift_kernel_t k = su3tab::shift_kernel(d.prec, op, d.W, (z->nmat + 64) * 9 < 0x7fffffffLL);
   if (!k) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
   const su3_tune tn = g_tune;
+  // Default: the TMA pipeline with a shifted operand -- the sources of a tile are a few contiguous runs of records, moved
+  // by bulk copies; across the sub-lattice boundary the consumer reads a rotated lane.  With 72-byte records (fp32,
+  // scalar layout) all runs of a launch must agree in (source - destination) mod 16, true unless r[dim]*P is odd.
+  const int64_t P = p.ostride * d.n_lorentz;
+  const bool odd72 = d.prec == SU3_F32 && d.W == 1 && ((int64_t)p.rd * P) % 2 != 0;
+  if ((tn.path == 0 || tn.path == 1) && !odd72 && P < 0x7fffffffLL) {
+    su3::ShiftInfo sh;
+    sh.P = P; sh.rd = p.rd; sh.dmod = p.disp % p.rd; sh.qrot = p.disp / p.rd; sh.simd_d = p.simd_d; sh.lstride = p.lstride;
+    sh.phase = (d.prec == SU3_F32 && d.W == 1 && ((int64_t)sh.dmod * P) % 2) ? 8 : 0;
+    const void *in[4] = {op == su3::SH_MUL ? x->ptr : y->ptr, op == su3::SH_MUL ? y->ptr : nullptr, nullptr, nullptr};
+    return launch_stream(op == su3::SH_MUL ? su3::OP_MUL : su3::OP_COPY, d.prec, d.W, z->ptr, in, z->nmat,
+                         z->nbytes * (op == su3::SH_MUL ? 3 : 2), (cudaStream_t)stream, &sh);
+  }
   if (op == su3::SH_COPY && tn.path != 2) {  // cp.async gather + TMA store (path = 2 keeps the register version)
     const bool small = (z->nmat + 64) * 9 < 0x7fffffffLL;
     shift_kernel_t ka = su3tab::cshift_async_kernel(d.prec, d.W, small);
@@ -598,6 +663,26 @@ su3_status su3_expr_disasm(const char *program, int n_operands, char *buf, size_
   return SU3_OK;
 }
 
+su3_status su3_expr_plan(const char *program, int n_operands, int real_fields, char *buf, size_t buf_len) {
+  if (!buf || buf_len == 0) return fail(SU3_ERR_NULL, "buf is NULL or empty");
+  ExprProgram pr;
+  su3_status st = compile_expr(program, n_operands, &pr);
+  if (st != SU3_OK) return st;
+  if (real_fields)
+    for (int i = 0; i < pr.nins; i++)
+      if (pr.ins[i].op == su3::EX_MUL) pr.ins[i].op = su3::EX_EMUL;
+  int map[4];
+  const int op = match_menu(pr, n_operands, real_fields != 0, map);
+  int n;
+  if (op < 0) n = snprintf(buf, buf_len, "interpreter");
+  else {
+    n = snprintf(buf, buf_len, "menu %d %s", op, kMenuPostfix[op]);
+    for (int k = 0; k < n_operands && n > 0 && (size_t)n < buf_len; k++) n += snprintf(buf + n, buf_len - n, " %d", map[k]);
+  }
+  if (n < 0 || (size_t)n >= buf_len) return fail(SU3_ERR_SIZE, "plan needs more than %zu bytes", buf_len);
+  return SU3_OK;
+}
+
 su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix) {
   ExprProgram pr;
   su3_status st = compile_expr(program, n_operands, &pr);
@@ -650,24 +735,16 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
     if (nrec == 0) return SU3_OK;
   }
   {
-    // the fixed menu: programs that ARE one of the ahead-of-time kernels run on them (same FMA chain, so the
-    // result is bit-identical either way; IEEE addition is commutative, so v + x*y is x*y + v)
-    const su3::ExprIns *in = pr.ins;
-    const bool first_on_operands = in[0].a < su3::EX_TEMP0 && in[0].b < su3::EX_TEMP0;
-    int op = -1;
-    const su3_field *fx = nullptr, *fy = nullptr, *fu = nullptr;
-    if (pr.nins >= 1 && first_on_operands && (in[0].op == su3::EX_MUL || in[0].op == su3::EX_ADD) && (!real || pr.nins == 1)) {
-      fx = operands[in[0].a]; fy = operands[in[0].b];
-      if (pr.nins == 1) op = in[0].op == su3::EX_MUL ? su3::OP_MUL : su3::OP_ADD;
-      else if (pr.nins == 2 && in[0].op == su3::EX_MUL && in[1].spill == su3::EX_NONE) {
-        if (in[1].op == su3::EX_MUL && in[1].a == su3::EX_SRC_ACC && in[1].b < su3::EX_TEMP0) { op = su3::OP_MUL3; fu = operands[in[1].b]; }
-        else if (in[1].op == su3::EX_ADD && in[1].a == su3::EX_SRC_ACC && in[1].b < su3::EX_TEMP0) { op = su3::OP_MUL_ADD; fu = operands[in[1].b]; }
-        else if (in[1].op == su3::EX_ADD && in[1].b == su3::EX_SRC_ACC && in[1].a < su3::EX_TEMP0) { op = su3::OP_MUL_ADD; fu = operands[in[1].a]; }
-      }
+    // the ahead-of-time menu: programs that ARE one of the compiled-in kernels run on them (same FMA chains, same
+    // order of operations as the interpreter, so the result is bit-identical either way)
+    int map[4];
+    const int op = g_tune.path == 3 ? -1 : match_menu(pr, n_operands, real, map);   // path = 3: always the interpreter
+    if (op >= 0) {
+      const void *in[4] = {nullptr, nullptr, nullptr, nullptr};
+      for (int k = 0; k < n_operands; k++) in[k] = operands[map[k]]->ptr;
+      return launch_stream(op, z->d.prec, su3tab::menu_elementwise(op) ? 1 : W_eff, z->ptr, in, nrec,
+                           z->nbytes * (n_operands + 1), (cudaStream_t)cuda_stream);
     }
-    if (op >= 0)
-      return launch_stream(op, z->d.prec, op == su3::OP_ADD ? 1 : W_eff, z->ptr, fx->ptr, fy->ptr, fu ? fu->ptr : nullptr, nrec,
-                           z->nbytes * (fu ? 4 : 3), (cudaStream_t)cuda_stream);
   }
   const su3_tune tn = g_tune;
   const int cb = 2 * z->d.prec;
@@ -785,9 +862,10 @@ su3_status su3_add(su3_field *z, const su3_field *x, const su3_field *y, void *s
   if ((st = on_current_device({z, x, y})) != SU3_OK) return st;
   const DevInfo &di = devinfo();
   const int path = g_tune.path;
-  if (path != 2)  // element-wise, hence layout-agnostic: the W = 1 pipeline over 9-complex records
-    return launch_stream(su3::OP_ADD, z->d.prec, 1, z->ptr, x->ptr, y->ptr, nullptr, z->nmat, 3 * z->nbytes,
-                         (cudaStream_t)stream);
+  if (path != 2) {  // element-wise, hence layout-agnostic: the W = 1 pipeline over 9-complex records
+    const void *in[4] = {x->ptr, y->ptr, nullptr, nullptr};
+    return launch_stream(su3::OP_ADD, z->d.prec, 1, z->ptr, in, z->nmat, 3 * z->nbytes, (cudaStream_t)stream);
+  }
   const size_t n16 = z->nbytes / 16;
   const int nrem = (int)((z->nbytes % 16) / z->d.prec);
   const unsigned grid = flat_grid(n16, 512, 8);
@@ -884,9 +962,36 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   }
   if (p.nrec == 0) return SU3_OK;
   const su3_tune tn_c = g_tune;
-  // fp32 (and fp64 vector -> scalar with W >= 8): staged through shared memory; path = 2 forces the unstaged kernel
+  // records whose scalar-side images are contiguous: up to the first dimension that is split over virtual nodes
+  long long run_sites = 1;
+  {
+    int k = 0;
+    for (; k < 4; k++) {
+      run_sites *= p.r[k];
+      if (v.simd[k] > 1) break;
+    }
+  }
+  p.run_recs = run_sites * v.n_lorentz;
   const char *err = nullptr;
-  if (!su3tab::launch_convert(v.prec, nc, v.W, tn_c.path != 2 && (v.prec == SU3_F32 || (v.W >= 8 && !p.to_vector)), p, (cudaStream_t)stream, &err))
+  // Default: the TMA kernel (bulk copies on both sides, transposition in shared memory).  With 8-byte complex numbers its
+  // bulk copies are 16-byte aligned only if every run starts and ends on an even complex index; odd geometries (and
+  // path = 2 / 3, kept for measurements) take the per-thread kernels: 3 = staged through shared memory, 2 = unstaged.
+  bool tma = tn_c.path == 0 || tn_c.path == 1;
+  if (tma && v.prec == SU3_F32) {
+    tma = (p.run_recs * nc) % 2 == 0;
+    for (int l = 0; l < v.W; l++) tma = tma && p.lane_off[l] % 2 == 0;
+  }
+  if (tma) {
+    const bool big = tn_c.tile_mats == 128;
+    const int K = su3tab::convert_tma_tile(v.prec, big) / v.W;             // complex numbers per lane row
+    const int phase = v.prec == SU3_F32 ? 16 : 8;                          // complex numbers per 128-byte wavefront
+    const int want = v.W < phase ? phase / v.W : 1;
+    int pad = ((want - K) % phase + phase) % phase;
+    if (v.prec == SU3_F32 && ((K + pad) & 1)) pad += 1;                    // rows must stay 16-byte aligned
+    p.pitch = K + pad;
+    if (!su3tab::launch_convert_tma(v.prec, nc, v.W, big, p, (cudaStream_t)stream, &err))
+      return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");
+  } else if (!su3tab::launch_convert(v.prec, nc, v.W, tn_c.path != 2 && (v.prec == SU3_F32 || (v.W >= 8 && !p.to_vector)), p, (cudaStream_t)stream, &err))
     return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_convert launch", e);
@@ -940,8 +1045,8 @@ su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y
     if (u_host) SU3_CK(cudaMemcpyAsync((char *)ud->ptr + off, (const char *)u_host + off, len, cudaMemcpyHostToDevice, g_hp.h2d));
     SU3_CK(cudaEventRecord(ev_in, g_hp.h2d));
     SU3_CK(cudaStreamWaitEvent(user, ev_in, 0));
-    st = launch_stream(op, prec, W, (char *)zd->ptr + off, (const char *)xd->ptr + off, (const char *)yd->ptr + off,
-                       has_u ? (const char *)ud->ptr + off : nullptr, nm, (has_u ? 4 : 3) * zd->nbytes, user);
+    const void *in[4] = {(const char *)xd->ptr + off, (const char *)yd->ptr + off, has_u ? (const char *)ud->ptr + off : nullptr, nullptr};
+    st = launch_stream(op, prec, W, (char *)zd->ptr + off, in, nm, (has_u ? 4 : 3) * zd->nbytes, user);
     if (st != SU3_OK) return st;
     SU3_CK(cudaEventRecord(ev_k, user));
     SU3_CK(cudaStreamWaitEvent(g_hp.d2h, ev_k, 0));
@@ -978,13 +1083,14 @@ su3_status su3_host_release(void) {
 }
 
 su3_status su3_tune_set(const su3_tune *t) {
-  su3_tune v = {0, 0, 0, 0, 0, {0, 0, 0}};
+  su3_tune v = {0, 0, 0, 0, 0, 0, {0, 0}};
   if (t) v = *t;
   if (v.tile_mats != 0 && v.tile_mats != 32 && v.tile_mats != 64 && v.tile_mats != 128)
     return fail(SU3_ERR_INVALID, "tile_mats = %d not in {0,32,64,128}", v.tile_mats);
   if (v.stages != 0 && (v.stages < 2 || v.stages > 16)) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16", v.stages);
   if (v.ctas_per_sm < 0 || v.ctas_per_sm > 8) return fail(SU3_ERR_INVALID, "ctas_per_sm = %d outside 0..8", v.ctas_per_sm);
-  if (v.l2_hint < 0 || v.l2_hint > 2) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..2", v.l2_hint);
+  if (v.l2_hint < 0 || v.l2_hint > 3) return fail(SU3_ERR_INVALID, "l2_hint = %d outside 0..3", v.l2_hint);
+  if (v.l2_pin_mb < 0) return fail(SU3_ERR_INVALID, "l2_pin_mb = %d is negative", v.l2_pin_mb);
   if (v.path < 0 || v.path > 3) return fail(SU3_ERR_INVALID, "path = %d outside 0..3", v.path);
   g_tune = v;
   return SU3_OK;

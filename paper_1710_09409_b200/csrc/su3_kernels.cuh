@@ -30,7 +30,6 @@
 
 namespace su3 {
 
-enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2, OP_ADD = 3 };
 
 // ---------------------------------------------------------------- complex helpers
 template <typename R> struct Cplx;
@@ -145,37 +144,169 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// ---------------------------------------------------------------- the streaming pipeline (A1-A4)
+// ---------------------------------------------------------------- the streaming pipeline (A1-A4, menu programs, shifts)
+// Register-machine instructions shared by the ahead-of-time menu below and by the interpreter (su3_expr_kernel):
+// sources 0..7 = operand slot of the stage, 8..15 = temporary, 255 = accumulator; the result goes to the accumulator;
+// `spill` parks the accumulator in a temporary first.
+enum { EX_MUL = 0, EX_ADD = 1, EX_SUB = 2, EX_COPY = 3, EX_EMUL = 4,  // EMUL: element-wise product of the reals (real scalar fields)
+       EX_SRC_ACC = 255, EX_NONE = 255, EX_TEMP0 = 8 };
+struct ExprIns {
+  unsigned char op, a, b, spill;
+};
+
+// The ahead-of-time menu: small programs compiled INTO the pipeline kernel (template parameter OP), so that the whole
+// tree is evaluated in registers by straight-line code (the expression is evaluated inside the one site loop;
+// this is the ahead-of-time counterpart of the paper's Jitify back-end).  su3_expr matches a compiled program
+// against these rows (up to a renaming of the operands and the order of the two sources of '+') and runs the
+// interpreter only for programs that are not on the menu.  Rows 0-3 are su3_mul, su3_mul3, su3_mul_add, su3_add.
+enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2, OP_ADD = 3,
+       OP_SUM_PROD = 4,     // a + b + a*b        "01+01*+"   (the paper's Listing 2 on matrices)
+       OP_MUL_MUL_ADD = 5,  // a*b + c*d          "01*23*+"
+       OP_MUL_MUL_SUB = 6,  // a*b - c*d          "01*23*-"
+       OP_MUL_SUB = 7,      // a*b - c            "01*2-"
+       OP_ADD3 = 8,         // a + b + c          "01+2+"
+       OP_ADD4 = 9,         // a + b + c + d      "01+2+3+"
+       OP_SUB = 10,         // a - b              "01-"
+       OP_EMUL = 11,        // reals: a*b         "01*" on real scalar fields
+       OP_SUM_EPROD = 12,   // reals: a + b + a*b "01+01*+" on real scalar fields (Listing 2 itself)
+       OP_COPY = 13,        // z = a (only used with a shifted operand: Cshift)
+       OP_COUNT = 14 };
+struct MenuProg {
+  int nin, nins, min_ctas;  // operands, instructions, resident CTAs per SM the registers must allow
+  ExprIns ins[4];
+};
+__host__ __device__ constexpr MenuProg menu_prog(int op) {
+  constexpr unsigned char A = EX_SRC_ACC, N = EX_NONE, T = EX_TEMP0;
+  switch (op) {
+    case OP_MUL: return {2, 1, 3, {{EX_MUL, 0, 1, N}}};
+    case OP_MUL3: return {3, 2, 3, {{EX_MUL, 0, 1, N}, {EX_MUL, A, 2, N}}};
+    case OP_MUL_ADD: return {3, 2, 3, {{EX_MUL, 0, 1, N}, {EX_ADD, A, 2, N}}};
+    case OP_ADD: return {2, 1, 3, {{EX_ADD, 0, 1, N}}};
+    case OP_SUM_PROD: return {2, 3, 2, {{EX_ADD, 0, 1, N}, {EX_MUL, 0, 1, T}, {EX_ADD, T, A, N}}};
+    case OP_MUL_MUL_ADD: return {4, 3, 2, {{EX_MUL, 0, 1, N}, {EX_MUL, 2, 3, T}, {EX_ADD, T, A, N}}};
+    case OP_MUL_MUL_SUB: return {4, 3, 2, {{EX_MUL, 0, 1, N}, {EX_MUL, 2, 3, T}, {EX_SUB, T, A, N}}};
+    case OP_MUL_SUB: return {3, 2, 3, {{EX_MUL, 0, 1, N}, {EX_SUB, A, 2, N}}};
+    case OP_ADD3: return {3, 2, 3, {{EX_ADD, 0, 1, N}, {EX_ADD, A, 2, N}}};
+    case OP_ADD4: return {4, 3, 2, {{EX_ADD, 0, 1, N}, {EX_ADD, A, 2, N}, {EX_ADD, A, 3, N}}};
+    case OP_SUB: return {2, 1, 3, {{EX_SUB, 0, 1, N}}};
+    case OP_EMUL: return {2, 1, 3, {{EX_EMUL, 0, 1, N}}};
+    case OP_SUM_EPROD: return {2, 3, 3, {{EX_ADD, 0, 1, N}, {EX_EMUL, 0, 1, T}, {EX_ADD, T, A, N}}};
+    case OP_COPY: return {1, 1, 3, {{EX_COPY, 0, N, N}}};
+  }
+  return {0, 0, 1, {}};
+}
+
+// A shifted operand (f3): the LAST operand of the program is read at site s + disp*dim_hat.  In storage order a
+// tile's sources are a few CONTIGUOUS runs of whole records: with oc = the outer coordinate of a record in the shifted
+// dimension, records with oc + dmod < rd come from record + dmod*P, the others ("carry": they wrap around the
+// sub-lattice) from record + (dmod - rd)*P, and oc advances every P = ostride*nl records.  The producer moves every
+// run with one bulk copy; a consumer thread then reads its matrix from lane (ic + qrot + carry) mod simd_d instead of
+// its own lane ic: across the sub-lattice boundary a shift is a lane rotation (the virtual-node map S3).
+struct ShiftInfo {
+  long long P;     // records per step of oc: prod_{k<dim} r[k] * n_lorentz
+  int rd;          // r[dim] = L[dim] / simd[dim]
+  int dmod, qrot;  // disp = qrot*rd + dmod, 0 <= disp < L[dim]
+  int simd_d, lstride;  // simd[dim], prod_{k<dim} simd[k]
+  int phase;       // fp32 scalar layout only: byte offset (0 or 8) of the shifted slot that makes source and destination
+                   // of every run agree mod 16 (records are 72 B; bulk copies need 16-byte alignment)
+};
+
 struct StreamParams {
   void *z;
   const void *x;
   const void *y;
   const void *u;   // third operand: w (OP_MUL3) or v (OP_MUL_ADD); unused for OP_MUL
+  const void *v;   // fourth operand of the menu programs with four inputs
   long long nmat;  // matrices in the range handled by this launch (multiple of W)
   int tile_mats;   // matrices per tile: multiple of 32 (hence of W), <= NCW*32
   int stages;      // ring depth >= 2
-  int hint;        // 1: L2 evict_first on loads and stores
+  int hint;        // 0 none; 1: L2 evict_first on loads and stores; 2: loads of the first pin_tiles tiles evict_last
+                   // (kept in L2 from one call to the next: Listing 3 repeats z = x*y on the same fields), rest evict_first
+  long long pin_tiles;
+  ShiftInfo sh;    // SHIFT kernels only
 };
 
-template <int OP> struct NumInputs { static const int value = (OP == OP_MUL || OP == OP_ADD) ? 2 : 3; };
+template <int OP> struct NumInputs { static const int value = menu_prog(OP).nin; };
+
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+
+// straight-line evaluation of menu program OP for one matrix: src[k] points at element 0 of the thread's matrix in
+// operand slot k (element e at src[k][e*W]); unrolled at compile time, so every source index is a constant
+template <int OP, int I, int W, typename C2, int NIN>
+__device__ __forceinline__ void menu_step(const C2 *const (&src)[NIN], C2 (&acc)[9], C2 (&t0)[9]) {
+  constexpr MenuProg P = menu_prog(OP);
+  if constexpr (I < P.nins) {
+    constexpr ExprIns in = P.ins[I];
+    static_assert(in.spill == EX_NONE || in.spill == EX_TEMP0, "menu programs use at most one temporary");
+    if constexpr (in.spill != EX_NONE) {
+#pragma unroll
+      for (int e = 0; e < 9; e++) t0[e] = acc[e];
+    }
+    C2 a[9], b[9];
+#pragma unroll
+    for (int e = 0; e < 9; e++) {
+      if constexpr (in.a == EX_SRC_ACC) a[e] = acc[e];
+      else if constexpr (in.a == EX_TEMP0) a[e] = t0[e];
+      else a[e] = src[in.a][e * W];
+    }
+    if constexpr (in.op != EX_COPY) {
+#pragma unroll
+      for (int e = 0; e < 9; e++) {
+        if constexpr (in.b == EX_SRC_ACC) b[e] = acc[e];
+        else if constexpr (in.b == EX_TEMP0) b[e] = t0[e];
+        else b[e] = src[in.b][e * W];
+      }
+    }
+    if constexpr (in.op == EX_MUL) {
+      mat33_mul(a, b, acc);
+    } else {
+#pragma unroll
+      for (int e = 0; e < 9; e++) {
+        if constexpr (in.op == EX_ADD) {
+          acc[e].x = add_rn(a[e].x, b[e].x);
+          acc[e].y = add_rn(a[e].y, b[e].y);
+        } else if constexpr (in.op == EX_SUB) {
+          acc[e].x = add_rn(a[e].x, -b[e].x);
+          acc[e].y = add_rn(a[e].y, -b[e].y);
+        } else if constexpr (in.op == EX_EMUL) {
+          acc[e].x = mul_rn(a[e].x, b[e].x);
+          acc[e].y = mul_rn(a[e].y, b[e].y);
+        } else {
+          acc[e] = a[e];
+        }
+      }
+    }
+    menu_step<OP, I + 1, W>(src, acc, t0);
+  }
+}
 
 // One thread's matrix: element e of lane l of record q sits at complex index (q*9 + e)*W + l
-// of the slot.  Thread t owns (q = t / W, l = t % W).  Bank check (DESIGN.md section 4.3): with
+// of the slot.  Thread t owns (q = t / W, l = t % W).  Bank check (DESIGN.md section 6.1): with
 // 16-byte (fp64) or 8-byte (fp32) complex numbers every quarter-/half-warp request covers
 // all 32 banks exactly once for every W in {1,2,4,8,16,32}.
-template <typename R, int W, int OP, int NCW>
-__global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_pipe_kernel(const StreamParams p) {
+// Stage layout: NSLOT operand slots of tile_mats*9 complex numbers (+16 bytes of slack for the phase of a shifted
+// slot).  The result is written over slot 0 and leaves by a bulk store; for OP_COPY with SHIFT the shifted operand
+// sits in slot 1 (a thread reads ANOTHER lane's matrix there, so it must not overwrite the slot it reads).
+template <typename R, int W, int OP, int NCW, int SHIFT>
+__global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pipe_kernel(const StreamParams p) {
   typedef typename Cplx<R>::type C2;
   constexpr int NIN = NumInputs<OP>::value;
+  constexpr int NSLOT = (SHIFT && NIN == 1) ? 2 : NIN;
+  constexpr int FIRST = NSLOT - NIN;  // slot of operand 0
   constexpr int CB = (int)sizeof(C2);
   extern __shared__ __align__(128) unsigned char smem[];
 
   const int TM = p.tile_mats;
   const int S = p.stages;
   const uint32_t slot_bytes = (uint32_t)TM * 9u * CB;
-  const uint32_t stage_bytes = NIN * slot_bytes;
+  const uint32_t stage_bytes = NSLOT * slot_bytes + (SHIFT ? 16u : 0u);
   uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)S * stage_bytes);
   uint64_t *empty = full + S;
+  int2 *tinfo = reinterpret_cast<int2 *>(empty + S);  // SHIFT: per stage (oc, record offset inside its P-block) of the tile's first record
 
   const int tid = threadIdx.x;
   const long long ntiles = (p.nmat + TM - 1) / TM;
@@ -193,10 +324,11 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_pipe_kernel(const Strea
   if (tid >= NCW * 32) {
     // ------------------------------------------------ producer: one elected lane issues the TMA bulk loads
     if (tid == NCW * 32) {
-      const unsigned char *src[3] = {(const unsigned char *)p.x, (const unsigned char *)p.y,
-                                     (const unsigned char *)p.u};
-      uint64_t pol = 0;
+      const unsigned char *src[4] = {(const unsigned char *)p.x, (const unsigned char *)p.y,
+                                     (const unsigned char *)p.u, (const unsigned char *)p.v};
+      uint64_t pol = 0, pol_keep = 0;
       if (p.hint) pol = policy_evict_first();
+      if (p.hint == 2) pol_keep = policy_evict_last();
       int s = 0;
       uint32_t ph = 0;
       for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -208,19 +340,59 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_pipe_kernel(const Strea
         const uint32_t b16 = bytes & ~15u;  // bulk copies move multiples of 16 bytes
         unsigned char *st = smem + (size_t)s * stage_bytes;
         const size_t goff = (size_t)m0 * 9u * CB;
+        const uint64_t tpol = (p.hint == 2 && tile < p.pin_tiles) ? pol_keep : pol;
+        constexpr int NPLAIN = SHIFT ? NIN - 1 : NIN;  // operands that are read at the site itself
         if (bytes != b16) {  // fp32 with an odd matrix count: 8 trailing bytes per operand
 #pragma unroll
-          for (int o = 0; o < NIN; o++)
-            *reinterpret_cast<uint64_t *>(st + o * slot_bytes + b16) =
+          for (int o = 0; o < NPLAIN; o++)
+            *reinterpret_cast<uint64_t *>(st + (FIRST + o) * slot_bytes + b16) =
                 *reinterpret_cast<const uint64_t *>(src[o] + goff + b16);
         }
-        mbar_arrive_expect_tx(&full[s], NIN * b16);
+        if (!SHIFT) {
+          mbar_arrive_expect_tx(&full[s], NIN * b16);
+        } else {
+          // the shifted operand: runs of whole records [Ra, Rb) whose sources are contiguous
+          const unsigned char *gy = src[NIN - 1];
+          unsigned char *sy = st + (NSLOT - 1) * slot_bytes + p.sh.phase;
+          const long long R0 = m0 / W, R1 = (m0 + nm) / W;
+          const uint32_t rb = 9u * W * CB;  // bytes per record
+          const long long blk0 = R0 / p.sh.P;
+          tinfo[s] = make_int2((int)(blk0 % p.sh.rd), (int)(R0 - blk0 * p.sh.P));
+          uint32_t total = NPLAIN * b16;
+          for (int pass = 0; pass < 2; pass++) {
+            long long Ra = R0;
+            while (Ra < R1) {
+              const long long blk = Ra / p.sh.P;
+              const int oc = (int)(blk % p.sh.rd);
+              const bool carry = oc + p.sh.dmod >= p.sh.rd;
+              const long long cyc = blk - oc;  // first block of this rd-cycle
+              long long Rb = (carry ? cyc + p.sh.rd : cyc + p.sh.rd - p.sh.dmod) * p.sh.P;
+              if (Rb > R1) Rb = R1;
+              const long long Rs = Ra + (long long)(carry ? p.sh.dmod - p.sh.rd : p.sh.dmod) * p.sh.P;
+              // byte ranges; with 72-byte records (fp32, W = 1) an odd source record starts on an 8-byte boundary: the
+              // first / last 8 bytes of the run then travel by a plain load/store and the aligned middle by TMA
+              size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
+              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
+              const size_t gs16 = (gs + 15) & ~(size_t)15, ge16 = ge & ~(size_t)15;
+              if (pass == 0) {
+                if (gs16 != gs) *reinterpret_cast<uint64_t *>(d) = *reinterpret_cast<const uint64_t *>(gy + gs);
+                if (ge16 != ge && ge16 >= gs16) *reinterpret_cast<uint64_t *>(d + (ge16 - gs)) = *reinterpret_cast<const uint64_t *>(gy + ge16);
+                if (ge16 > gs16) total += (uint32_t)(ge16 - gs16);
+              } else if (ge16 > gs16) {
+                if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
+                else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
+              }
+              Ra = Rb;
+            }
+            if (pass == 0) mbar_arrive_expect_tx(&full[s], total);
+          }
+        }
 #pragma unroll
-        for (int o = 0; o < NIN; o++) {
+        for (int o = 0; o < NPLAIN; o++) {
           if (p.hint)
-            bulk_g2s_hint(st + o * slot_bytes, src[o] + goff, b16, &full[s], pol);
+            bulk_g2s_hint(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s], tpol);
           else
-            bulk_g2s(st + o * slot_bytes, src[o] + goff, b16, &full[s]);
+            bulk_g2s(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s]);
         }
         if (++s == S) {
           s = 0;
@@ -245,40 +417,27 @@ __global__ void __launch_bounds__((NCW + 1) * 32, 3) su3_pipe_kernel(const Strea
     unsigned char *st = smem + (size_t)s * stage_bytes;
     mbar_wait(&full[s], ph);
     if (t < nm) {
-      C2 *sx = reinterpret_cast<C2 *>(st) + base;
-      const C2 *sy = reinterpret_cast<const C2 *>(st + slot_bytes) + base;
-      C2 a[9], b[9], c[9];
+      const C2 *src[NIN];
 #pragma unroll
-      for (int e = 0; e < 9; e++) a[e] = sx[e * W];
-#pragma unroll
-      for (int e = 0; e < 9; e++) b[e] = sy[e * W];
-      if (OP == OP_ADD) {
-#pragma unroll
-        for (int e = 0; e < 9; e++) {
-          c[e].x = add_rn(a[e].x, b[e].x);
-          c[e].y = add_rn(a[e].y, b[e].y);
+      for (int o = 0; o < NIN; o++) src[o] = reinterpret_cast<const C2 *>(st + (FIRST + o) * slot_bytes) + base;
+      if (SHIFT) {
+        int lsrc = t % W;
+        if (W > 1 && p.sh.simd_d > 1) {  // which lane holds my neighbour: a step across the sub-lattice boundary rotates lanes
+          const int2 ti = tinfo[s];
+          const int r = ti.y + t / W;
+          const int oc = (ti.x + r / (int)p.sh.P) % p.sh.rd;
+          const int carry = oc + p.sh.dmod >= p.sh.rd ? 1 : 0;
+          const int ic = (lsrc / p.sh.lstride) % p.sh.simd_d;
+          const int icn = (ic + p.sh.qrot + carry) % p.sh.simd_d;
+          lsrc += (icn - ic) * p.sh.lstride;
         }
-      } else {
-        mat33_mul(a, b, c);
+        src[NIN - 1] = reinterpret_cast<const C2 *>(st + (NSLOT - 1) * slot_bytes + p.sh.phase) + (t / W) * 9 * W + lsrc;
       }
-      if (OP == OP_MUL3) {
-        const C2 *su = reinterpret_cast<const C2 *>(st + 2 * slot_bytes) + base;
+      C2 acc[9], t0[9];
+      menu_step<OP, 0, W>(src, acc, t0);
+      C2 *so = reinterpret_cast<C2 *>(st) + base;  // every read of this thread's own slots is done
 #pragma unroll
-        for (int e = 0; e < 9; e++) b[e] = su[e * W];
-        mat33_mul(c, b, a);
-#pragma unroll
-        for (int e = 0; e < 9; e++) c[e] = a[e];
-      } else if (OP == OP_MUL_ADD) {
-        const C2 *su = reinterpret_cast<const C2 *>(st + 2 * slot_bytes) + base;
-#pragma unroll
-        for (int e = 0; e < 9; e++) {
-          C2 v = su[e * W];
-          c[e].x = add_rn(c[e].x, v.x);
-          c[e].y = add_rn(c[e].y, v.y);
-        }
-      }
-#pragma unroll
-      for (int e = 0; e < 9; e++) sx[e * W] = c[e];
+      for (int e = 0; e < 9; e++) so[e * W] = acc[e];
     }
     fence_proxy_async();  // generic-proxy smem writes -> visible to the bulk (async-proxy) store
     named_bar_sync(1, NCW * 32);
@@ -362,11 +521,6 @@ __global__ void __launch_bounds__(256) su3_direct_kernel(const StreamParams p) {
 // accumulator.  The program is uniform over the grid, so the interpreter's branches never diverge.
 // Same pipeline as su3_pipe_kernel (TMA bulk in, TMA bulk out), same mat33_mul, hence bit-identical
 // to su3_mul / su3_mul3 / su3_mul_add on their three programs.
-enum { EX_MUL = 0, EX_ADD = 1, EX_SUB = 2, EX_COPY = 3, EX_EMUL = 4,  // EMUL: element-wise product of the reals (real scalar fields)
-       EX_SRC_ACC = 255, EX_NONE = 255, EX_TEMP0 = 8 };
-struct ExprIns {
-  unsigned char op, a, b, spill;  // sources: 0..7 operand slot, 8..15 temporary, 255 accumulator
-};
 struct ExprParams {
   void *z;
   const void *ops[8];
@@ -1049,6 +1203,8 @@ struct ConvertParams {
   long long sstride[4]; // scalar-site stride of dimension d: 1, L0, L0*L1, L0*L1*L2
   long long lane_off[32]; // (site offset of lane l) * nl * NC, in complex numbers (NC = 9 matrix, 3 colour vector)
   int to_vector;        // 1: dst is the vector layout; 0: dst is the scalar layout
+  long long run_recs;   // su3_convert_tma_kernel: consecutive vector records whose scalar-side images are contiguous
+  int pitch;            // su3_convert_tma_kernel: shared-memory row pitch of one lane's run, in complex numbers
 };
 
 template <typename C2, int W, int TR, int NC>
@@ -1197,6 +1353,112 @@ __global__ void __launch_bounds__(256) su3_convert_staged_kernel(const ConvertPa
       const int k = idx - l * m, rl = k / NC, e = k - rl * NC;
       dst[sbase[rl] + p.lane_off[l] + e] = tile[(rl * NC + e) * TS + l];
     }
+  }
+}
+
+
+// TMA variant (default for every aligned geometry): NO per-thread global access at all.  For each lane l the
+// scalar-side image of a tile of TR consecutive vector records is a handful of CONTIGUOUS runs (one, unless the tile
+// crosses a row of the sub-lattice: runs break every p.run_recs records), so lane l's data moves between global
+// memory and row l of a shared-memory tile with 1-D bulk copies issued by thread l; the vector side of the tile is
+// one contiguous range and moves with a single bulk copy.  In between, the block transposes rows <-> element
+// vectors through registers, in place ([lane][k] with a padded, conflict-free pitch <-> dense [k][lane]).
+// Bulk copies need 16-byte alignment: with 8-byte complex numbers (fp32) the host only selects this kernel when every
+// run starts and ends on an even complex index (true for every even lattice); otherwise the staged kernel above runs.
+template <typename C2, int W, int NC, int N, int NT>
+__global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams p) {
+  constexpr int CB = (int)sizeof(C2);
+  constexpr int TR = N / (NC * W);      // records per tile
+  constexpr int PER = (N + NT - 1) / NT;
+  static_assert(TR * NC * W == N && TR >= 1, "tile must hold whole records");
+  extern __shared__ __align__(128) unsigned char smem[];
+  C2 *tile = reinterpret_cast<C2 *>(smem);
+  const int pitch = p.pitch;
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + (size_t)CB * (W * pitch > N ? W * pitch : N));
+  const int tid = threadIdx.x;
+  const long long rec0 = (long long)blockIdx.x * TR;
+  const long long left = p.nrec - rec0;
+  const int nr = left < TR ? (int)left : TR;
+  const int n = nr * NC * W;
+  const unsigned char *src = reinterpret_cast<const unsigned char *>(p.src);
+  unsigned char *dst = reinterpret_cast<unsigned char *>(p.dst);
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    fence_mbar_init();
+    fence_proxy_async();
+  }
+  __syncthreads();
+  // scalar-side complex index of (vector record rec, lane 0, element 0): the virtual-node map S3 for the outer site
+  auto sbase = [&](long long rec) {
+    long long o = rec / p.nl;
+    const int mu = (int)(rec - o * p.nl);
+    long long site = 0;
+#pragma unroll
+    for (int d = 0; d < 4; d++) {
+      const long long q = o / p.r[d];
+      site += (o - q * p.r[d]) * p.sstride[d];
+      o = q;
+    }
+    return (site * p.nl + mu) * NC;
+  };
+  // lane l's runs of the tile: [a, b) in records, cut at multiples of run_recs
+  auto for_runs = [&](auto &&fn) {
+    long long a = rec0;
+    const long long end = rec0 + nr;
+    while (a < end) {
+      long long b = (a / p.run_recs + 1) * p.run_recs;
+      if (b > end) b = end;
+      fn(a, b);
+      a = b;
+    }
+  };
+  if (p.to_vector) {
+    if (tid < 32) {
+      if (tid == 0) mbar_arrive_expect_tx(bar, (uint32_t)n * CB);
+      __syncwarp();
+      if (tid < W) {
+        const long long loff = p.lane_off[tid];
+        for_runs([&](long long a, long long b) {
+          bulk_g2s(tile + (size_t)tid * pitch + (a - rec0) * NC, src + (size_t)(sbase(a) + loff) * CB,
+                   (uint32_t)((b - a) * NC) * CB, bar);
+        });
+      }
+    }
+  } else if (tid == 0) {
+    mbar_arrive_expect_tx(bar, (uint32_t)n * CB);
+    bulk_g2s(tile, src + (size_t)rec0 * NC * W * CB, (uint32_t)n * CB, bar);
+  }
+  mbar_wait(bar, 0);
+  C2 v[PER];
+#pragma unroll
+  for (int i = 0; i < PER; i++) {
+    const int idx = i * NT + tid;  // dense (vector-side) index: lane fastest
+    if (idx < n) v[i] = p.to_vector ? tile[(idx % W) * pitch + idx / W] : tile[idx];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < PER; i++) {
+    const int idx = i * NT + tid;
+    if (idx < n) {
+      if (p.to_vector) tile[idx] = v[i];
+      else tile[(idx % W) * pitch + idx / W] = v[i];
+    }
+  }
+  fence_proxy_async();
+  __syncthreads();
+  if (p.to_vector) {
+    if (tid == 0) {
+      bulk_s2g(dst + (size_t)rec0 * NC * W * CB, tile, (uint32_t)n * CB);
+      bulk_commit();
+      bulk_wait_all<0>();
+    }
+  } else if (tid < W) {
+    const long long loff = p.lane_off[tid];
+    for_runs([&](long long a, long long b) {
+      bulk_s2g(dst + (size_t)(sbase(a) + loff) * CB, tile + (size_t)tid * pitch + (a - rec0) * NC, (uint32_t)((b - a) * NC) * CB);
+    });
+    bulk_commit();
+    bulk_wait_all<0>();
   }
 }
 

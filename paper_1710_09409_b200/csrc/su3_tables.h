@@ -8,16 +8,40 @@ namespace su3tab {
 typedef void (*stream_kernel_t)(const su3::StreamParams);
 constexpr int NCW = 4;  // consumer warps per CTA of the pipeline kernel (tile <= 128 matrices)
 
-template <typename R, int OP> stream_kernel_t pipe_for_w(int W) {
+template <typename R, int OP, int SHIFT = 0> stream_kernel_t pipe_for_w(int W) {
   switch (W) {
-    case 1: return su3::su3_pipe_kernel<R, 1, OP, NCW>;
-    case 2: return su3::su3_pipe_kernel<R, 2, OP, NCW>;
-    case 4: return su3::su3_pipe_kernel<R, 4, OP, NCW>;
-    case 8: return su3::su3_pipe_kernel<R, 8, OP, NCW>;
-    case 16: return su3::su3_pipe_kernel<R, 16, OP, NCW>;
-    case 32: return su3::su3_pipe_kernel<R, 32, OP, NCW>;
+    case 1: return su3::su3_pipe_kernel<R, 1, OP, NCW, SHIFT>;
+    case 2: return su3::su3_pipe_kernel<R, 2, OP, NCW, SHIFT>;
+    case 4: return su3::su3_pipe_kernel<R, 4, OP, NCW, SHIFT>;
+    case 8: return su3::su3_pipe_kernel<R, 8, OP, NCW, SHIFT>;
+    case 16: return su3::su3_pipe_kernel<R, 16, OP, NCW, SHIFT>;
+    case 32: return su3::su3_pipe_kernel<R, 32, OP, NCW, SHIFT>;
   }
   return nullptr;
+}
+// the menu programs beyond su3_mul / mul3 / mul_add / add (su3_kernels.cuh: menu_prog): element-wise rows are layout-
+// agnostic and exist for W = 1 only
+template <typename R> stream_kernel_t menu_any(int op, int W) {
+  switch (op) {
+    case su3::OP_SUM_PROD: return pipe_for_w<R, su3::OP_SUM_PROD>(W);
+    case su3::OP_MUL_MUL_ADD: return pipe_for_w<R, su3::OP_MUL_MUL_ADD>(W);
+    case su3::OP_MUL_MUL_SUB: return pipe_for_w<R, su3::OP_MUL_MUL_SUB>(W);
+    case su3::OP_MUL_SUB: return pipe_for_w<R, su3::OP_MUL_SUB>(W);
+    case su3::OP_ADD3: return su3::su3_pipe_kernel<R, 1, su3::OP_ADD3, NCW, 0>;
+    case su3::OP_ADD4: return su3::su3_pipe_kernel<R, 1, su3::OP_ADD4, NCW, 0>;
+    case su3::OP_SUB: return su3::su3_pipe_kernel<R, 1, su3::OP_SUB, NCW, 0>;
+    case su3::OP_EMUL: return su3::su3_pipe_kernel<R, 1, su3::OP_EMUL, NCW, 0>;
+    case su3::OP_SUM_EPROD: return su3::su3_pipe_kernel<R, 1, su3::OP_SUM_EPROD, NCW, 0>;
+  }
+  return nullptr;
+}
+inline bool menu_elementwise(int op) {
+  return op == su3::OP_ADD || op == su3::OP_ADD3 || op == su3::OP_ADD4 || op == su3::OP_SUB || op == su3::OP_EMUL ||
+         op == su3::OP_SUM_EPROD;
+}
+// the pipeline with a shifted last operand: z = x . y(+disp) (OP_MUL) and z = y(+disp) (OP_COPY, Cshift)
+template <typename R> stream_kernel_t shift_pipe_any(int op, int W) {
+  return op == su3::OP_MUL ? pipe_for_w<R, su3::OP_MUL, 1>(W) : pipe_for_w<R, su3::OP_COPY, 1>(W);
 }
 template <typename R, int OP> stream_kernel_t direct_for_w(int W) {
   switch (W) {
@@ -122,11 +146,17 @@ template <typename R> stream_kernel_t stream_any(int family, int op, int W) {
 }
 stream_kernel_t stream_f64(int family, int op, int W);
 stream_kernel_t stream_f32(int family, int op, int W);
+stream_kernel_t menu_f64(int op, int W);
+stream_kernel_t menu_f32(int op, int W);
+stream_kernel_t shift_pipe_kernel(int prec, int op, int W);
 stream_kernel_t matvec_kernel(int prec, int W);
 expr_kernel_t expr_kernel(int prec, int W);
 shift_kernel_t shift_kernel(int prec, int op, int W, bool idx32);        // register version (SH_COPY / SH_MUL)
 shift_kernel_t cshift_async_kernel(int prec, int W, bool idx32);
 // layout conversion: launches the kernel for (prec, nc, W); returns false if W is not supported
 bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertParams &p, cudaStream_t s, const char **err);
+// the TMA variant: complex numbers per tile for (prec, big), and the launch (p.pitch and p.run_recs must be set)
+int convert_tma_tile(int prec, bool big);
+bool launch_convert_tma(int prec, int nc, int W, bool big, const su3::ConvertParams &p, cudaStream_t s, const char **err);
 
 }  // namespace su3tab

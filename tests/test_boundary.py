@@ -107,7 +107,7 @@ def test_wrap_errors_without_touching_memory():
 
 def test_tune_validation_roundtrip():
     su3.su3_tune_set(tile_mats=64, stages=3, ctas_per_sm=2, l2_hint=1, path=1)
-    assert su3.su3_tune_get() == dict(tile_mats=64, stages=3, ctas_per_sm=2, l2_hint=1, path=1)
+    assert su3.su3_tune_get() == dict(tile_mats=64, stages=3, ctas_per_sm=2, l2_hint=1, path=1, l2_pin_mb=0)
     with pytest.raises(su3.Su3Error):
         su3.su3_tune_set(tile_mats=100)
     with pytest.raises(su3.Su3Error):
@@ -314,3 +314,29 @@ def test_eval_host_rejects_absurd_chunk_counts_before_any_cuda_work():
         assert su3.lib.su3_eval_host(0, None, None, None, None, h, h, h, None, 1 << 20, None) in (su3.SU3_ERR_INVALID, su3.SU3_ERR_CUDA)
     assert su3.lib.su3_host_release() == su3.SU3_OK
     su3.lib.su3_field_free(h)
+
+
+def test_ahead_of_time_menu_rows_and_matching():
+    """host-only: every row of the ahead-of-time menu is reached by its own postfix program, by any renaming of the
+    operands and by either order of the sources of '+'; everything else goes to the interpreter"""
+    rows = {}
+    for prog, n in [("01*", 2), ("01*2*", 3), ("01*2+", 3), ("01+", 2), ("01+01*+", 2), ("01*23*+", 4), ("01*23*-", 4),
+                    ("01*2-", 3), ("01+2+", 3), ("01+2+3+", 4), ("01-", 2)]:
+        plan = su3.su3_expr_plan(prog, n)
+        assert plan[0] == "menu" and plan[2] == prog and plan[3] == list(range(n)), (prog, plan)
+        rows[prog] = plan[1]
+    assert sorted(rows.values()) == list(range(11))          # eleven distinct rows for matrix fields
+    # renamed operands: slot k of the row holds the operand that plays its part
+    assert su3.su3_expr_plan("10*", 2) == ("menu", rows["01*"], "01*", [1, 0])
+    assert su3.su3_expr_plan("20*1+", 3) == ("menu", rows["01*2+"], "01*2+", [2, 0, 1])
+    assert su3.su3_expr_plan("201*+", 3) == ("menu", rows["01*2+"], "01*2+", [0, 1, 2])       # v + x*y = x*y + v
+    assert su3.su3_expr_plan("10+01*+", 2)[:2] == ("menu", rows["01+01*+"])
+    assert su3.su3_expr_plan("32*10*+", 4) == ("menu", rows["01*23*+"], "01*23*+", [3, 2, 1, 0])
+    # not on the menu: repeated fields, other shapes, non-commutative swaps
+    for prog, n in [("00*", 1), ("012**", 3), ("201*-", 3), ("01*21*-", 3), ("01*23*45*++", 6), ("0", 1), ("01-2-", 3)]:
+        assert su3.su3_expr_plan(prog, n) == "interpreter", prog
+    # real scalar fields: '*' is element-wise; Listing 2's two programs are on the menu
+    assert su3.su3_expr_plan("01+", 2, real_fields=True)[:2] == ("menu", rows["01+"])
+    p1, p2 = su3.su3_expr_plan("01*", 2, real_fields=True), su3.su3_expr_plan("01+01*+", 2, real_fields=True)
+    assert p1[0] == "menu" and p2[0] == "menu" and p1[1] not in rows.values() and p2[1] not in rows.values()
+    assert su3.su3_expr_plan("01*2*", 3, real_fields=True) == "interpreter"

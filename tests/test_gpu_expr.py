@@ -165,3 +165,56 @@ def test_lattice_front_end_assign():
     v3.assign(v1 + v2 + v1 * v2)
     torch.cuda.synchronize()
     assert bool((v3.field.tensor.view(torch.float32) == 5.0).all())
+
+
+MENU = [("01+01*+", 2), ("10+01*+", 2), ("01*23*+", 4), ("32*10*+", 4), ("01*23*-", 4), ("01*2-", 3), ("01+2+", 3),
+        ("01+2+3+", 4), ("01-", 2), ("10-", 2), ("201*+", 3)]
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", [((4, 6, 4, 8), 1, SC, 1), ((3, 3, 3, 3), 1, SC, 1), ((6, 2, 10, 2), 4, VE, 8),
+                                           ((8, 8, 8, 8), 1, VE, 4), ((2, 2, 2, 2), 4, VE, 16), ((4, 4, 4, 8), 1, VE, 32),
+                                           ((16, 16, 8, 10), 1, VE, 2)])
+def test_menu_programs_against_oracle_and_interpreter(prec, L, nl, layout, W):
+    """the ahead-of-time rows of the pipeline kernel: within tolerance of the oracle, and bit-identical to what the
+    interpreter gives for the same program (same order of operations, same FMA chains)"""
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    g = geom_of(desc)
+    hosts = [host_field(desc, 47, f, kind="su3" if f % 2 == 0 else "gauss") for f in range(4)]
+    fs, z = [upload(desc, h) for h in hosts], su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    for prog, n in MENU:
+        assert su3.su3_expr_plan(prog, n)[0] == "menu", prog
+        su3.su3_tune_set()
+        z.tensor.fill_(0xFF)
+        su3.su3_expr(z, prog, fs[:n])
+        got = download(z)
+        ref = oracle.expr(g, prog, *hosts[:n])
+        scale = max(np.abs(ref).max(), 1.0)
+        assert np.isfinite(got).all() and np.abs(got - ref).max() / scale <= 4 * TOL[prec], prog
+        if "-" not in prog:                      # no cancellation: the per-matrix norm of S15 applies as well
+            assert rel_err(got, ref, Wn)[0] <= 4 * TOL[prec], prog
+        su3.su3_tune_set(path=3)                 # the interpreter
+        z.tensor.fill_(0xFF)
+        su3.su3_expr(z, prog, fs[:n])
+        assert np.array_equal(download(z), got), prog
+        for tile, stages, ctas in [(32, 2, 1), (128, 2, 1)]:
+            su3.su3_tune_set(tile_mats=tile, stages=stages, ctas_per_sm=ctas)
+            su3.su3_expr(z, prog, fs[:n])
+            assert np.array_equal(download(z), got), (prog, tile)
+    # z may alias any operand of a menu program
+    su3.su3_tune_set()
+    su3.su3_expr(z, "01*23*+", fs)
+    want = download(z)
+    su3.su3_expr(fs[3], "01*23*+", fs)
+    assert np.array_equal(download(fs[3]), want)
+
+
+def test_menu_programs_integer_inputs_bit_exact_against_oracle():
+    for prec, layout, W in ((F64, SC, 1), (F32, VE, 8), (F64, VE, 4)):
+        desc = su3.make_desc((4, 4, 4, 8), prec=prec, layout=layout, W=W)
+        k = np.arange(1, 4).reshape(-1, 1, 1)
+        hosts = [const_field(desc, m) for m in (IC["A"] * k, IC["B"], IC["C"], IC["A"] - IC["C"])]
+        for prog, n in MENU:
+            z = run_expr(desc, prog, hosts[:n])
+            assert np.array_equal(z.astype(np.float64), oracle.expr(geom_of(desc), prog, *hosts[:n])), prog

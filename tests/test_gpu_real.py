@@ -75,3 +75,33 @@ def test_real_kind_is_checked():
             call()
         assert e.value.status == su3.SU3_ERR_MISMATCH
     assert su3.su3_launch_count() == n0
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_real_menu_programs_equal_the_interpreter(prec):
+    """Listing 2's programs on real fields run on ahead-of-time rows of the pipeline kernel: same bits as the interpreter"""
+    desc = su3.make_desc((16, 12, 10, 9), n_lorentz=4, prec=prec)     # 69120 reals = 3840 records of 18
+    n = 16 * 12 * 10 * 9 * 4
+    rng = np.random.default_rng(9)
+    hosts = [rng.standard_normal(n).astype(NP[prec]) for _ in range(4)]
+    fs = []
+    for h in hosts:
+        f = su3.alloc_real(desc)
+        f.tensor.copy_(torch.from_numpy(h.view(np.uint8)))
+        fs.append(f)
+    z = su3.alloc_real(desc)
+    for prog in ["01+", "01*", "10*", "01-", "01+01*+", "01+2+", "01+2+3+"]:
+        k = max(int(c) for c in prog if c.isdigit()) + 1
+        assert su3.su3_expr_plan(prog, k, real_fields=True)[0] == "menu", prog
+        su3.su3_tune_set()
+        z.tensor.fill_(0xFF)
+        su3.su3_expr(z, prog, fs[:k])
+        got = down(z)
+        ref = oracle.expr_real(prog, *hosts[:k])
+        tol = 1e-14 if prec == F64 else 1e-5
+        assert np.abs(got.astype(np.float64) - ref).max() <= tol * max(1.0, np.abs(ref).max()), prog
+        su3.su3_tune_set(path=3)
+        z.tensor.fill_(0xFF)
+        su3.su3_expr(z, prog, fs[:k])
+        assert np.array_equal(down(z), got), prog
+    su3.su3_tune_set()
