@@ -91,7 +91,7 @@ typedef struct su3_field su3_field; /* opaque: validated descriptor + device poi
  *             whose knobs are stages = ring depth per warp (2..) and ctas_per_sm; its tile is 32 matrices
  *   su3_cshift / su3_mul_shift: default = the pipeline with a shifted operand (knobs as above); path = 2 the register
  *             kernels, path = 3 the cp.async-gather Cshift; for those ctas_per_sm = blocks per SM of the grid
- *   su3_convert: default = TMA bulk copies on both sides (tile_mats = 128: 36 KB tiles instead of 18 KB);
+ *   su3_convert: default = TMA bulk copies on both sides;
  *                path = 3 the per-thread kernel staged through shared memory, path = 2 the unstaged kernel */
 typedef struct {
   int32_t tile_mats;    /* matrices per pipeline tile: 32, 64 or 128 (su3_copy: x matrix bytes) */

@@ -249,7 +249,16 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
     // L2 policy (l2_hint): 0/1 none (evict_first measured neutral at every HBM-bound size), 2 evict_first
     // everywhere, 3 keep the first l2_pin_mb MB of every operand in L2 (evict_last) and stream the rest (evict_first)
     p.hint = tn.l2_hint == 2 ? 1 : (tn.l2_hint == 3 ? 2 : 0);
-    if (p.hint == 2) p.pin_tiles = (int64_t)((size_t)tn.l2_pin_mb * 1000000 / ((size_t)tm * 9 * cb));
+    size_t pin_bytes = (size_t)tn.l2_pin_mb * 1000000;   // per operand
+    if (tn.l2_hint == 0 && footprint_bytes > (size_t)di.l2 * 6 / 10 && footprint_bytes <= (size_t)di.l2 * 2) {
+      // auto, footprint between 0.6 and 2 x L2 ("straddling"): a plain LRU keeps NOTHING of a cyclic sweep that is a
+      // little larger than the cache; keeping ~36 % of L2 worth of operand prefixes resident from one call to the next
+      // (Listing 3 repeats z = x*y on the same fields) and streaming the rest measured +32 % at 24^4 fp64, +7 % at
+      // 32^4 fp32; beyond 2 x L2 the same policy costs 2-4 %, so it is not applied there
+      p.hint = 2;
+      pin_bytes = (size_t)di.l2 * 36 / 100 / nin;
+    }
+    if (p.hint == 2) p.pin_tiles = (int64_t)(pin_bytes / ((size_t)tm * 9 * cb));
     const int64_t ntiles = (nmat + tm - 1) / tm;
     const unsigned grid = (unsigned)(ntiles < max_grid ? ntiles : max_grid);
     k<<<grid, (NCW + 1) * 32, smem, stream>>>(p);
@@ -419,7 +428,46 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   // scalar layout) all runs of a launch must agree in (source - destination) mod 16, true unless r[dim]*P is odd.
   const int64_t P = p.ostride * d.n_lorentz;
   const bool odd72 = d.prec == SU3_F32 && d.W == 1 && ((int64_t)p.rd * P) % 2 != 0;
-  if ((tn.path == 0 || tn.path == 1) && !odd72 && P < 0x7fffffffLL) {
+  // Cshift: the pure TMA copy (su3_cshift_bulk_kernel: the ceiling kernel with its loads split into runs).  Bulk copies
+  // need 16-byte alignment; with 72-byte records (fp32, scalar layout) that means every run boundary and every source
+  // record is even: P even and an even record count.
+  const int64_t nrec_all = z->nmat / d.W;
+  const bool bulk72_ok = !(d.prec == SU3_F32 && d.W == 1) || (P % 2 == 0 && nrec_all % 2 == 0);
+  if (op == su3::SH_COPY && (tn.path == 0 || tn.path == 1) && bulk72_ok && z->nmat < 0x7fffffffLL) {
+    stream_kernel_t kb = su3tab::cshift_bulk_kernel(d.prec, d.W);
+    if (!kb) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
+    const int cbb = 2 * d.prec, rbytes = 9 * d.W * cbb;
+    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 3;           // as su3_copy
+    int tm = tn.tile_mats > 0 ? tn.tile_mats : 18432 / (9 * cbb);      // 18 KB tiles
+    if (tm < d.W) tm = d.W;
+    tm = tm / d.W * d.W;
+    while (tm > 2 * d.W && (z->nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas && (tm / 2) % d.W == 0 && ((tm / 2 / d.W) * rbytes) % 16 == 0) tm >>= 1;
+    if (((tm / d.W) * rbytes) % 16) tm += d.W;                           // fp32 scalar: an even number of 72-byte records per tile
+    int stages = tn.stages > 0 ? tn.stages : 2;
+    const size_t tile_bytes = (size_t)(tm / d.W) * rbytes;
+    const size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+    while (stages > 2 && (size_t)stages * tile_bytes + 256 > budget) stages--;
+    const size_t smem_b = (size_t)stages * tile_bytes + stages * sizeof(uint64_t);
+    if (smem_b > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "su3_cshift pipeline needs %zu B of shared memory", smem_b);
+    cudaError_t eb = allow_max_smem((const void *)kb, di.smem_optin);
+    if (eb != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", eb);
+    su3::StreamParams sp;
+    memset(&sp, 0, sizeof sp);
+    sp.z = z->ptr; sp.x = y->ptr; sp.nmat = z->nmat; sp.tile_mats = tm; sp.stages = stages;
+    sp.sh.P = P; sp.sh.rd = p.rd; sp.sh.dmod = p.disp % p.rd; sp.sh.qrot = p.disp / p.rd; sp.sh.simd_d = p.simd_d; sp.sh.lstride = p.lstride;
+    const int64_t ntiles_b = (z->nmat + tm - 1) / tm, cap_b = (int64_t)di.sms * ctas;
+    kb<<<(unsigned)(ntiles_b < cap_b ? ntiles_b : cap_b), 32, smem_b, (cudaStream_t)stream>>>(sp);
+    eb = cudaGetLastError();
+    if (eb != cudaSuccess) return cuda_fail("cshift kernel launch", eb);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return SU3_OK;
+  }
+  // The shifted product: the TMA pipeline with a shifted operand for fp64 whenever a tile has at most ~2 runs (a cycle of
+  // rd*P records is at least a tile long); measured at 48^4: 0.94-1.00 x copy against 0.89-0.97 for the register kernel.
+  // fp32 stays on the register kernel (0.97-0.99 x copy against 0.90-0.98).  path = 1 forces the pipeline.
+  const int64_t tile_recs = (9216 / (9 * 2 * d.prec)) / d.W;
+  const bool pipe_pays = d.prec == SU3_F64 && (int64_t)p.rd * P >= tile_recs;
+  if (op == su3::SH_MUL && (tn.path == 1 || (tn.path == 0 && pipe_pays)) && !odd72 && z->nmat < 0x7fffffffLL) {  // record indices fit 31 bits (P <= records)
     su3::ShiftInfo sh;
     sh.P = P; sh.rd = p.rd; sh.dmod = p.disp % p.rd; sh.qrot = p.disp / p.rd; sh.simd_d = p.simd_d; sh.lstride = p.lstride;
     sh.phase = (d.prec == SU3_F32 && d.W == 1 && ((int64_t)sh.dmod * P) % 2) ? 8 : 0;
@@ -752,15 +800,17 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", W_eff);
   // Every warp is a self-contained pipeline with a private ring of `sw` stages of 32 matrices per operand.  Long programs are latency-bound per tile, so the launch maximises resident warps per SM
   // under the shared-memory budget (ring depth 2, 3 if there is room for >= 8 warps anyway), at most 16.
-  const int mps = 32;
+  // matrices per stage and operand: 32 (one per lane); fp32 programs with <= 3 operands take 64 (4608-byte slots as in
+  // fp64: measured +4..13 % there, -20 % with 4 operands, where shared memory then holds too few warps)
+  const int mps = (z->d.prec == SU3_F32 && n_operands <= 3 && tn.tile_mats != 32) ? 64 : 32;
   const size_t slot = (size_t)mps * 9 * cb;
   const size_t stage_bytes = (size_t)n_operands * slot;
   const size_t sm_bytes = (size_t)di.smem_optin - 4096;  // what one SM can give to its resident CTAs, minus slack
   int sw = tn.stages > 0 ? tn.stages : 3;
-  int warps = (int)(sm_bytes / (sw * stage_bytes + pr.ntemp * slot + 64));
+  int warps = (int)(sm_bytes / (sw * stage_bytes + (pr.ntemp + 1) * slot + 64));   // + 1: the warp's result slot
   if (tn.stages == 0 && warps < 8) {
     sw = 2;
-    warps = (int)(sm_bytes / (sw * stage_bytes + pr.ntemp * slot + 64));
+    warps = (int)(sm_bytes / (sw * stage_bytes + (pr.ntemp + 1) * slot + 64));
   }
   const int reg_cap = z->d.prec == SU3_F64 ? 12 : 16;  // warps/SM the kernel's registers allow in whole CTAs of NCW warps
   if (warps > reg_cap) warps = reg_cap;
@@ -771,7 +821,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   if (ncw > NCW) ncw = NCW;
   if (ncw < 1) { ncw = 1; ctas = warps; }
   const int stages = sw;
-  const size_t smem = (size_t)ncw * sw * stage_bytes + (size_t)ncw * pr.ntemp * slot + (size_t)ncw * sw * sizeof(uint64_t) + 16;
+  const size_t smem = (size_t)ncw * sw * stage_bytes + (size_t)ncw * (pr.ntemp + 1) * slot + (size_t)ncw * sw * sizeof(uint64_t) + 16;
   const int tm = mps;
   cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
   if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
@@ -976,20 +1026,19 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   // Default: the TMA kernel (bulk copies on both sides, transposition in shared memory).  With 8-byte complex numbers its
   // bulk copies are 16-byte aligned only if every run starts and ends on an even complex index; odd geometries (and
   // path = 2 / 3, kept for measurements) take the per-thread kernels: 3 = staged through shared memory, 2 = unstaged.
-  bool tma = tn_c.path == 0 || tn_c.path == 1;
+  bool tma = (tn_c.path == 0 || tn_c.path == 1) && dst->volume < 0x7fffffffLL;  // the kernel decodes sites in 32 bits
   if (tma && v.prec == SU3_F32) {
     tma = (p.run_recs * nc) % 2 == 0;
     for (int l = 0; l < v.W; l++) tma = tma && p.lane_off[l] % 2 == 0;
   }
   if (tma) {
-    const bool big = tn_c.tile_mats == 128;
-    const int K = su3tab::convert_tma_tile(v.prec, big) / v.W;             // complex numbers per lane row
+    const int K = su3tab::convert_tma_tile(v.prec) / v.W;                  // complex numbers per lane row
     const int phase = v.prec == SU3_F32 ? 16 : 8;                          // complex numbers per 128-byte wavefront
     const int want = v.W < phase ? phase / v.W : 1;
     int pad = ((want - K) % phase + phase) % phase;
     if (v.prec == SU3_F32 && ((K + pad) & 1)) pad += 1;                    // rows must stay 16-byte aligned
     p.pitch = K + pad;
-    if (!su3tab::launch_convert_tma(v.prec, nc, v.W, big, p, (cudaStream_t)stream, &err))
+    if (!su3tab::launch_convert_tma(v.prec, nc, v.W, p, (cudaStream_t)stream, &err))
       return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");
   } else if (!su3tab::launch_convert(v.prec, nc, v.W, tn_c.path != 2 && (v.prec == SU3_F32 || (v.W >= 8 && !p.to_vector)), p, (cudaStream_t)stream, &err))
     return fail(SU3_ERR_SIZE, "su3_convert: %s", err ? err : "unsupported W");

@@ -4,7 +4,7 @@ namespace su3tab {
 expr_kernel_t expr_kernel(int prec, int W) { return prec == 8 ? expr_for_w<double>(W) : expr_for_w<float>(W); }
 stream_kernel_t matvec_kernel(int prec, int W) { return prec == 8 ? matvec_for_w<double>(W) : matvec_for_w<float>(W); }
 
-// TMA convert: N complex numbers per tile (18 KB, or 36 KB with big = true), 128 threads
+// TMA convert: N complex numbers per tile (18 KB), 128 threads, 8 blocks per SM by registers
 template <typename C2, int NC, int N> bool convert_tma_w(int W, const su3::ConvertParams &p, cudaStream_t s, const char **err) {
   constexpr int NT = 128;
   const long long tr = N / (NC * W);
@@ -20,14 +20,10 @@ template <typename C2, int NC, int N> bool convert_tma_w(int W, const su3::Conve
   *err = "unsupported W";
   return false;
 }
-int convert_tma_tile(int prec, bool big) { return (prec == 8 ? 1152 : 2304) * (big ? 2 : 1); }
-bool launch_convert_tma(int prec, int nc, int W, bool big, const su3::ConvertParams &p, cudaStream_t s, const char **err) {
-  if (prec == 8) {
-    if (nc == 9) return big ? convert_tma_w<double2, 9, 2304>(W, p, s, err) : convert_tma_w<double2, 9, 1152>(W, p, s, err);
-    return big ? convert_tma_w<double2, 3, 2304>(W, p, s, err) : convert_tma_w<double2, 3, 1152>(W, p, s, err);
-  }
-  if (nc == 9) return big ? convert_tma_w<float2, 9, 4608>(W, p, s, err) : convert_tma_w<float2, 9, 2304>(W, p, s, err);
-  return big ? convert_tma_w<float2, 3, 4608>(W, p, s, err) : convert_tma_w<float2, 3, 2304>(W, p, s, err);
+int convert_tma_tile(int prec) { return prec == 8 ? 1152 : 2304; }
+bool launch_convert_tma(int prec, int nc, int W, const su3::ConvertParams &p, cudaStream_t s, const char **err) {
+  if (prec == 8) return nc == 9 ? convert_tma_w<double2, 9, 1152>(W, p, s, err) : convert_tma_w<double2, 3, 1152>(W, p, s, err);
+  return nc == 9 ? convert_tma_w<float2, 9, 2304>(W, p, s, err) : convert_tma_w<float2, 3, 2304>(W, p, s, err);
 }
 
 bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertParams &p, cudaStream_t s, const char **err) {

@@ -140,6 +140,13 @@ template <int N> __device__ __forceinline__ void bulk_wait_read() {
 template <int N> __device__ __forceinline__ void bulk_wait_all() {
   asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
 }
+// 8-byte asynchronous copy global -> shared (LDGSTS) and its completion as an arrival on an mbarrier
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src_gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive_noinc(uint64_t *bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -298,6 +305,9 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
   constexpr int NSLOT = (SHIFT && NIN == 1) ? 2 : NIN;
   constexpr int FIRST = NSLOT - NIN;  // slot of operand 0
   constexpr int CB = (int)sizeof(C2);
+  // 72-byte records (fp32, scalar layout): a run of the shifted operand may start / end on an 8-byte boundary; those 8
+  // bytes travel by cp.async (LDGSTS), whose completion is the SECOND arrival every phase of full[s] then waits for
+  constexpr bool FIX8 = SHIFT && CB == 8 && W == 1;
   extern __shared__ __align__(128) unsigned char smem[];
 
   const int TM = p.tile_mats;
@@ -313,7 +323,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
 
   if (tid == 0) {
     for (int s = 0; s < S; s++) {
-      mbar_init(&full[s], 1);
+      mbar_init(&full[s], FIX8 ? 2 : 1);
       mbar_init(&empty[s], 1);
     }
     fence_mbar_init();
@@ -348,44 +358,45 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
             *reinterpret_cast<uint64_t *>(st + (FIRST + o) * slot_bytes + b16) =
                 *reinterpret_cast<const uint64_t *>(src[o] + goff + b16);
         }
-        if (!SHIFT) {
-          mbar_arrive_expect_tx(&full[s], NIN * b16);
-        } else {
-          // the shifted operand: runs of whole records [Ra, Rb) whose sources are contiguous
+        uint32_t total = NPLAIN * b16;
+        if (SHIFT) {
+          // the shifted operand: runs of whole records [Ra, Rb) whose sources are contiguous.  Record indices fit 31 bits
+          // (checked by the host), so the run arithmetic is 32-bit; only byte offsets are 64-bit.
           const unsigned char *gy = src[NIN - 1];
           unsigned char *sy = st + (NSLOT - 1) * slot_bytes + p.sh.phase;
-          const long long R0 = m0 / W, R1 = (m0 + nm) / W;
-          const uint32_t rb = 9u * W * CB;  // bytes per record
-          const long long blk0 = R0 / p.sh.P;
-          tinfo[s] = make_int2((int)(blk0 % p.sh.rd), (int)(R0 - blk0 * p.sh.P));
-          uint32_t total = NPLAIN * b16;
-          for (int pass = 0; pass < 2; pass++) {
-            long long Ra = R0;
-            while (Ra < R1) {
-              const long long blk = Ra / p.sh.P;
-              const int oc = (int)(blk % p.sh.rd);
-              const bool carry = oc + p.sh.dmod >= p.sh.rd;
-              const long long cyc = blk - oc;  // first block of this rd-cycle
-              long long Rb = (carry ? cyc + p.sh.rd : cyc + p.sh.rd - p.sh.dmod) * p.sh.P;
-              if (Rb > R1) Rb = R1;
-              const long long Rs = Ra + (long long)(carry ? p.sh.dmod - p.sh.rd : p.sh.dmod) * p.sh.P;
-              // byte ranges; with 72-byte records (fp32, W = 1) an odd source record starts on an 8-byte boundary: the
-              // first / last 8 bytes of the run then travel by a plain load/store and the aligned middle by TMA
-              size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
-              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
-              const size_t gs16 = (gs + 15) & ~(size_t)15, ge16 = ge & ~(size_t)15;
-              if (pass == 0) {
-                if (gs16 != gs) *reinterpret_cast<uint64_t *>(d) = *reinterpret_cast<const uint64_t *>(gy + gs);
-                if (ge16 != ge && ge16 >= gs16) *reinterpret_cast<uint64_t *>(d + (ge16 - gs)) = *reinterpret_cast<const uint64_t *>(gy + ge16);
-                if (ge16 > gs16) total += (uint32_t)(ge16 - gs16);
-              } else if (ge16 > gs16) {
-                if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
-                else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
-              }
-              Ra = Rb;
+          const int P = (int)p.sh.P, rd = p.sh.rd, dmod = p.sh.dmod;
+          const int R0 = (int)(m0 / W), R1 = (int)((m0 + nm) / W);
+          constexpr uint32_t rb = 9u * W * CB;  // bytes per record
+          int blk = R0 / P;
+          int oc = blk % rd;
+          tinfo[s] = make_int2(oc, R0 - blk * P);
+          int Ra = R0;
+          while (Ra < R1) {
+            const bool carry = oc + dmod >= rd;
+            const int cyc = blk - oc;  // first block of this rd-cycle
+            const int eb = carry ? cyc + rd : cyc + rd - dmod;  // first block after this run
+            const long long Rbl = (long long)eb * P;
+            const int Rb = Rbl < R1 ? (int)Rbl : R1;
+            const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
+            const size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
+            unsigned char *d = sy + (size_t)(Ra - R0) * rb;
+            size_t gs16 = gs, ge16 = ge;
+            if (FIX8) {  // the first / last 8 bytes of a run that is not 16-byte aligned
+              gs16 = (gs + 15) & ~(size_t)15;
+              ge16 = ge & ~(size_t)15;
+              if (gs16 != gs) cp_async8(d, gy + gs);
+              if (ge16 != ge && ge16 >= gs16) cp_async8(d + (ge16 - gs), gy + ge16);
             }
-            if (pass == 0) mbar_arrive_expect_tx(&full[s], total);
+            if (ge16 > gs16) {
+              total += (uint32_t)(ge16 - gs16);
+              if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
+              else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
+            }
+            Ra = Rb;
+            blk = eb;          // the next run starts at the block where the carry status flips
+            oc = eb % rd;
           }
+          if (FIX8) cp_async_arrive_noinc(&full[s]);  // arrives once all cp.async copies above have landed (at once if none)
         }
 #pragma unroll
         for (int o = 0; o < NPLAIN; o++) {
@@ -394,6 +405,9 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
           else
             bulk_g2s(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s]);
         }
+        // expect-tx and the producer's arrival come LAST: the phase cannot complete before this arrival, and by now
+        // the byte count of the runs is known (the transaction count may be transiently negative until here)
+        mbar_arrive_expect_tx(&full[s], total);
         if (++s == S) {
           s = 0;
           ph ^= 1u;
@@ -462,6 +476,108 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
     }
   }
   if (t == 0) bulk_wait_all<0>();  // smem must outlive the last store; writes complete before exit
+}
+
+// ---------------------------------------------------------------- Cshift as a pure TMA copy (f3)
+// z[s] = y[s + disp*dim_hat] moves whole records, and in storage order a tile's sources are a few contiguous runs (see
+// ShiftInfo).  So Cshift is the ceiling kernel su3_bulk_copy_kernel with its one load per tile split into runs: one warp
+// per CTA, lane 0 moves tiles global -> shared -> global with bulk copies through a ring of `stages` buffers, and no
+// register ever holds data -- except for records that cross the sub-lattice boundary in a dimension that is split over
+// virtual nodes (simd_d > 1): their lanes rotate (S3), which the warp does in place in shared memory before the store.
+// p.x = the shifted field y, p.z = z; p.tile_mats = matrices per tile (a multiple of W).
+template <typename R, int W>
+__global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams p) {
+  typedef typename Cplx<R>::type C2;
+  constexpr int CB = (int)sizeof(C2);
+  constexpr uint32_t rb = 9u * W * CB;  // bytes per record
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int S = p.stages, lane = threadIdx.x;
+  const int TR = p.tile_mats / W;  // records per tile
+  const uint32_t tile_bytes = (uint32_t)TR * rb;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem + (size_t)S * tile_bytes);
+  const int P = (int)p.sh.P, rd = p.sh.rd, dmod = p.sh.dmod;
+  const int nrec = (int)(p.nmat / W);
+  const int ntiles = (nrec + TR - 1) / TR;
+  const unsigned char *gy = (const unsigned char *)p.x;
+  unsigned char *gz = (unsigned char *)p.z;
+  const int mine = ntiles > (int)blockIdx.x ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+  // runs of tile [R0, R1): fn(first record, one past the last, carry)
+  auto for_runs = [&](int R0, int R1, auto &&fn) {
+    int blk = R0 / P, oc = blk % rd, Ra = R0;
+    while (Ra < R1) {
+      const bool carry = oc + dmod >= rd;
+      const int eb = blk - oc + (carry ? rd : rd - dmod);  // first block after this run
+      const long long Rbl = (long long)eb * P;
+      const int Rb = Rbl < R1 ? (int)Rbl : R1;
+      fn(Ra, Rb, carry);
+      Ra = Rb;
+      blk = eb;
+      oc = eb % rd;
+    }
+  };
+  auto load = [&](int i) {  // lane 0 only
+    const int s = i % S;
+    const int R0 = ((int)blockIdx.x + i * (int)gridDim.x) * TR;
+    const int R1 = R0 + TR < nrec ? R0 + TR : nrec;
+    unsigned char *buf = smem + (size_t)s * tile_bytes;
+    mbar_arrive_expect_tx(&full[s], (uint32_t)(R1 - R0) * rb);
+    for_runs(R0, R1, [&](int Ra, int Rb, bool carry) {
+      const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
+      bulk_g2s(buf + (size_t)(Ra - R0) * rb, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
+    });
+  };
+  if (lane == 0) {
+    for (int s = 0; s < S; s++) mbar_init(&full[s], 1);
+    fence_mbar_init();
+    fence_proxy_async();
+    for (int i = 0; i < mine && i < S; i++) load(i);
+  }
+  __syncwarp();
+  for (int i = 0; i < mine; i++) {
+    const int s = i % S;
+    const int R0 = ((int)blockIdx.x + i * (int)gridDim.x) * TR;
+    const int R1 = R0 + TR < nrec ? R0 + TR : nrec;
+    unsigned char *buf = smem + (size_t)s * tile_bytes;
+    mbar_wait(&full[s], (uint32_t)((i / S) & 1));
+    if (W > 1 && p.sh.simd_d > 1) {
+      // lane rotation of the records whose neighbour sits in another virtual node: new[e][l] = old[e][l'], with
+      // ic' = (ic + qrot + carry) mod simd_d
+      for_runs(R0, R1, [&](int Ra, int Rb, bool carry) {
+        const int rot = (p.sh.qrot + (carry ? 1 : 0)) % p.sh.simd_d;
+        if (rot == 0) return;
+        constexpr int PER = (9 * W + 31) / 32;
+        for (int r = Ra; r < Rb; r++) {
+          C2 *rec = reinterpret_cast<C2 *>(buf + (size_t)(r - R0) * rb);
+          C2 v[PER];
+#pragma unroll
+          for (int k = 0; k < PER; k++) {
+            const int idx = k * 32 + lane;
+            if (idx < 9 * W) {
+              const int l = idx % W, ic = (l / p.sh.lstride) % p.sh.simd_d;
+              const int ls = l + ((ic + rot) % p.sh.simd_d - ic) * p.sh.lstride;
+              v[k] = rec[idx - l + ls];
+            }
+          }
+          __syncwarp();
+#pragma unroll
+          for (int k = 0; k < PER; k++)
+            if (k * 32 + lane < 9 * W) rec[k * 32 + lane] = v[k];
+        }
+      });
+      fence_proxy_async();
+    }
+    __syncwarp();
+    if (lane == 0) {
+      bulk_s2g(gz + (size_t)R0 * rb, buf, (uint32_t)(R1 - R0) * rb);
+      bulk_commit();
+      // the store before this one has finished reading its buffer: refill that buffer
+      if (i >= 1) {
+        bulk_wait_read<1>();
+        if (i - 1 + S < mine) load(i - 1 + S);
+      }
+    }
+  }
+  if (lane == 0) bulk_wait_all<0>();
 }
 
 // ---------------------------------------------------------------- direct path (path = 2)
@@ -542,20 +658,23 @@ template <typename R, int W, int NCW>
 __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams p) {
   typedef typename Cplx<R>::type C2;
   constexpr int CB = (int)sizeof(C2);
-  constexpr int MPS = 32;
   extern __shared__ __align__(128) unsigned char smem[];
+  const int MPS = p.tile_mats;  // matrices per stage and operand: 32, or 64 (two per lane) for fp32 programs with few operands
   const int SW = p.stages, ncw = p.ncw, S = SW * ncw, NIN = p.nops;
-  constexpr uint32_t slot_bytes = (uint32_t)MPS * 9u * CB;
+  const uint32_t slot_bytes = (uint32_t)MPS * 9u * CB;
   const uint32_t stage_bytes = NIN * slot_bytes;
   unsigned char *temps = smem + (size_t)S * stage_bytes;  // [ncw][ntemp] slots, private to a warp
-  uint64_t *full = reinterpret_cast<uint64_t *>(temps + (size_t)ncw * p.ntemp * slot_bytes);
+  unsigned char *outs = temps + (size_t)ncw * p.ntemp * slot_bytes;  // [ncw] result slots: the bulk store's source
+  uint64_t *full = reinterpret_cast<uint64_t *>(outs + (size_t)ncw * slot_bytes);
   const int tid = threadIdx.x;
   const long long ntiles = (p.nmat + MPS - 1) / MPS;
   // every warp is a self-contained pipeline: lane 0 issues the bulk loads of the warp's own tiles into the
-  // warp's private ring of SW stages and re-arms a stage as soon as the warp's store has read it
+  // warp's private ring of SW stages.  The result of a tile goes to the warp's own result slot, so a stage is
+  // re-armed as soon as the warp has finished READING it -- the refill never waits for the store.
   const int lane = tid & 31, w = tid >> 5;
   if (w >= ncw) return;
   unsigned char *mytemps = temps + (size_t)w * p.ntemp * slot_bytes;
+  unsigned char *myout = outs + (size_t)w * slot_bytes;
   const long long gw = (long long)blockIdx.x * ncw + w, GW = (long long)gridDim.x * ncw;
   const long long mine = ntiles > gw ? (ntiles - gw + GW - 1) / GW : 0;  // my tiles: gw, gw + GW, ...
   auto load = [&](long long j) {  // lane 0 only
@@ -588,6 +707,9 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
     const long long left = p.nmat - m0;
     const int nm = left < MPS ? (int)left : MPS;
     unsigned char *st = smem + (size_t)s * stage_bytes;
+    // the previous tile's store (issued a whole tile ago) must have finished READING the result slot
+    if (lane == 0) bulk_wait_read<0>();
+    __syncwarp();
     mbar_wait(&full[s], (uint32_t)((j / SW) & 1));
 #pragma unroll 1
     for (int t = lane; t < nm; t += 32) {
@@ -646,23 +768,23 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
           for (int e = 0; e < 9; e++) acc[e] = a[e];
         }
       }
-      C2 *so = reinterpret_cast<C2 *>(st) + base;  // result over operand slot 0: every read of this thread is done
+      C2 *so = reinterpret_cast<C2 *>(myout) + base;  // the warp's own result slot
 #pragma unroll
       for (int e = 0; e < 9; e++) so[e * W] = acc[e];
     }
     fence_proxy_async();
     __syncwarp();
+    // every lane has read what it needs from stage s (operand slots are only read): re-arm it with my tile j + SW
+    // at once -- the refill never waits for the store -- and send the result on its way
     if (lane == 0) {
+      if (j + SW < mine) load(j + SW);
       const uint32_t bytes = (uint32_t)nm * 9u * CB;
       const uint32_t b16 = bytes & ~15u;
       unsigned char *zdst = (unsigned char *)p.z + (size_t)m0 * 9u * CB;
-      bulk_s2g(zdst, st, b16);
+      bulk_s2g(zdst, myout, b16);
       bulk_commit();
-      if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(st + b16);
-      bulk_wait_read<0>();  // the store has read the stage: refill it with my tile j + SW
-      if (j + SW < mine) load(j + SW);
+      if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(myout + b16);
     }
-    __syncwarp();
   }
   if (lane == 0) bulk_wait_all<0>();
 }
@@ -1366,7 +1488,7 @@ __global__ void __launch_bounds__(256) su3_convert_staged_kernel(const ConvertPa
 // Bulk copies need 16-byte alignment: with 8-byte complex numbers (fp32) the host only selects this kernel when every
 // run starts and ends on an even complex index (true for every even lattice); otherwise the staged kernel above runs.
 template <typename C2, int W, int NC, int N, int NT>
-__global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams p) {
+__global__ void __launch_bounds__(NT, 8) su3_convert_tma_kernel(const ConvertParams p) {
   constexpr int CB = (int)sizeof(C2);
   constexpr int TR = N / (NC * W);      // records per tile
   constexpr int PER = (N + NT - 1) / NT;
@@ -1388,18 +1510,20 @@ __global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams
     fence_proxy_async();
   }
   __syncthreads();
-  // scalar-side complex index of (vector record rec, lane 0, element 0): the virtual-node map S3 for the outer site
+  // scalar-side complex index of (vector record rec, lane 0, element 0): the virtual-node map S3 for the outer site.
+  // Record and site indices fit 31 bits (one launch has < 2^31 blocks of >= 1 record and the host checks the volume),
+  // so the decomposition runs in 32-bit arithmetic; only the final complex index is 64-bit.
   auto sbase = [&](long long rec) {
-    long long o = rec / p.nl;
-    const int mu = (int)(rec - o * p.nl);
-    long long site = 0;
+    unsigned o = (unsigned)rec / (unsigned)p.nl;
+    const unsigned mu = (unsigned)rec - o * (unsigned)p.nl;
+    unsigned site = 0;
 #pragma unroll
     for (int d = 0; d < 4; d++) {
-      const long long q = o / p.r[d];
-      site += (o - q * p.r[d]) * p.sstride[d];
+      const unsigned q = o / (unsigned)p.r[d];
+      site += (o - q * (unsigned)p.r[d]) * (unsigned)p.sstride[d];
       o = q;
     }
-    return (site * p.nl + mu) * NC;
+    return ((long long)site * p.nl + mu) * NC;
   };
   // lane l's runs of the tile: [a, b) in records, cut at multiples of run_recs
   auto for_runs = [&](auto &&fn) {
@@ -1429,19 +1553,38 @@ __global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams
     bulk_g2s(tile, src + (size_t)rec0 * NC * W * CB, (uint32_t)n * CB, bar);
   }
   mbar_wait(bar, 0);
+  // Slot idx of the block handles element (lane l, row k).  Plain order (l fastest) is conflict-free on both sides for
+  // 16-byte complex numbers and for W <= 8; with 8-byte complex numbers and W >= 16 a half-warp would hit 16 rows whose
+  // bases are all even (rows are 16-byte aligned), i.e. 8 bank pairs: there lanes 0-7 of a 16-lane group take row 2j
+  // and lanes 8-15 row 2j+1 in one half-warp, the other way round in the next (pitch = 2 mod 16).
+  const int K = nr * NC;
+  auto decode = [&](int idx, int &l, int &k) {
+    if (CB == 8 && W >= 16) {
+      const int i = idx & 31, blk = idx >> 5;
+      constexpr int G = W >= 16 ? W / 16 : 1;  // 16-lane groups per record
+      const int g = blk % G, kp = blk / G;
+      l = 16 * g + (i & 15);
+      k = 2 * kp + (((i >> 4) + ((i & 15) >> 3)) & 1);
+    } else {
+      l = idx % W;
+      k = idx / W;
+    }
+  };
   C2 v[PER];
 #pragma unroll
   for (int i = 0; i < PER; i++) {
-    const int idx = i * NT + tid;  // dense (vector-side) index: lane fastest
-    if (idx < n) v[i] = p.to_vector ? tile[(idx % W) * pitch + idx / W] : tile[idx];
+    int l, k;
+    decode(i * NT + tid, l, k);
+    if (k < K) v[i] = p.to_vector ? tile[l * pitch + k] : tile[k * W + l];
   }
   __syncthreads();
 #pragma unroll
   for (int i = 0; i < PER; i++) {
-    const int idx = i * NT + tid;
-    if (idx < n) {
-      if (p.to_vector) tile[idx] = v[i];
-      else tile[(idx % W) * pitch + idx / W] = v[i];
+    int l, k;
+    decode(i * NT + tid, l, k);
+    if (k < K) {
+      if (p.to_vector) tile[k * W + l] = v[i];
+      else tile[l * pitch + k] = v[i];
     }
   }
   fence_proxy_async();
@@ -1450,7 +1593,7 @@ __global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams
     if (tid == 0) {
       bulk_s2g(dst + (size_t)rec0 * NC * W * CB, tile, (uint32_t)n * CB);
       bulk_commit();
-      bulk_wait_all<0>();
+      bulk_wait_read<0>();  // the tile may be handed to the next block once the store has READ it; the grid's completion covers the write
     }
   } else if (tid < W) {
     const long long loff = p.lane_off[tid];
@@ -1458,7 +1601,7 @@ __global__ void __launch_bounds__(NT) su3_convert_tma_kernel(const ConvertParams
       bulk_s2g(dst + (size_t)(sbase(a) + loff) * CB, tile + (size_t)tid * pitch + (a - rec0) * NC, (uint32_t)((b - a) * NC) * CB);
     });
     bulk_commit();
-    bulk_wait_all<0>();
+    bulk_wait_read<0>();
   }
 }
 

@@ -39,6 +39,17 @@ inline bool menu_elementwise(int op) {
   return op == su3::OP_ADD || op == su3::OP_ADD3 || op == su3::OP_ADD4 || op == su3::OP_SUB || op == su3::OP_EMUL ||
          op == su3::OP_SUM_EPROD;
 }
+template <typename R> stream_kernel_t cshift_bulk_for_w(int W) {
+  switch (W) {
+    case 1: return su3::su3_cshift_bulk_kernel<R, 1>;
+    case 2: return su3::su3_cshift_bulk_kernel<R, 2>;
+    case 4: return su3::su3_cshift_bulk_kernel<R, 4>;
+    case 8: return su3::su3_cshift_bulk_kernel<R, 8>;
+    case 16: return su3::su3_cshift_bulk_kernel<R, 16>;
+    case 32: return su3::su3_cshift_bulk_kernel<R, 32>;
+  }
+  return nullptr;
+}
 // the pipeline with a shifted last operand: z = x . y(+disp) (OP_MUL) and z = y(+disp) (OP_COPY, Cshift)
 template <typename R> stream_kernel_t shift_pipe_any(int op, int W) {
   return op == su3::OP_MUL ? pipe_for_w<R, su3::OP_MUL, 1>(W) : pipe_for_w<R, su3::OP_COPY, 1>(W);
@@ -149,14 +160,15 @@ stream_kernel_t stream_f32(int family, int op, int W);
 stream_kernel_t menu_f64(int op, int W);
 stream_kernel_t menu_f32(int op, int W);
 stream_kernel_t shift_pipe_kernel(int prec, int op, int W);
+stream_kernel_t cshift_bulk_kernel(int prec, int W);
 stream_kernel_t matvec_kernel(int prec, int W);
 expr_kernel_t expr_kernel(int prec, int W);
 shift_kernel_t shift_kernel(int prec, int op, int W, bool idx32);        // register version (SH_COPY / SH_MUL)
 shift_kernel_t cshift_async_kernel(int prec, int W, bool idx32);
 // layout conversion: launches the kernel for (prec, nc, W); returns false if W is not supported
 bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertParams &p, cudaStream_t s, const char **err);
-// the TMA variant: complex numbers per tile for (prec, big), and the launch (p.pitch and p.run_recs must be set)
-int convert_tma_tile(int prec, bool big);
-bool launch_convert_tma(int prec, int nc, int W, bool big, const su3::ConvertParams &p, cudaStream_t s, const char **err);
+// the TMA variant: complex numbers per tile, and the launch (p.pitch and p.run_recs must be set)
+int convert_tma_tile(int prec);
+bool launch_convert_tma(int prec, int nc, int W, const su3::ConvertParams &p, cudaStream_t s, const char **err);
 
 }  // namespace su3tab
