@@ -787,12 +787,33 @@ def profile_pass(args):
             su3.su3_tune_set(path=2)
             su3.su3_add(z, x, y); su3.su3_copy(z, x)
             su3.su3_tune_set()
+            su3.su3_expr(z, "01+01*+", [x, y]); su3.su3_expr(z, "01*23*+", [x, y, w, x])        # menu rows of the pipeline
+            su3.su3_tune_set(path=3)                                                             # the interpreter
             su3.su3_expr(z, "01+01*+", [x, y]); su3.su3_expr(z, "01*23*+", [x, y, w, x])
-            su3.su3_cshift(z, y, 0, 1); su3.su3_cshift(z, y, 3, 1); su3.su3_mul_shift(z, x, y, 1, 1)
+            su3.su3_tune_set()
+            su3.su3_expr(z, "01*2*3*", [x, y, w, x])                                            # not on the menu
+            order.append("%s expr: menu x2, interpreter x3" % name)
+            for dim in (0, 3):
+                su3.su3_cshift(z, y, dim, 1); su3.su3_mul_shift(z, x, y, dim, 1)                 # bulk-run Cshift, shifted pipeline
+            su3.su3_tune_set(path=2)
+            su3.su3_cshift(z, y, 0, 1); su3.su3_mul_shift(z, x, y, 1, 1)                         # register kernels
+            su3.su3_tune_set(path=3)
+            su3.su3_cshift(z, y, 0, 1)                                                           # cp.async gather
+            su3.su3_tune_set()
             psi = su3.su3_vec_wrap(x.desc, w.tensor[:su3.su3_vec_bytes(x.desc)])
             yv_ = su3.su3_vec_wrap(x.desc, z.tensor[:su3.su3_vec_bytes(x.desc)])
             su3.su3_matvec(yv_, x, psi)
         su3.su3_convert(zs, zv)
+        for path in (3, 2):                       # the per-thread convert kernels (staged / unstaged), both directions
+            su3.su3_tune_set(path=path)
+            su3.su3_convert(xv, xs); su3.su3_convert(zs, xv)
+        su3.su3_tune_set()
+        if prec == su3.SU3_F32:                   # A5 at the long vector lengths of the W sweep (f1)
+            for Wl in (16, 32):
+                dl = su3.make_desc(L, prec=prec, layout=su3.SU3_VECTOR, W=Wl)
+                xl = su3.alloc_field(dl)
+                su3.su3_convert(xl, xs); su3.su3_convert(zs, xl)
+                del xl
         torch.cuda.synchronize()
         del xs, ys, ws, zs, xv, yv, wv, zv
         torch.cuda.empty_cache()

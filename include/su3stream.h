@@ -173,8 +173,8 @@ su3_status su3_expr_plan(const char *program, int n_operands, int real_fields, c
 su3_status su3_expr_cost(const char *program, int n_operands, int32_t *streams, int32_t *flops_per_matrix);
 
 /* Circular shift, Grid's Cshift(x, dim, disp) (P:219 names it as the next obstacle after the site-local
- * product): z[s] = x[s + disp*dim_hat], periodic, for every site s and every mu; dim in 0..3, disp any
- * integer.  A pure, bit-exact permutation of matrices in either layout (in the vector layout a step across
+ * product): z[s] = x[s + disp*dim_hat], periodic ON THE LOCAL LATTICE OF THE HANDLE (one rank's slab in a multi-GPU
+ * job: see the su3_face_* calls below), for every site s and every mu; dim in 0..3, disp any integer.  A pure, bit-exact permutation of matrices in either layout (in the vector layout a step across
  * a sub-lattice boundary moves a matrix to another lane).  Identical descriptors (SU3_ERR_MISMATCH); z and
  * x must not be the same field (SU3_ERR_MISMATCH); dim outside 0..3 -> SU3_ERR_INVALID. */
 su3_status su3_cshift(su3_field *z, const su3_field *x, int dim, int disp, void *cuda_stream);
@@ -217,6 +217,24 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *cuda_stream);
 /* dst = src, own 128-bit copy kernel: the same-run bandwidth ceiling.  Fields
  * must have identical descriptors.  A6. */
 su3_status su3_copy(su3_field *dst, const su3_field *src, void *cuda_stream);
+
+/* Faces of a slab: what a Cshift along `dim` needs from the neighbouring rank when the lattice is split into x_dim slabs
+ * over GPUs (the first exchange step of this code base; P:219 names Cshift as the operation after the site-local
+ * product, and Grid's Cshift sends exactly such faces).  su3_cshift / su3_mul_shift are periodic on the LOCAL lattice of
+ * the handle; a multi-GPU shift = the local shift + these calls around one send/recv (paper_1710_09409_b200/halo.py).
+ * The face of planes x_dim in [plane0, plane0 + nplanes) is moved between a field (either layout) and a PACKED device
+ * buffer in plane order, the same for every layout so that ranks may exchange it blindly: matrix
+ *   b = (x0 + L0*(x1 + L1*(x2 + L2*x3)) with (x_dim - plane0) in place of x_dim and nplanes in place of L[dim]) * n_lorentz + mu
+ * sits at complex index b*9 (b*3 for colour-vector fields), row-major, (re, im) adjacent -- i.e. the packed face IS a
+ * scalar-layout field of extents L with L[dim] = nplanes.  su3_face_bytes = its size.  Bit-exact permutations.
+ *   su3_face_pack  : buffer <- planes of x          su3_face_unpack: planes of z <- buffer
+ *   su3_face_copy  : planes [z_plane0, +n) of z <- planes [x_plane0, +n) of x, same descriptor; x may be memory of a PEER
+ *                    device mapped into this process (NVLink P2P): the exchange is then this single launch.
+ * plane range outside 0..L[dim] -> SU3_ERR_INVALID; buffer too small -> SU3_ERR_SIZE, misaligned -> SU3_ERR_ALIGN. */
+su3_status su3_face_bytes(const su3_field *f, int dim, int nplanes, size_t *nbytes);
+su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, int dim, int plane0, int nplanes, void *cuda_stream);
+su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, int dim, int plane0, int nplanes, void *cuda_stream);
+su3_status su3_face_copy(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes, void *cuda_stream);
 
 /* End-to-end z = x*y with HOST buffers: x_host, y_host (inputs) and z_host (output) are host
  * arrays of su3_field_bytes bytes in the layout of the (identical) descriptors of the three

@@ -17,7 +17,8 @@ SU3_SCALAR, SU3_VECTOR = 0, 1
 EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normalize", "su3_field_wrap",
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
            "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_expr_plan", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
-           "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release"]
+           "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release",
+           "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy"]
 
 
 class su3_desc(ctypes.Structure):
@@ -78,6 +79,10 @@ def _load():
         "su3_device_info": (i32, [ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), ctypes.POINTER(i32)]),
         "su3_device_name": (i32, [ctypes.c_char_p, sz, ctypes.POINTER(i32)]),
         "su3_host_release": (i32, []),
+        "su3_face_bytes": (i32, [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(sz)]),
+        "su3_face_pack": (i32, [vp, sz, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
+        "su3_face_unpack": (i32, [vp, vp, sz, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
+        "su3_face_copy": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -338,3 +343,24 @@ def su3_device_name():
 
 def su3_host_release():
     _ck(lib.su3_host_release())
+
+
+def su3_face_bytes(field, dim, nplanes):
+    n = ctypes.c_size_t()
+    _ck(lib.su3_face_bytes(field.handle, int(dim), int(nplanes), ctypes.byref(n)))
+    return n.value
+
+
+def su3_face_pack(buf, x, dim, plane0, nplanes, stream=None):
+    """buf (a uint8 device tensor) <- planes [plane0, plane0+nplanes) of x along dim, in plane order"""
+    _ck(lib.su3_face_pack(ctypes.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size(), x.handle, int(dim),
+                          int(plane0), int(nplanes), _stream(stream)))
+
+
+def su3_face_unpack(z, buf, dim, plane0, nplanes, stream=None):
+    _ck(lib.su3_face_unpack(z.handle, ctypes.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size(), int(dim),
+                            int(plane0), int(nplanes), _stream(stream)))
+
+
+def su3_face_copy(z, z_plane0, x, x_plane0, dim, nplanes, stream=None):
+    _ck(lib.su3_face_copy(z.handle, int(z_plane0), x.handle, int(x_plane0), int(dim), int(nplanes), _stream(stream)))

@@ -1048,6 +1048,85 @@ su3_status su3_convert(su3_field *dst, const su3_field *src, void *stream) {
   return SU3_OK;
 }
 
+// ---------------------------------------------------------------- faces of a slab (multi-GPU Cshift)
+static su3_status face_args(const su3_field *f, int dim, int plane0, int nplanes, size_t *bytes) {
+  if (!f) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (f->ncomp == 0) return fail(SU3_ERR_MISMATCH, "faces exist for colour-matrix and colour-vector fields only");
+  if (dim < 0 || dim > 3) return fail(SU3_ERR_INVALID, "dim = %d outside 0..3", dim);
+  if (nplanes < 0 || plane0 < 0 || (int64_t)plane0 + nplanes > f->d.L[dim])
+    return fail(SU3_ERR_INVALID, "planes [%d, %d) outside 0..%d of dimension %d", plane0, plane0 + nplanes, f->d.L[dim], dim);
+  *bytes = (size_t)(f->volume / f->d.L[dim]) * (size_t)nplanes * f->d.n_lorentz * f->ncomp * 2 * f->d.prec;
+  return SU3_OK;
+}
+
+static void face_side(su3::FaceSide *g, const su3_field *f, bool packed, int plane0) {
+  g->packed = packed ? 1 : 0;
+  g->plane0 = plane0;
+  g->W = f->d.W;
+  g->nl = f->d.n_lorentz;
+  for (int k = 0; k < 4; k++) {
+    g->L[k] = f->d.L[k];
+    g->simd[k] = f->d.simd[k];
+  }
+}
+
+// geo = the field whose descriptor defines the face; dpacked / spacked say which side is the plane-order buffer
+static su3_status launch_face_copy(const su3_field *geo, void *dst, bool dpacked, int dplane0, const void *src, bool spacked,
+                                   int splane0, int dim, int nplanes, void *stream) {
+  su3::FaceParams p;
+  memset(&p, 0, sizeof p);
+  p.dst = dst; p.src = src; p.dim = dim;
+  face_side(&p.d, geo, dpacked, dplane0);
+  face_side(&p.s, geo, spacked, splane0);
+  long long n = 1;
+  for (int k = 0; k < 4; k++) {
+    p.F[k] = k == dim ? nplanes : geo->d.L[k];
+    n *= p.F[k];
+  }
+  p.ncplx = n * geo->d.n_lorentz * geo->ncomp;
+  if (p.ncplx == 0) return SU3_OK;
+  su3tab::launch_face(geo->d.prec, geo->ncomp, flat_grid((size_t)p.ncplx, 1024, 8), p, (cudaStream_t)stream);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("su3_face launch", e);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return SU3_OK;
+}
+
+su3_status su3_face_bytes(const su3_field *f, int dim, int nplanes, size_t *nbytes) {
+  if (!nbytes) return fail(SU3_ERR_NULL, "nbytes is NULL");
+  return face_args(f, dim, 0, nplanes, nbytes);
+}
+
+su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, int dim, int plane0, int nplanes, void *stream) {
+  size_t need = 0;
+  if (su3_status st = face_args(x, dim, plane0, nplanes, &need)) return st;
+  if (!buf_dev) return fail(SU3_ERR_NULL, "buffer pointer is NULL");
+  if ((uintptr_t)buf_dev % 16) return fail(SU3_ERR_ALIGN, "face buffer is not 16-byte aligned");
+  if (buf_bytes < need) return fail(SU3_ERR_SIZE, "face buffer has %zu bytes, the face needs %zu", buf_bytes, need);
+  if (su3_status sd = on_current_device({x})) return sd;
+  return launch_face_copy(x, buf_dev, true, 0, x->ptr, false, plane0, dim, nplanes, stream);
+}
+
+su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, int dim, int plane0, int nplanes, void *stream) {
+  size_t need = 0;
+  if (su3_status st = face_args(z, dim, plane0, nplanes, &need)) return st;
+  if (!buf_dev) return fail(SU3_ERR_NULL, "buffer pointer is NULL");
+  if ((uintptr_t)buf_dev % 16) return fail(SU3_ERR_ALIGN, "face buffer is not 16-byte aligned");
+  if (buf_bytes < need) return fail(SU3_ERR_SIZE, "face buffer has %zu bytes, the face needs %zu", buf_bytes, need);
+  if (su3_status sd = on_current_device({z})) return sd;
+  return launch_face_copy(z, z->ptr, false, plane0, buf_dev, true, 0, dim, nplanes, stream);
+}
+
+su3_status su3_face_copy(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes, void *stream) {
+  size_t need = 0;
+  if (su3_status st = face_args(z, dim, z_plane0, nplanes, &need)) return st;
+  if (su3_status st = face_args(x, dim, x_plane0, nplanes, &need)) return st;
+  if (!same_desc(z->d, x->d) || z->ncomp != x->ncomp) return fail(SU3_ERR_MISMATCH, "su3_face_copy needs identical descriptors and field kinds");
+  if (z->ptr == x->ptr) return fail(SU3_ERR_MISMATCH, "su3_face_copy: z and x must be different fields");
+  if (su3_status sd = on_current_device({z})) return sd;  // x may be peer memory: only the destination must be local
+  return launch_face_copy(z, z->ptr, false, z_plane0, x->ptr, false, x_plane0, dim, nplanes, stream);
+}
+
 su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
                          su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream) {
   if (op != SU3_OP_MUL && op != SU3_OP_MUL3 && op != SU3_OP_MUL_ADD) return fail(SU3_ERR_INVALID, "op = %d not in {0,1,2}", op);

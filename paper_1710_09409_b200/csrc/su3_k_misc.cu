@@ -20,6 +20,13 @@ template <typename C2, int NC, int N> bool convert_tma_w(int W, const su3::Conve
   *err = "unsupported W";
   return false;
 }
+void launch_face(int prec, int nc, unsigned grid, const su3::FaceParams &p, cudaStream_t s) {
+  if (prec == 8 && nc == 9) su3::su3_face_kernel<double2, 9><<<grid, 256, 0, s>>>(p);
+  else if (prec == 8) su3::su3_face_kernel<double2, 3><<<grid, 256, 0, s>>>(p);
+  else if (nc == 9) su3::su3_face_kernel<float2, 9><<<grid, 256, 0, s>>>(p);
+  else su3::su3_face_kernel<float2, 3><<<grid, 256, 0, s>>>(p);
+}
+
 int convert_tma_tile(int prec) { return prec == 8 ? 1152 : 2304; }
 bool launch_convert_tma(int prec, int nc, int W, const su3::ConvertParams &p, cudaStream_t s, const char **err) {
   if (prec == 8) return nc == 9 ? convert_tma_w<double2, 9, 1152>(W, p, s, err) : convert_tma_w<double2, 3, 1152>(W, p, s, err);

@@ -545,23 +545,27 @@ __global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams 
       for_runs(R0, R1, [&](int Ra, int Rb, bool carry) {
         const int rot = (p.sh.qrot + (carry ? 1 : 0)) % p.sh.simd_d;
         if (rot == 0) return;
-        constexpr int PER = (9 * W + 31) / 32;
-        for (int r = Ra; r < Rb; r++) {
-          C2 *rec = reinterpret_cast<C2 *>(buf + (size_t)(r - R0) * rb);
-          C2 v[PER];
+        // the run's complex numbers, flat: index j holds lane j % W of its element vector, and the source of j lies in the
+        // same W-aligned group; chunks of 32*U numbers (whole groups) are read completely, then written back
+        constexpr int U = 8;
+        C2 *run = reinterpret_cast<C2 *>(buf + (size_t)(Ra - R0) * rb);
+        const int cnt = (Rb - Ra) * 9 * W;
+        const int l = lane % W, ic = (l / p.sh.lstride) % p.sh.simd_d;
+        const int delta = ((ic + rot) % p.sh.simd_d - ic) * p.sh.lstride;   // source lane - own lane (32 % W == 0: same for all j of this thread)
+        for (int c0 = 0; c0 < cnt; c0 += 32 * U) {
+          C2 v[U];
 #pragma unroll
-          for (int k = 0; k < PER; k++) {
-            const int idx = k * 32 + lane;
-            if (idx < 9 * W) {
-              const int l = idx % W, ic = (l / p.sh.lstride) % p.sh.simd_d;
-              const int ls = l + ((ic + rot) % p.sh.simd_d - ic) * p.sh.lstride;
-              v[k] = rec[idx - l + ls];
-            }
+          for (int u = 0; u < U; u++) {
+            const int j = c0 + u * 32 + lane;
+            if (j < cnt) v[u] = run[j + delta];
           }
           __syncwarp();
 #pragma unroll
-          for (int k = 0; k < PER; k++)
-            if (k * 32 + lane < 9 * W) rec[k * 32 + lane] = v[k];
+          for (int u = 0; u < U; u++) {
+            const int j = c0 + u * 32 + lane;
+            if (j < cnt) run[j] = v[u];
+          }
+          __syncwarp();
         }
       });
       fence_proxy_async();
@@ -1602,6 +1606,66 @@ __global__ void __launch_bounds__(NT, 8) su3_convert_tma_kernel(const ConvertPar
     });
     bulk_commit();
     bulk_wait_read<0>();
+  }
+}
+
+// ---------------------------------------------------------------- faces of a slab (multi-GPU Cshift)
+// A lattice split into x_dim slabs over ranks needs, for a shift along dim, the planes x_dim in [plane0, plane0+n) of a
+// neighbouring rank's slab.  One kernel moves such a FACE between any two of: a field in its own layout (scalar or
+// vector: the index function is S2/S3), and a packed buffer in plane order -- matrix b of the buffer is
+// (site of the face in lexicographic order with x_dim - plane0 in place of x_dim, x0 fastest)*nl + mu, its NC complex
+// numbers adjacent.  pack = field -> buffer (what is sent), unpack = buffer -> field (what was received), copy =
+// field -> field (the source may be PEER memory mapped over NVLink: the exchange is then this one launch).
+// One thread per complex number, consecutive threads = consecutive elements of one face matrix.
+struct FaceSide {
+  int packed;   // 1: packed buffer (plane order); 0: field
+  int plane0;   // field: first plane of the face along dim
+  int W, nl;
+  int L[4], simd[4];
+};
+struct FaceParams {
+  void *dst;
+  const void *src;
+  FaceSide d, s;
+  int dim;
+  int F[4];          // extents of the face: L with L[dim] replaced by the number of planes
+  long long ncplx;   // complex numbers to move = prod(F) * nl * NC
+};
+
+template <int NC>
+__device__ __forceinline__ long long face_index(const FaceSide &g, int dim, const int (&c)[4], int mu, int e, long long packed_idx) {
+  if (g.packed) return packed_idx;
+  long long o = 0, ostride = 1, site = 0, sstride = 1;
+  int l = 0, lstride = 1;
+#pragma unroll
+  for (int k = 0; k < 4; k++) {
+    const int x = c[k] + (k == dim ? g.plane0 : 0);
+    const int r = g.L[k] / g.simd[k];
+    site += x * sstride;  sstride *= g.L[k];
+    o += (x % r) * ostride;  ostride *= r;
+    l += (x / r) * lstride;  lstride *= g.simd[k];
+  }
+  if (g.W == 1) return (site * g.nl + mu) * NC + e;
+  return ((o * g.nl + mu) * NC + e) * g.W + l;
+}
+
+template <typename C2, int NC>
+__global__ void __launch_bounds__(256) su3_face_kernel(const FaceParams p) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.ncplx; i += stride) {
+    const int e = (int)(i % NC);
+    long long b = i / NC;
+    const int mu = (int)(b % p.d.nl);
+    b /= p.d.nl;
+    int c[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+      c[k] = (int)(b % p.F[k]);
+      b /= p.F[k];
+    }
+    const long long si = face_index<NC>(p.s, p.dim, c, mu, e, i);
+    const long long di = face_index<NC>(p.d, p.dim, c, mu, e, i);
+    reinterpret_cast<C2 *>(p.dst)[di] = reinterpret_cast<const C2 *>(p.src)[si];
   }
 }
 

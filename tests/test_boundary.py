@@ -340,3 +340,33 @@ def test_ahead_of_time_menu_rows_and_matching():
     p1, p2 = su3.su3_expr_plan("01*", 2, real_fields=True), su3.su3_expr_plan("01+01*+", 2, real_fields=True)
     assert p1[0] == "menu" and p2[0] == "menu" and p1[1] not in rows.values() and p2[1] not in rows.values()
     assert su3.su3_expr_plan("01*2*", 3, real_fields=True) == "interpreter"
+
+
+def test_face_calls_validate_before_any_cuda_work():
+    """su3_face_*: sizes by the header's formula; bad dim / plane range / buffer are rejected host-side"""
+    d = su3.make_desc((6, 4, 2, 8), n_lorentz=4, prec=su3.SU3_F32, layout=su3.SU3_VECTOR, W=4)
+    h, hv, hr = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+    assert su3.lib.su3_field_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), su3.su3_field_bytes(d), ctypes.byref(h)) == su3.SU3_OK
+    assert su3.lib.su3_vec_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), su3.su3_vec_bytes(d), ctypes.byref(hv)) == su3.SU3_OK
+    assert su3.lib.su3_real_wrap(ctypes.byref(d), ctypes.c_void_p(0x1000), su3.su3_real_bytes(d), ctypes.byref(hr)) == su3.SU3_OK
+    n = ctypes.c_size_t()
+    for dim, L in enumerate((6, 4, 2, 8)):
+        assert su3.lib.su3_face_bytes(h, dim, 1, ctypes.byref(n)) == su3.SU3_OK
+        assert n.value == (6 * 4 * 2 * 8 // L) * 4 * 72           # one plane of 72-byte matrices, 4 Lorentz indices
+        assert su3.lib.su3_face_bytes(hv, dim, L, ctypes.byref(n)) == su3.SU3_OK
+        assert n.value == su3.su3_vec_bytes(d)                     # all planes = the whole field
+        assert su3.lib.su3_face_bytes(h, dim, L + 1, ctypes.byref(n)) == su3.SU3_ERR_INVALID
+    assert su3.lib.su3_face_bytes(h, 4, 1, ctypes.byref(n)) == su3.SU3_ERR_INVALID
+    assert su3.lib.su3_face_bytes(hr, 3, 1, ctypes.byref(n)) == su3.SU3_ERR_MISMATCH
+    assert su3.lib.su3_face_bytes(None, 3, 1, ctypes.byref(n)) == su3.SU3_ERR_NULL
+    buf, big = ctypes.c_void_p(0x4000), 1 << 30
+    assert su3.lib.su3_face_pack(buf, big, h, 3, 7, 2, None) == su3.SU3_ERR_INVALID          # planes 7..8 of 0..7
+    assert su3.lib.su3_face_pack(buf, big, h, 3, -1, 1, None) == su3.SU3_ERR_INVALID
+    assert su3.lib.su3_face_pack(None, big, h, 3, 0, 1, None) == su3.SU3_ERR_NULL
+    assert su3.lib.su3_face_pack(ctypes.c_void_p(0x4008), big, h, 3, 0, 1, None) == su3.SU3_ERR_ALIGN
+    assert su3.lib.su3_face_pack(buf, 100, h, 3, 0, 1, None) == su3.SU3_ERR_SIZE
+    assert su3.lib.su3_face_unpack(h, buf, 100, 3, 0, 1, None) == su3.SU3_ERR_SIZE
+    assert su3.lib.su3_face_copy(h, 0, h, 1, 3, 1, None) == su3.SU3_ERR_MISMATCH              # same field
+    assert su3.lib.su3_face_copy(h, 0, hv, 1, 3, 1, None) == su3.SU3_ERR_MISMATCH             # kinds differ
+    for x in (h, hv, hr):
+        su3.lib.su3_field_free(x)
