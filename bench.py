@@ -676,11 +676,19 @@ def run_next_rows(args, r):
         ops = [su3.su3_field_wrap(d, f[n].tensor[:nb]) for n in names]
         z = su3.su3_field_wrap(d, f["zc"].tensor[:nb])
         lay = "scalar" if layout == 0 else "vector W=%d" % W
-        for prog in ("01*", "01*2*", "01*2+", "01+01*+", "01*23*+", "01+2+3+"):
+        # programs on the ahead-of-time menu (they run on the pipeline kernel), programs that are not (the interpreter),
+        # and two menu programs forced through the interpreter (launch knob path = 3) for comparison
+        for prog, force in (("01*", 0), ("01*2*", 0), ("01*2+", 0), ("01+01*+", 0), ("01*23*+", 0), ("01+2+3+", 0),
+                            ("01*2*3*", 0), ("01*23**", 0), ("012**", 0), ("01+01*+", 1), ("01*23*+", 1)):
             n = max(int(c) for c in prog if c.isdigit()) + 1
             st, fl = su3.su3_expr_cost(prog, n)
+            plan = su3.su3_expr_plan(prog, n)
+            if force:
+                su3.su3_tune_set(path=3)
             mn, _, _ = time_calls(torch, lambda: su3.su3_expr(z, prog, ops[:n]))
+            su3.su3_tune_set()
             out["expr"].append({"program": prog, "layout": lay, "streams": st, "flops_per_matrix": fl,
+                                "kernel": "interpreter" if force or plan == "interpreter" else "menu row %d" % plan[1],
                                 "GBps": st * nb / (mn * 1e-3) / 1e9, "GFLOPps": fl * Ln ** 4 / (mn * 1e-3) / 1e9,
                                 "frac_of_copy": st * nb / (mn * 1e-3) / 1e9 / c64})
         for dim in range(4):
@@ -691,6 +699,21 @@ def run_next_rows(args, r):
                                  "cshift_frac_of_copy": 2 * nb / (mn * 1e-3) / 1e9 / c64,
                                  "mul_shift_frac_of_copy": 3 * nb / (mn2 * 1e-3) / 1e9 / c64,
                                  "mul_shift_GFLOPps": FLOPS["mul"] * Ln ** 4 / (mn2 * 1e-3) / 1e9})
+    # (e) the kernels of the multi-GPU shift: pack + unpack of the x3 face of 1 and 4 planes (bytes = 2 x face, each way)
+    out["face"] = []
+    for layout, W, name in ((0, 1, "xs"), (1, W64, "xv")):
+        d = su3.make_desc(Ln, layout=layout, W=W)
+        nb = su3.su3_field_bytes(d)
+        x = su3.su3_field_wrap(d, f[name].tensor[:nb])
+        z = su3.su3_field_wrap(d, f["zc"].tensor[:nb])
+        for n in (1, 4):
+            fb = su3.su3_face_bytes(x, 3, n)
+            buf = torch.empty(fb, dtype=torch.uint8, device=x.tensor.device)
+            t1, _, _ = time_calls(torch, lambda: su3.su3_face_pack(buf, x, 3, 0, n), graph_below_us=60.0)
+            t2, _, _ = time_calls(torch, lambda: su3.su3_face_unpack(z, buf, 3, Ln - n, n), graph_below_us=60.0)
+            out["face"].append({"layout": "scalar" if layout == 0 else "vector W=%d" % W, "planes": n, "face_MB": fb / 1e6,
+                                "pack_us": t1 * 1e3, "unpack_us": t2 * 1e3, "pack_GBps": 2 * fb / (t1 * 1e-3) / 1e9,
+                                "unpack_GBps": 2 * fb / (t2 * 1e-3) / 1e9})
     # BASELINE.json configs[2] and configs[3] as bench points (their parity is in tests/test_gpu_fullsize.py)
     out["configs"] = []
     if args.L >= 48:

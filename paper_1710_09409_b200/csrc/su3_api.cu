@@ -179,9 +179,11 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
   // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
   // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
   // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
+  // Up to 0.6 x L2 (everything stays resident from call to call) the direct kernel wins by 8-40 %; between 0.6 and 2 x L2
+  // the pipeline with its pinned operand prefixes (below) is 6-18 % faster than the direct kernel, which has no L2 policy
+  // (measured at 24^4 fp64 W=4: 7668 vs 7226 GB/s; 28^4 fp32 W=8: 7974 vs 7187).
   const bool direct = base_op && op != su3::OP_ADD &&  // OP_ADD has no direct kernel (su3_add's path = 2 is its own plain kernel)
-                      (tn.path == 2 || (tn.path == 0 && W * cb >= 32 &&
-                                        footprint_bytes <= (size_t)di.l2 * 2));  // measured cross-over with the pipeline: ~2 x L2
+                      (tn.path == 2 || (tn.path == 0 && W * cb >= 32 && footprint_bytes <= (size_t)di.l2 * 6 / 10));
   const bool warp = base_op && !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
   const int family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
   stream_kernel_t k = nullptr;
@@ -437,8 +439,12 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
     stream_kernel_t kb = su3tab::cshift_bulk_kernel(d.prec, d.W);
     if (!kb) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
     const int cbb = 2 * d.prec, rbytes = 9 * d.W * cbb;
-    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 3;           // as su3_copy
-    int tm = tn.tile_mats > 0 ? tn.tile_mats : 18432 / (9 * cbb);      // 18 KB tiles
+    // as su3_copy: 3 one-warp CTAs per SM with 18 KB tiles -- unless the shift crosses virtual nodes (W > 1 and the
+    // dimension is split): the lane rotation is done by the CTA's one warp between load and store, so twice as many CTAs
+    // with 9 KB tiles keep the TMA engine busy meanwhile (measured at 48^4 fp64 W=4, dims 2/3: 0.95 -> 0.995 x copy)
+    const bool rotates = d.W > 1 && p.simd_d > 1;
+    const int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (rotates ? 6 : 3);
+    int tm = tn.tile_mats > 0 ? tn.tile_mats : (rotates ? 9216 : 18432) / (9 * cbb);
     if (tm < d.W) tm = d.W;
     tm = tm / d.W * d.W;
     while (tm > 2 * d.W && (z->nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas && (tm / 2) % d.W == 0 && ((tm / 2 / d.W) * rbytes) % 16 == 0) tm >>= 1;
@@ -798,41 +804,41 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   const int cb = 2 * z->d.prec;
   expr_kernel_t k = su3tab::expr_kernel(z->d.prec, W_eff);
   if (!k) return fail(SU3_ERR_INVALID, "no expression kernel for W %d", W_eff);
-  // Every warp is a self-contained pipeline with a private ring of `sw` stages of 32 matrices per operand.  Long programs are latency-bound per tile, so the launch maximises resident warps per SM
-  // under the shared-memory budget (ring depth 2, 3 if there is room for >= 8 warps anyway), at most 16.
-  // matrices per stage and operand: 32 (one per lane); fp32 programs with <= 3 operands take 64 (4608-byte slots as in
-  // fp64: measured +4..13 % there, -20 % with 4 operands, where shared memory then holds too few warps)
+  // Every CTA (96 threads: three threads per matrix, su3_kernels.cuh) is a self-contained pipeline with a private ring of
+  // `sw` stages of `mps` matrices per operand.  Interpreted programs are latency-bound per tile, so the launch maximises
+  // resident CTAs per SM under the shared-memory budget (ring depth 3 if there is room for >= 4 CTAs anyway, else 2).
+  // matrices per stage and operand: 32 (one per lane and row warp); fp32 programs with <= 3 operands take 64 (4608-byte
+  // slots as in fp64)
   const int mps = (z->d.prec == SU3_F32 && n_operands <= 3 && tn.tile_mats != 32) ? 64 : 32;
   const size_t slot = (size_t)mps * 9 * cb;
   const size_t stage_bytes = (size_t)n_operands * slot;
-  const size_t sm_bytes = (size_t)di.smem_optin - 4096;  // what one SM can give to its resident CTAs, minus slack
-  int sw = tn.stages > 0 ? tn.stages : 3;
-  int warps = (int)(sm_bytes / (sw * stage_bytes + (pr.ntemp + 1) * slot + 64));   // + 1: the warp's result slot
-  if (tn.stages == 0 && warps < 8) {
-    sw = 2;
-    warps = (int)(sm_bytes / (sw * stage_bytes + (pr.ntemp + 1) * slot + 64));
-  }
-  const int reg_cap = z->d.prec == SU3_F64 ? 12 : 16;  // warps/SM the kernel's registers allow in whole CTAs of NCW warps
-  if (warps > reg_cap) warps = reg_cap;
-  if (warps < 1 || sw < 2) return fail(SU3_ERR_INVALID, "expression needs more shared memory than the device has (%d operands, %d temporaries)",
-                                       n_operands, pr.ntemp);
-  int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (warps + NCW - 1) / NCW;
-  int ncw = warps / ctas;
-  if (ncw > NCW) ncw = NCW;
-  if (ncw < 1) { ncw = 1; ctas = warps; }
-  const int stages = sw;
-  const size_t smem = (size_t)ncw * sw * stage_bytes + (size_t)ncw * (pr.ntemp + 1) * slot + (size_t)ncw * sw * sizeof(uint64_t) + 16;
-  const int tm = mps;
+  int xchg = 0;  // a product whose RIGHT factor is the accumulator: one more slot to make it whole
+  for (int i = 0; i < pr.nins; i++)
+    if (pr.ins[i].op == su3::EX_MUL && pr.ins[i].b == su3::EX_SRC_ACC) xchg = 1;
+  const size_t fixed = (size_t)(pr.ntemp + xchg + 2) * slot + 128;              // temporaries, exchange slot, two result slots, barriers
+  const size_t sm_bytes = (size_t)di.smem_optin;                                // what one SM can give to its resident CTAs
+  auto ctas_for = [&](int sw_) { return (int)((sm_bytes + 1024) / (sw_ * stage_bytes + fixed + 1024)); };  // 1 KB reserved per CTA
+  // ring depth 2 and as many CTAs as fit: measured at 48^4, more resident warps beat a deeper ring for every program
+  // (`01+01*+` fp64: 4 CTAs x 3 stages 0.79, 6 x 3 0.92, 8 x 2 0.99 x copy)
+  int sw = tn.stages > 0 ? tn.stages : 2;
+  int ctas = ctas_for(sw);
+  const int reg_cap = z->d.prec == SU3_F64 ? 10 : 16;  // CTAs of 96 threads per SM that 56-62 (fp64) / 40 (fp32) registers per thread allow
+  if (ctas > reg_cap) ctas = reg_cap;
+  if (tn.ctas_per_sm > 0 && tn.ctas_per_sm < ctas) ctas = tn.ctas_per_sm;
+  if (ctas < 1 || sw < 2) return fail(SU3_ERR_INVALID, "expression needs more shared memory than the device has (%d operands, %d temporaries)",
+                                      n_operands, pr.ntemp);
+  const size_t smem = (size_t)sw * stage_bytes + fixed;
+  if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "expression needs %zu B of shared memory, device allows %d", smem, di.smem_optin);
   cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
   if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
   su3::ExprParams p;
   memset(&p, 0, sizeof p);
   p.z = z->ptr;
   for (int i = 0; i < n_operands; i++) p.ops[i] = operands[i]->ptr;
-  p.nmat = nrec; p.tile_mats = tm; p.stages = stages; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.ncw = ncw;
+  p.nmat = nrec; p.tile_mats = mps; p.stages = sw; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.xchg = xchg;
   for (int i = 0; i < pr.nins; i++) p.ins[i] = pr.ins[i];
-  const int64_t ntiles = (nrec + tm - 1) / tm, blocks_needed = (ntiles + ncw - 1) / ncw, max_grid = (int64_t)di.sms * ctas;
-  k<<<(unsigned)(blocks_needed < max_grid ? blocks_needed : max_grid), NCW * 32, smem, (cudaStream_t)cuda_stream>>>(p);
+  const int64_t ntiles = (nrec + mps - 1) / mps, max_grid = (int64_t)di.sms * ctas;
+  k<<<(unsigned)(ntiles < max_grid ? ntiles : max_grid), 96, smem, (cudaStream_t)cuda_stream>>>(p);
   e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_expr launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);

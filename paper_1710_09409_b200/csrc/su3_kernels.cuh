@@ -645,44 +645,63 @@ struct ExprParams {
   void *z;
   const void *ops[8];
   long long nmat;
-  int tile_mats, stages, nops, nins, ntemp, hint;  // stages = ring depth PER consumer warp
-  int ncw;                                          // active consumer warps (<= NCW of the kernel)
+  int tile_mats, stages, nops, nins, ntemp, hint;  // stages = ring depth of the CTA's private ring
+  int xchg;                                          // 1: the program multiplies by a computed value on the RIGHT (one more slot)
   ExprIns ins[16];
 };
 
-// Pipeline granularity: unlike su3_pipe_kernel, every consumer WARP owns whole stages (tile k of the CTA goes
-// to consumer warp w = k % ncw and to stage (k / ncw) % SW of that warp's PRIVATE ring, so every mbarrier has one
-// waiting warp that sees its phases strictly in order), so ncw tiles are evaluated concurrently per CTA without
-// any barrier between warps.  Long programs are bound by the latency of the interpreter's LDS/FMA/STS chain per
-// tile, not by throughput (measured: 3 CTAs/SM of the CTA-wide design gave 6.85 instead of 5.47 TB/s on
-// `01+01*+`, but do not fit once there are more than two operands); warp-granular stages give that concurrency
-// without spending shared memory on it.  A stage holds MPS = 32 matrices per operand (one per lane): 4608 B
-// (fp64) / 2304 B (fp32) per bulk copy.  There is no producer warp: lane 0 of every warp issues the warp's own loads.
-template <typename R, int W, int NCW>
-__global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams p) {
+// row `c` = row `a` of the left factor times the full right factor: the rows of mat33_mul, operation for operation
+// (k ascending, the same FMA chain per element), so a row-split product is bit-identical to mat33_mul
+template <typename C2>
+__device__ __forceinline__ void mat33_mul_row(const C2 (&a)[3], const C2 (&b)[9], C2 (&c)[3]) {
+#pragma unroll
+  for (int j = 0; j < 3; j++) {
+    auto re = mul_rn(a[0].x, b[j].x);
+    auto im = mul_rn(a[0].x, b[j].y);
+    re = fma_rn(-a[0].y, b[j].y, re);
+    im = fma_rn(a[0].y, b[j].x, im);
+#pragma unroll
+    for (int k = 1; k < 3; k++) {
+      re = fma_rn(a[k].x, b[3 * k + j].x, re);
+      im = fma_rn(a[k].x, b[3 * k + j].y, im);
+      re = fma_rn(-a[k].y, b[3 * k + j].y, re);
+      im = fma_rn(a[k].y, b[3 * k + j].x, im);
+    }
+    c[j].x = re;
+    c[j].y = im;
+  }
+}
+
+// Pipeline granularity and work split.  An interpreted program is bound by the latency of its LDS -> FMA chain per
+// tile, not by throughput, and the bytes a warp keeps in flight (its ring of stages) cost shared memory: with one thread
+// per matrix a 4-operand program left room for 4-5 warps per SM, one per scheduler, issuing 0.3 instructions per clock
+// (ncu, round 2) -- 0.69-0.80 x the copy ceiling.  So a CTA is ONE self-contained pipeline of 96 threads that evaluates a
+// tile of MPS = 32 matrices (64 for fp32 programs with few operands) per stage with THREE threads per matrix: warp r
+// computes row r of every intermediate.  A row of a product needs the same row of the left factor and the whole right
+// factor; operands are whole in the stage, so only a product whose RIGHT factor is a computed value (the accumulator or
+// a temporary) makes the three warps exchange rows through shared memory (two CTA barriers); element-wise
+// instructions and spills are row-local.  Same smem per pipeline as before, three times the warps, a third of the
+// registers per thread; tid 0 issues the CTA's bulk loads and stores (no producer warp), results leave through two
+// alternating result slots so that a stage is re-armed the moment the CTA has finished reading it.
+template <typename R, int W>
+__global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
   typedef typename Cplx<R>::type C2;
   constexpr int CB = (int)sizeof(C2);
   extern __shared__ __align__(128) unsigned char smem[];
-  const int MPS = p.tile_mats;  // matrices per stage and operand: 32, or 64 (two per lane) for fp32 programs with few operands
-  const int SW = p.stages, ncw = p.ncw, S = SW * ncw, NIN = p.nops;
+  const int MPS = p.tile_mats;
+  const int SW = p.stages, NIN = p.nops;
   const uint32_t slot_bytes = (uint32_t)MPS * 9u * CB;
   const uint32_t stage_bytes = NIN * slot_bytes;
-  unsigned char *temps = smem + (size_t)S * stage_bytes;  // [ncw][ntemp] slots, private to a warp
-  unsigned char *outs = temps + (size_t)ncw * p.ntemp * slot_bytes;  // [ncw] result slots: the bulk store's source
-  uint64_t *full = reinterpret_cast<uint64_t *>(outs + (size_t)ncw * slot_bytes);
-  const int tid = threadIdx.x;
+  unsigned char *temps = smem + (size_t)SW * stage_bytes;                       // [ntemp] slots
+  unsigned char *xchg = temps + (size_t)p.ntemp * slot_bytes;                   // [xchg] slot: the accumulator, made whole
+  unsigned char *outs = xchg + (size_t)p.xchg * slot_bytes;                     // [2] result slots: the bulk stores' sources
+  uint64_t *full = reinterpret_cast<uint64_t *>(outs + 2 * (size_t)slot_bytes);
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
   const long long ntiles = (p.nmat + MPS - 1) / MPS;
-  // every warp is a self-contained pipeline: lane 0 issues the bulk loads of the warp's own tiles into the
-  // warp's private ring of SW stages.  The result of a tile goes to the warp's own result slot, so a stage is
-  // re-armed as soon as the warp has finished READING it -- the refill never waits for the store.
-  const int lane = tid & 31, w = tid >> 5;
-  if (w >= ncw) return;
-  unsigned char *mytemps = temps + (size_t)w * p.ntemp * slot_bytes;
-  unsigned char *myout = outs + (size_t)w * slot_bytes;
-  const long long gw = (long long)blockIdx.x * ncw + w, GW = (long long)gridDim.x * ncw;
+  const long long gw = blockIdx.x, GW = gridDim.x;
   const long long mine = ntiles > gw ? (ntiles - gw + GW - 1) / GW : 0;  // my tiles: gw, gw + GW, ...
-  auto load = [&](long long j) {  // lane 0 only
-    const int s = w * SW + (int)(j % SW);
+  auto load = [&](long long j) {  // tid 0 only
+    const int s = (int)(j % SW);
     const long long m0 = (gw + j * GW) * MPS;
     const long long left = p.nmat - m0;
     const int nm = left < MPS ? (int)left : MPS;
@@ -698,89 +717,107 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
     for (int o = 0; o < NIN; o++)
       bulk_g2s(st + o * slot_bytes, (const unsigned char *)p.ops[o] + goff, b16, &full[s]);
   };
-  if (lane == 0) {
-    for (int q = 0; q < SW; q++) mbar_init(&full[w * SW + q], 1);
+  if (tid == 0) {
+    for (int q = 0; q < SW; q++) mbar_init(&full[q], 1);
     fence_mbar_init();
     fence_proxy_async();
     for (long long j = 0; j < mine && j < SW; j++) load(j);
   }
-  __syncwarp();
+  __syncthreads();
   for (long long j = 0; j < mine; j++) {
-    const int s = w * SW + (int)(j % SW);
+    const int s = (int)(j % SW);
     const long long m0 = (gw + j * GW) * MPS;
     const long long left = p.nmat - m0;
     const int nm = left < MPS ? (int)left : MPS;
     unsigned char *st = smem + (size_t)s * stage_bytes;
-    // the previous tile's store (issued a whole tile ago) must have finished READING the result slot
-    if (lane == 0) bulk_wait_read<0>();
-    __syncwarp();
+    unsigned char *myout = outs + (size_t)(j & 1) * slot_bytes;
     mbar_wait(&full[s], (uint32_t)((j / SW) & 1));
+    // every lane runs every iteration (the barriers below are CTA-wide); lanes past the ragged end compute on stale
+    // shared memory inside the slot and their rows are never stored
 #pragma unroll 1
-    for (int t = lane; t < nm; t += 32) {
-      const int base = (t / W) * 9 * W + (t % W);
-      C2 acc[9], a[9], b[9];
+    for (int t = lane; t < MPS; t += 32) {
+      const int base = (t / W) * 9 * W + (t % W);   // element 0 of matrix t
+      const int rbase = base + 3 * row * W;         // element (row, 0)
+      C2 acc[3], a[3], b[9];
 #pragma unroll 1
       for (int i = 0; i < p.nins; i++) {
         const ExprIns in = p.ins[i];
         if (in.spill != EX_NONE) {
-          C2 *sp = reinterpret_cast<C2 *>(mytemps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + base;
+          C2 *sp = reinterpret_cast<C2 *>(temps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + rbase;
 #pragma unroll
-          for (int e = 0; e < 9; e++) sp[e * W] = acc[e];
+          for (int e = 0; e < 3; e++) sp[e * W] = acc[e];
         }
         if (in.a == EX_SRC_ACC) {
 #pragma unroll
-          for (int e = 0; e < 9; e++) a[e] = acc[e];
+          for (int e = 0; e < 3; e++) a[e] = acc[e];
         } else {
           const C2 *sa = reinterpret_cast<const C2 *>(in.a < EX_TEMP0 ? st + in.a * slot_bytes
-                                                                     : mytemps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + base;
+                                                                     : temps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + rbase;
 #pragma unroll
-          for (int e = 0; e < 9; e++) a[e] = sa[e * W];
-        }
-        if (in.op != EX_COPY) {
-          if (in.b == EX_SRC_ACC) {
-#pragma unroll
-            for (int e = 0; e < 9; e++) b[e] = acc[e];
-          } else {
-            const C2 *sb = reinterpret_cast<const C2 *>(in.b < EX_TEMP0 ? st + in.b * slot_bytes
-                                                                       : mytemps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
-#pragma unroll
-            for (int e = 0; e < 9; e++) b[e] = sb[e * W];
-          }
+          for (int e = 0; e < 3; e++) a[e] = sa[e * W];
         }
         if (in.op == EX_MUL) {
-          mat33_mul(a, b, acc);
-        } else if (in.op == EX_ADD) {
+          if (in.b < EX_TEMP0) {
+            const C2 *sb = reinterpret_cast<const C2 *>(st + in.b * slot_bytes) + base;
 #pragma unroll
-          for (int e = 0; e < 9; e++) {
-            acc[e].x = add_rn(a[e].x, b[e].x);
-            acc[e].y = add_rn(a[e].y, b[e].y);
-          }
-        } else if (in.op == EX_SUB) {
+            for (int e = 0; e < 9; e++) b[e] = sb[e * W];
+          } else {
+            // the right factor is a computed value: its rows live in three different warps
+            const C2 *whole;
+            if (in.b == EX_SRC_ACC) {
+              C2 *xs = reinterpret_cast<C2 *>(xchg) + rbase;
 #pragma unroll
-          for (int e = 0; e < 9; e++) {
-            acc[e].x = add_rn(a[e].x, -b[e].x);
-            acc[e].y = add_rn(a[e].y, -b[e].y);
-          }
-        } else if (in.op == EX_EMUL) {
+              for (int e = 0; e < 3; e++) xs[e * W] = acc[e];
+              whole = reinterpret_cast<const C2 *>(xchg) + base;
+            } else {
+              whole = reinterpret_cast<const C2 *>(temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
+            }
+            __syncthreads();  // all three rows written
 #pragma unroll
-          for (int e = 0; e < 9; e++) {
-            acc[e].x = mul_rn(a[e].x, b[e].x);
-            acc[e].y = mul_rn(a[e].y, b[e].y);
+            for (int e = 0; e < 9; e++) b[e] = whole[e * W];
+            __syncthreads();  // all three warps have read: the slot may be written again
           }
+          mat33_mul_row(a, b, acc);
+        } else if (in.op == EX_COPY) {
+#pragma unroll
+          for (int e = 0; e < 3; e++) acc[e] = a[e];
         } else {
+          C2 bb[3];
+          if (in.b == EX_SRC_ACC) {
 #pragma unroll
-          for (int e = 0; e < 9; e++) acc[e] = a[e];
+            for (int e = 0; e < 3; e++) bb[e] = acc[e];
+          } else {
+            const C2 *sb = reinterpret_cast<const C2 *>(in.b < EX_TEMP0 ? st + in.b * slot_bytes
+                                                                       : temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + rbase;
+#pragma unroll
+            for (int e = 0; e < 3; e++) bb[e] = sb[e * W];
+          }
+#pragma unroll
+          for (int e = 0; e < 3; e++) {
+            if (in.op == EX_ADD) {
+              acc[e].x = add_rn(a[e].x, bb[e].x);
+              acc[e].y = add_rn(a[e].y, bb[e].y);
+            } else if (in.op == EX_SUB) {
+              acc[e].x = add_rn(a[e].x, -bb[e].x);
+              acc[e].y = add_rn(a[e].y, -bb[e].y);
+            } else {  // EX_EMUL
+              acc[e].x = mul_rn(a[e].x, bb[e].x);
+              acc[e].y = mul_rn(a[e].y, bb[e].y);
+            }
+          }
         }
       }
-      C2 *so = reinterpret_cast<C2 *>(myout) + base;  // the warp's own result slot
+      C2 *so = reinterpret_cast<C2 *>(myout) + rbase;
 #pragma unroll
-      for (int e = 0; e < 9; e++) so[e * W] = acc[e];
+      for (int e = 0; e < 3; e++) so[e * W] = acc[e];
     }
     fence_proxy_async();
-    __syncwarp();
-    // every lane has read what it needs from stage s (operand slots are only read): re-arm it with my tile j + SW
-    // at once -- the refill never waits for the store -- and send the result on its way
-    if (lane == 0) {
+    // store j-1 (issued a whole tile ago) has finished READING the other result slot, which tile j+1 writes
+    if (tid == 0) bulk_wait_read<0>();
+    __syncthreads();
+    // every thread has read what it needs from stage s and written its rows of the result: re-arm the stage with my
+    // tile j + SW at once -- the refill never waits for the store -- and send the result on its way
+    if (tid == 0) {
       if (j + SW < mine) load(j + SW);
       const uint32_t bytes = (uint32_t)nm * 9u * CB;
       const uint32_t b16 = bytes & ~15u;
@@ -790,7 +827,7 @@ __global__ void __launch_bounds__(NCW * 32, 2) su3_expr_kernel(const ExprParams 
       if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(myout + b16);
     }
   }
-  if (lane == 0) bulk_wait_all<0>();
+  if (tid == 0) bulk_wait_all<0>();
 }
 
 // ---------------------------------------------------------------- real scalar fields (Listing 2 of the paper)

@@ -98,12 +98,12 @@ template <typename R> stream_kernel_t pick(int op, int W, bool direct) {
 typedef void (*expr_kernel_t)(const su3::ExprParams);
 template <typename R> expr_kernel_t expr_for_w(int W) {
   switch (W) {
-    case 1: return su3::su3_expr_kernel<R, 1, NCW>;
-    case 2: return su3::su3_expr_kernel<R, 2, NCW>;
-    case 4: return su3::su3_expr_kernel<R, 4, NCW>;
-    case 8: return su3::su3_expr_kernel<R, 8, NCW>;
-    case 16: return su3::su3_expr_kernel<R, 16, NCW>;
-    case 32: return su3::su3_expr_kernel<R, 32, NCW>;
+    case 1: return su3::su3_expr_kernel<R, 1>;
+    case 2: return su3::su3_expr_kernel<R, 2>;
+    case 4: return su3::su3_expr_kernel<R, 4>;
+    case 8: return su3::su3_expr_kernel<R, 8>;
+    case 16: return su3::su3_expr_kernel<R, 16>;
+    case 32: return su3::su3_expr_kernel<R, 32>;
   }
   return nullptr;
 }
