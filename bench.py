@@ -823,6 +823,9 @@ def profile_pass(args):
             su3.su3_tune_set(path=3)
             su3.su3_cshift(z, y, 0, 1)                                                           # cp.async gather
             su3.su3_tune_set()
+            fb = su3.su3_face_bytes(x, 3, 2)                                                     # (e) faces of a slab: 2 planes
+            buf = torch.empty(fb, dtype=torch.uint8, device="cuda")
+            su3.su3_face_pack(buf, x, 3, 0, 2); su3.su3_face_unpack(z, buf, 3, L - 2, 2); su3.su3_face_copy(z, 0, x, L - 2, 3, 2)
             psi = su3.su3_vec_wrap(x.desc, w.tensor[:su3.su3_vec_bytes(x.desc)])
             yv_ = su3.su3_vec_wrap(x.desc, z.tensor[:su3.su3_vec_bytes(x.desc)])
             su3.su3_matvec(yv_, x, psi)

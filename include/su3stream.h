@@ -236,6 +236,16 @@ su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, in
 su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, int dim, int plane0, int nplanes, void *cuda_stream);
 su3_status su3_face_copy(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes, void *cuda_stream);
 
+/* Cshift along x3 on one slab of an x3-split lattice with the neighbouring slab mapped into this process (peer memory
+ * over NVLink, or simply another field on the same device): z[s] = X[s + disp*e3], X = the slab x continued by x_nbr --
+ * the NEXT rank's slab for disp > 0, the PREVIOUS rank's for disp < 0; 0 < |disp| < L[3] of the slab (disp = 0 copies x;
+ * SU3_ERR_INVALID beyond).  Identical descriptors, colour-matrix fields.  Exchange and shift are ONE kernel whenever no
+ * record mixes lanes of the two slabs (scalar layout, or simd[3] = 1): the TMA copy kernel of su3_cshift reads the runs
+ * that leave the slab from x_nbr at the same record offset.  Otherwise (x3 split over virtual nodes) two launches: the
+ * periodic shift of x, then su3_face_copy of the |disp| wrapped planes from x_nbr.  Bit-exact either way.  z and x
+ * must live on the current device; x_nbr is only read. */
+su3_status su3_cshift_slab(su3_field *z, const su3_field *x, const su3_field *x_nbr, int disp, void *cuda_stream);
+
 /* End-to-end z = x*y with HOST buffers: x_host, y_host (inputs) and z_host (output) are host
  * arrays of su3_field_bytes bytes in the layout of the (identical) descriptors of the three
  * DEVICE staging fields zd, xd, yd.  Enqueues, on cuda_stream, chunked host->device copies

@@ -18,7 +18,7 @@ EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normali
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
            "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_expr_plan", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release",
-           "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy"]
+           "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy", "su3_cshift_slab"]
 
 
 class su3_desc(ctypes.Structure):
@@ -83,6 +83,7 @@ def _load():
         "su3_face_pack": (i32, [vp, sz, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_face_unpack": (i32, [vp, vp, sz, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_face_copy": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
+        "su3_cshift_slab": (i32, [vp, vp, vp, ctypes.c_int, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -364,3 +365,8 @@ def su3_face_unpack(z, buf, dim, plane0, nplanes, stream=None):
 
 def su3_face_copy(z, z_plane0, x, x_plane0, dim, nplanes, stream=None):
     _ck(lib.su3_face_copy(z.handle, int(z_plane0), x.handle, int(x_plane0), int(dim), int(nplanes), _stream(stream)))
+
+
+def su3_cshift_slab(z, x, x_nbr, disp, stream=None):
+    """Cshift along x3 of slab x continued by the neighbouring slab x_nbr (next rank's for disp > 0, previous for disp < 0)"""
+    _ck(lib.su3_cshift_slab(z.handle, x.handle, x_nbr.handle, int(disp), _stream(stream)))

@@ -401,7 +401,11 @@ const char *const kMenuPostfix[su3::OP_COUNT] = {"01*", "01*2*", "01*2+", "01+",
                                                  "01+2+", "01+2+3+", "01-", "01*", "01+01*+", "0"};
 
 // ---------------------------------------------------------------- Cshift / shifted product
-su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream) {
+// alt != NULL (su3_cshift_slab, op = SH_COPY only): the runs that leave the slab are read from the neighbouring slab
+// `alt` by the bulk-copy kernel; returns SU3_ERR_INVALID + *fused = false when that kernel does not apply (the caller
+// then shifts locally and copies the face).
+su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *stream,
+                        const su3_field *alt = nullptr, bool *fused = nullptr) {
   if (!z || !y || (op == su3::SH_MUL && !x)) return fail(SU3_ERR_NULL, "field handle is NULL");
   if (!same_desc(z->d, y->d) || (x && !same_desc(z->d, x->d))) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
   if (z->ncomp != 9 || y->ncomp != 9 || (x && x->ncomp != 9)) return fail(SU3_ERR_MISMATCH, "colour-matrix fields expected");
@@ -435,7 +439,13 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   // record is even: P even and an even record count.
   const int64_t nrec_all = z->nmat / d.W;
   const bool bulk72_ok = !(d.prec == SU3_F32 && d.W == 1) || (P % 2 == 0 && nrec_all % 2 == 0);
-  if (op == su3::SH_COPY && (tn.path == 0 || tn.path == 1) && bulk72_ok && z->nmat < 0x7fffffffLL) {
+  const bool bulk_applies = op == su3::SH_COPY && (tn.path == 0 || tn.path == 1) && bulk72_ok && z->nmat < 0x7fffffffLL;
+  if (alt) {
+    const bool ok = bulk_applies && !(d.W > 1 && p.simd_d > 1) && p.disp != 0;   // lanes of one record would come from two slabs
+    if (fused) *fused = ok;
+    if (!ok) return SU3_ERR_INVALID;
+  }
+  if (bulk_applies) {
     stream_kernel_t kb = su3tab::cshift_bulk_kernel(d.prec, d.W);
     if (!kb) return fail(SU3_ERR_INVALID, "no shift kernel for W %d", d.W);
     const int cbb = 2 * d.prec, rbytes = 9 * d.W * cbb;
@@ -461,6 +471,10 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
     memset(&sp, 0, sizeof sp);
     sp.z = z->ptr; sp.x = y->ptr; sp.nmat = z->nmat; sp.tile_mats = tm; sp.stages = stages;
     sp.sh.P = P; sp.sh.rd = p.rd; sp.sh.dmod = p.disp % p.rd; sp.sh.qrot = p.disp / p.rd; sp.sh.simd_d = p.simd_d; sp.sh.lstride = p.lstride;
+    if (alt) {
+      sp.sh.alt = alt->ptr;
+      sp.sh.alt_carry = disp > 0 ? 1 : 0;   // disp > 0: the wrapping (carry) runs belong to the next slab; disp < 0: the others to the previous one
+    }
     const int64_t ntiles_b = (z->nmat + tm - 1) / tm, cap_b = (int64_t)di.sms * ctas;
     kb<<<(unsigned)(ntiles_b < cap_b ? ntiles_b : cap_b), 32, smem_b, (cudaStream_t)stream>>>(sp);
     eb = cudaGetLastError();
@@ -474,7 +488,7 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   const int64_t tile_recs = (9216 / (9 * 2 * d.prec)) / d.W;
   const bool pipe_pays = d.prec == SU3_F64 && (int64_t)p.rd * P >= tile_recs;
   if (op == su3::SH_MUL && (tn.path == 1 || (tn.path == 0 && pipe_pays)) && !odd72 && z->nmat < 0x7fffffffLL) {  // record indices fit 31 bits (P <= records)
-    su3::ShiftInfo sh;
+    su3::ShiftInfo sh = {};
     sh.P = P; sh.rd = p.rd; sh.dmod = p.disp % p.rd; sh.qrot = p.disp / p.rd; sh.simd_d = p.simd_d; sh.lstride = p.lstride;
     sh.phase = (d.prec == SU3_F32 && d.W == 1 && ((int64_t)sh.dmod * P) % 2) ? 8 : 0;
     const void *in[4] = {op == su3::SH_MUL ? x->ptr : y->ptr, op == su3::SH_MUL ? y->ptr : nullptr, nullptr, nullptr};
@@ -809,7 +823,7 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   // resident CTAs per SM under the shared-memory budget (ring depth 3 if there is room for >= 4 CTAs anyway, else 2).
   // matrices per stage and operand: 32 (one per lane and row warp); fp32 programs with <= 3 operands take 64 (4608-byte
   // slots as in fp64)
-  const int mps = (z->d.prec == SU3_F32 && n_operands <= 3 && tn.tile_mats != 32) ? 64 : 32;
+  const int mps = tn.tile_mats > 0 ? tn.tile_mats : ((z->d.prec == SU3_F32 && n_operands <= 3) ? 64 : 32);
   const size_t slot = (size_t)mps * 9 * cb;
   const size_t stage_bytes = (size_t)n_operands * slot;
   int xchg = 0;  // a product whose RIGHT factor is the accumulator: one more slot to make it whole
@@ -850,6 +864,26 @@ su3_status su3_cshift(su3_field *z, const su3_field *x, int dim, int disp, void 
 }
 su3_status su3_mul_shift(su3_field *z, const su3_field *x, const su3_field *y, int dim, int disp, void *cuda_stream) {
   return launch_shift(su3::SH_MUL, z, x, y, dim, disp, cuda_stream);
+}
+
+static su3_status launch_face_copy(const su3_field *geo, void *dst, bool dpacked, int dplane0, const void *src, bool spacked,
+                                   int splane0, int dim, int nplanes, void *stream);
+
+su3_status su3_cshift_slab(su3_field *z, const su3_field *x, const su3_field *x_nbr, int disp, void *cuda_stream) {
+  if (!z || !x || !x_nbr) return fail(SU3_ERR_NULL, "field handle is NULL");
+  if (!same_desc(z->d, x->d) || !same_desc(z->d, x_nbr->d)) return fail(SU3_ERR_MISMATCH, "operand descriptors differ");
+  if (z->ncomp != 9 || x->ncomp != 9 || x_nbr->ncomp != 9) return fail(SU3_ERR_MISMATCH, "colour-matrix fields expected");
+  if (z->ptr == x->ptr || z->ptr == x_nbr->ptr) return fail(SU3_ERR_MISMATCH, "the output must not be one of the shifted slabs");
+  const int l3 = z->d.L[3];
+  if (disp <= -l3 || disp >= l3) return fail(SU3_ERR_INVALID, "su3_cshift_slab: |disp| = %d must be below the slab's %d planes", disp < 0 ? -disp : disp, l3);
+  if (disp == 0) return su3_copy(z, x, cuda_stream);
+  bool fused = false;
+  su3_status st = launch_shift(su3::SH_COPY, z, nullptr, x, 3, disp, cuda_stream, x_nbr, &fused);   // x_nbr may be peer memory: not device-checked
+  if (fused || st != SU3_ERR_INVALID) return st;
+  // two launches: the periodic shift of the slab, then the planes that wrapped, straight from the neighbouring slab
+  if ((st = launch_shift(su3::SH_COPY, z, nullptr, x, 3, disp, cuda_stream)) != SU3_OK) return st;
+  const int n = disp > 0 ? disp : -disp;
+  return launch_face_copy(z, z->ptr, false, disp > 0 ? l3 - n : 0, x_nbr->ptr, false, disp > 0 ? 0 : l3 - n, 3, n, cuda_stream);
 }
 
 su3_status su3_vec_index(const su3_desc *desc, int64_t site, int mu, int i, int reim, int64_t *off) {
@@ -1091,7 +1125,9 @@ static su3_status launch_face_copy(const su3_field *geo, void *dst, bool dpacked
   }
   p.ncplx = n * geo->d.n_lorentz * geo->ncomp;
   if (p.ncplx == 0) return SU3_OK;
-  su3tab::launch_face(geo->d.prec, geo->ncomp, flat_grid((size_t)p.ncplx, 1024, 8), p, (cudaStream_t)stream);
+  // 32-bit indices when every complex index of the field (and a grid stride beyond the face) fits 31 bits
+  const bool idx32 = (geo->nmat + 1) * geo->ncomp * geo->d.W < 0x3fffffffLL && p.ncplx < 0x3fffffffLL;
+  su3tab::launch_face(geo->d.prec, geo->ncomp, idx32, flat_grid((size_t)p.ncplx, 1024, 8), p, (cudaStream_t)stream);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("su3_face launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);

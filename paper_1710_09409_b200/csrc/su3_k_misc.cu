@@ -20,11 +20,15 @@ template <typename C2, int NC, int N> bool convert_tma_w(int W, const su3::Conve
   *err = "unsupported W";
   return false;
 }
-void launch_face(int prec, int nc, unsigned grid, const su3::FaceParams &p, cudaStream_t s) {
-  if (prec == 8 && nc == 9) su3::su3_face_kernel<double2, 9><<<grid, 256, 0, s>>>(p);
-  else if (prec == 8) su3::su3_face_kernel<double2, 3><<<grid, 256, 0, s>>>(p);
-  else if (nc == 9) su3::su3_face_kernel<float2, 9><<<grid, 256, 0, s>>>(p);
-  else su3::su3_face_kernel<float2, 3><<<grid, 256, 0, s>>>(p);
+template <typename IT> void launch_face_it(int prec, int nc, unsigned grid, const su3::FaceParams &p, cudaStream_t s) {
+  if (prec == 8 && nc == 9) su3::su3_face_kernel<double2, 9, IT><<<grid, 256, 0, s>>>(p);
+  else if (prec == 8) su3::su3_face_kernel<double2, 3, IT><<<grid, 256, 0, s>>>(p);
+  else if (nc == 9) su3::su3_face_kernel<float2, 9, IT><<<grid, 256, 0, s>>>(p);
+  else su3::su3_face_kernel<float2, 3, IT><<<grid, 256, 0, s>>>(p);
+}
+void launch_face(int prec, int nc, bool idx32, unsigned grid, const su3::FaceParams &p, cudaStream_t s) {
+  if (idx32) launch_face_it<int>(prec, nc, grid, p, s);
+  else launch_face_it<long long>(prec, nc, grid, p, s);
 }
 
 int convert_tma_tile(int prec) { return prec == 8 ? 1152 : 2304; }

@@ -216,6 +216,11 @@ struct ShiftInfo {
   int simd_d, lstride;  // simd[dim], prod_{k<dim} simd[k]
   int phase;       // fp32 scalar layout only: byte offset (0 or 8) of the shifted slot that makes source and destination
                    // of every run agree mod 16 (records are 72 B; bulk copies need 16-byte alignment)
+  // su3_cshift_bulk_kernel on a slab of a multi-GPU lattice (su3_cshift_slab): the runs that leave the slab -- the
+  // carry runs for disp > 0 (alt_carry = 1), the others for disp < 0 (alt_carry = 0) -- are read at the same record
+  // offset from the NEIGHBOURING rank's slab `alt` (peer memory over NVLink, or local); NULL: periodic on the slab
+  const void *alt;
+  int alt_carry;
 };
 
 struct StreamParams {
@@ -499,6 +504,7 @@ __global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams 
   const int nrec = (int)(p.nmat / W);
   const int ntiles = (nrec + TR - 1) / TR;
   const unsigned char *gy = (const unsigned char *)p.x;
+  const unsigned char *galt = (const unsigned char *)p.sh.alt;
   unsigned char *gz = (unsigned char *)p.z;
   const int mine = ntiles > (int)blockIdx.x ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
   // runs of tile [R0, R1): fn(first record, one past the last, carry)
@@ -523,7 +529,8 @@ __global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams 
     mbar_arrive_expect_tx(&full[s], (uint32_t)(R1 - R0) * rb);
     for_runs(R0, R1, [&](int Ra, int Rb, bool carry) {
       const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
-      bulk_g2s(buf + (size_t)(Ra - R0) * rb, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
+      const unsigned char *base = (galt && (int)carry == p.sh.alt_carry) ? galt : gy;
+      bulk_g2s(buf + (size_t)(Ra - R0) * rb, base + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
     });
   };
   if (lane == 0) {
@@ -1669,39 +1676,57 @@ struct FaceParams {
   long long ncplx;   // complex numbers to move = prod(F) * nl * NC
 };
 
-template <int NC>
-__device__ __forceinline__ long long face_index(const FaceSide &g, int dim, const int (&c)[4], int mu, int e, long long packed_idx) {
+template <int NC, typename IT>
+__device__ __forceinline__ IT face_index(const FaceSide &g, int dim, const int (&c)[4], int mu, int e, IT packed_idx) {
   if (g.packed) return packed_idx;
-  long long o = 0, ostride = 1, site = 0, sstride = 1;
+  if (g.W == 1) {  // scalar layout: no virtual-node map
+    IT site = 0, sstride = 1;
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+      site += (c[k] + (k == dim ? g.plane0 : 0)) * sstride;
+      sstride *= g.L[k];
+    }
+    return (site * g.nl + mu) * NC + e;
+  }
+  IT o = 0, ostride = 1;
   int l = 0, lstride = 1;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
     const int x = c[k] + (k == dim ? g.plane0 : 0);
-    const int r = g.L[k] / g.simd[k];
-    site += x * sstride;  sstride *= g.L[k];
-    o += (x % r) * ostride;  ostride *= r;
-    l += (x / r) * lstride;  lstride *= g.simd[k];
+    if (g.simd[k] > 1) {  // only split dimensions cost a division
+      const int r = g.L[k] / g.simd[k];
+      const int ic = x / r;
+      o += (x - ic * r) * ostride;  ostride *= r;
+      l += ic * lstride;  lstride *= g.simd[k];
+    } else {
+      o += x * ostride;  ostride *= g.L[k];
+    }
   }
-  if (g.W == 1) return (site * g.nl + mu) * NC + e;
   return ((o * g.nl + mu) * NC + e) * g.W + l;
 }
 
-template <typename C2, int NC>
+// One thread per complex number.  IT = int whenever every complex index of both sides fits 31 bits (the host checks):
+// the kernel spends its time on integer divisions, not on memory (a 4-way unrolled version with more loads in flight
+// was 2.6 x SLOWER), so 64-bit ones are avoided and unsplit dimensions skip theirs.
+template <typename C2, int NC, typename IT>
 __global__ void __launch_bounds__(256) su3_face_kernel(const FaceParams p) {
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.ncplx; i += stride) {
+  const IT stride = (IT)gridDim.x * blockDim.x, n = (IT)p.ncplx;
+  const int nlsh = p.d.nl == 4 ? 2 : 0;  // n_lorentz is 1 or 4
+  for (IT i = (IT)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     const int e = (int)(i % NC);
-    long long b = i / NC;
-    const int mu = (int)(b % p.d.nl);
-    b /= p.d.nl;
+    IT b = i / NC;
+    const int mu = (int)(b & (p.d.nl - 1));
+    b >>= nlsh;
     int c[4];
 #pragma unroll
-    for (int k = 0; k < 4; k++) {
-      c[k] = (int)(b % p.F[k]);
-      b /= p.F[k];
+    for (int k = 0; k < 3; k++) {
+      const IT q = b / p.F[k];
+      c[k] = (int)(b - q * p.F[k]);
+      b = q;
     }
-    const long long si = face_index<NC>(p.s, p.dim, c, mu, e, i);
-    const long long di = face_index<NC>(p.d, p.dim, c, mu, e, i);
+    c[3] = (int)b;
+    const IT si = face_index<NC, IT>(p.s, p.dim, c, mu, e, i);
+    const IT di = face_index<NC, IT>(p.d, p.dim, c, mu, e, i);
     reinterpret_cast<C2 *>(p.dst)[di] = reinterpret_cast<const C2 *>(p.src)[si];
   }
 }

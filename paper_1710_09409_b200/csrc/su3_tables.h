@@ -171,6 +171,6 @@ bool launch_convert(int prec, int nc, int W, bool staged, const su3::ConvertPara
 int convert_tma_tile(int prec);
 bool launch_convert_tma(int prec, int nc, int W, const su3::ConvertParams &p, cudaStream_t s, const char **err);
 // face of a slab: pack / unpack / field-to-field copy of planes (nc = 9 or 3)
-void launch_face(int prec, int nc, unsigned grid, const su3::FaceParams &p, cudaStream_t s);
+void launch_face(int prec, int nc, bool idx32, unsigned grid, const su3::FaceParams &p, cudaStream_t s);
 
 }  // namespace su3tab

@@ -195,3 +195,47 @@ class SlabShift:
 
     def mul_shift(self, z, x, y, dim, disp):
         self.finish_mul_shift(z, x, self.start(y, dim, disp))
+
+
+class PeerShift:
+    """The same shifts when the neighbouring slabs are MAPPED into this process (peer memory over NVLink: CUDA IPC or
+    symmetric memory give a device pointer that su3_field_wrap takes like any other; in the 1-GPU tests the
+    "neighbours" are simply other fields on the same device).  No staging buffer and no collective call: the kernels
+    read the neighbour's planes themselves.  |disp| must be below the slab's extent; both neighbours are passed and
+    the sign of disp picks one."""
+
+    def __init__(self):
+        import torch
+        import paper_1710_09409_b200 as su3
+        self.su3, self.torch = su3, torch
+        self._buf = {}
+
+    def cshift(self, z, y, y_next, y_prev, disp):
+        """z[s] = Y[s + disp*e3], one kernel (su3_cshift_slab) unless x3 is split over virtual nodes (then two)."""
+        self.su3.su3_cshift_slab(z, y, y_next if disp > 0 else y_prev, disp)
+
+    def mul_shift(self, z, x, y, y_next, y_prev, disp):
+        """z[s] = x[s] . Y[s + disp*e3]: the periodic product on the slab, then the |disp| wrapped planes again as
+        su3_mul on packed faces -- x's planes times the neighbour's planes, packed straight out of its memory."""
+        su3 = self.su3
+        su3.su3_mul_shift(z, x, y, shard.SLAB_DIM, disp)
+        n = abs(disp)
+        if n == 0:
+            return
+        l3 = x.desc.L[shard.SLAB_DIM]
+        if n >= l3:
+            raise ValueError("|disp| = %d must be below the slab's %d planes" % (n, l3))
+        nbr = y_next if disp > 0 else y_prev
+        dst0, src0 = (l3 - n, 0) if disp > 0 else (0, l3 - n)
+        nb = su3.su3_face_bytes(x, shard.SLAB_DIM, n)
+        key = (nb, str(x.tensor.device))
+        if key not in self._buf:
+            self._buf[key] = [self.torch.empty(nb, dtype=self.torch.uint8, device=x.tensor.device) for _ in range(3)]
+        xb, hb, zb = self._buf[key]
+        su3.su3_face_pack(xb, x, shard.SLAB_DIM, dst0, n)
+        su3.su3_face_pack(hb, nbr, shard.SLAB_DIM, src0, n)
+        L = tuple(x.desc.L)
+        d = su3.make_desc((L[0], L[1], L[2], n), n_lorentz=x.desc.n_lorentz, prec=x.desc.prec)
+        fz, fx, fh = (su3.su3_field_wrap(d, t) for t in (zb, xb, hb))
+        su3.su3_mul(fz, fx, fh)
+        su3.su3_face_unpack(z, zb, shard.SLAB_DIM, dst0, n)

@@ -132,3 +132,44 @@ def test_sharded_shifts_equal_the_oracle_on_the_global_lattice(prec, world, gL, 
             su3.su3_mul(t, xs[r], zc[r])
             torch.cuda.synchronize()
             assert torch.equal(t.tensor, zm[r].tensor), (dim, disp, r)
+
+
+@pytest.mark.parametrize("prec", [su3.SU3_F64, su3.SU3_F32])
+@pytest.mark.parametrize("world,gL,nl,W,simd", [(2, (8, 4, 4, 12), 1, 1, None), (3, (4, 4, 4, 12), 4, 1, None), (2, (8, 4, 4, 12), 1, 4, None),
+                                                (2, (8, 4, 4, 8), 1, 4, (2, 2, 1, 1)), (4, (4, 2, 4, 16), 1, 8, (2, 2, 2, 1)),
+                                                (2, (16, 8, 8, 16), 1, 1, None), (2, (6, 2, 2, 6), 1, 1, None)])
+def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
+    """su3_cshift_slab / halo.PeerShift: the neighbour's slab is read by the shift kernel itself (here: another field on the
+    same device stands for peer memory).  Fused (scalar layout, simd[3] = 1) and two-launch (x3 split) variants."""
+    g, gx = _global(gL, nl, prec, su3gen.FIELD_X)
+    _, gy = _global(gL, nl, prec, su3gen.FIELD_Y)
+    lL = (gL[0], gL[1], gL[2], gL[3] // world)
+    d = su3.make_desc(lL, n_lorentz=nl, prec=prec, layout=VEC if W > 1 else su3.SU3_SCALAR, W=W, simd=simd)
+
+    def slabs(gflat):
+        out = []
+        for r in range(world):
+            m0, m1 = shard.matrix_range(gL, nl, r, world)
+            out.append(upload(d, oracle.convert(geom_of(d), geom_of(scalar_desc(d)), gflat[m0 * 18:m1 * 18].copy())))
+        return out
+    xs, ys = slabs(gx), slabs(gy)
+    ps = halo.PeerShift()
+    l3 = lL[3]
+    for disp in (1, -1, 2, -(l3 - 1), l3 - 1, 0):
+        zc = [su3.alloc_field(d) for _ in range(world)]
+        zm = [su3.alloc_field(d) for _ in range(world)]
+        for r in range(world):
+            nxt, prv = ys[(r + 1) % world], ys[(r - 1) % world]
+            n0 = su3.su3_launch_count()
+            ps.cshift(zc[r], ys[r], nxt, prv, disp)
+            fused = W == 1 or su3.su3_desc_normalize(d).simd[3] == 1
+            if disp != 0:
+                assert su3.su3_launch_count() - n0 == (1 if fused else 2)
+            ps.mul_shift(zm[r], xs[r], ys[r], nxt, prv, disp)
+        assert np.array_equal(_gather(d, zc), oracle.cshift(g, gy, 3, disp)), disp
+        e, _ = rel_err(_gather(d, zm), oracle.mul_shift(g, gx, gy, 3, disp), 1)
+        assert e <= TOL[prec], (disp, e)
+    with pytest.raises(su3.Su3Error):
+        su3.su3_cshift_slab(zc[0], ys[0], ys[1], l3)
+    with pytest.raises(su3.Su3Error):
+        su3.su3_cshift_slab(ys[0], ys[0], ys[1], 1)
