@@ -61,6 +61,11 @@ def parse_args():
     ap.add_argument("--profile-pass", action="store_true",
                     help="launch every kernel variant of the library once at 48^4 (no timing): the command ncu wraps "
                          "for profiles/*_all_kernels.md")
+    ap.add_argument("--profile-knee", action="store_true",
+                    help="three back-to-back z = x*y calls per configuration at the knee of the volume sweep (24^4 fp64, 28^4 and "
+                         "32^4 fp32, scalar and vector; footprints 0.6-2 x L2), no timing: the command ncu wraps with "
+                         "--cache-control none for profiles/*_knee.md (the third call of each triple sees the L2 state the "
+                         "warm protocol of the sweep sees)")
     return ap.parse_args()
 
 
@@ -846,6 +851,24 @@ def profile_pass(args):
     print(json.dumps({"profile_pass": True, "L": L, "launches": su3.su3_launch_count() - n0}), flush=True)
 
 
+def profile_knee(args):
+    import torch
+
+    import paper_1710_09409_b200 as su3
+    torch.cuda.set_device(0)
+    n0 = su3.su3_launch_count()
+    for L, prec, W in ((24, su3.SU3_F64, W64), (28, su3.SU3_F32, W32), (32, su3.SU3_F32, W32)):
+        dt = torch.float64 if prec == su3.SU3_F64 else torch.float32
+        for layout in (su3.SU3_SCALAR, su3.SU3_VECTOR):
+            d = su3.make_desc(L, prec=prec, layout=layout, W=W if layout == su3.SU3_VECTOR else 1)
+            x, y, z = (su3.alloc_field(d) for _ in range(3))
+            x.tensor.view(dt).normal_(); y.tensor.view(dt).normal_()
+            for _ in range(3):
+                su3.su3_mul(z, x, y)
+            torch.cuda.synchronize()
+    print(json.dumps({"profile_knee": True, "launches": su3.su3_launch_count() - n0}), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -859,9 +882,9 @@ def main():
     if args.impl == "reference":
         run_reference(args, rank)
         return
-    if args.profile_pass:
+    if args.profile_pass or args.profile_knee:
         if rank == 0:
-            profile_pass(args)
+            (profile_pass if args.profile_pass else profile_knee)(args)
         return
     if world != args.gpus:
         log("note: --gpus %d but WORLD_SIZE=%d; using WORLD_SIZE (launch N>1 with torch.distributed.run)" % (args.gpus, world))

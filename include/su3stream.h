@@ -88,7 +88,8 @@ typedef struct su3_field su3_field; /* opaque: validated descriptor + device poi
  *   pipeline (su3_mul/mul3/mul_add/add, su3_matvec): tile_mats, stages = ring depth, ctas_per_sm, l2_hint, path
  *   su3_copy: tile = tile_mats x matrix bytes, stages, ctas_per_sm, l2_hint; path = 2 selects the plain LDG copy
  *   su3_expr: programs on the ahead-of-time menu run on the pipeline (knobs as above); path = 3 forces the interpreter,
- *             whose knobs are stages = ring depth per CTA (2..) and ctas_per_sm (96-thread CTAs per SM); its tile is 32 matrices
+ *             whose knobs are tile_mats = matrices per stage and operand (default 32; 64 for fp32 programs with <= 3
+ *             operands), stages = ring depth per CTA (default 2) and ctas_per_sm (an upper limit on its 96-thread CTAs per SM)
  *   su3_cshift / su3_mul_shift: default = the pipeline with a shifted operand (knobs as above); path = 2 the register
  *             kernels, path = 3 the cp.async-gather Cshift; for those ctas_per_sm = blocks per SM of the grid
  *   su3_convert: default = TMA bulk copies on both sides;

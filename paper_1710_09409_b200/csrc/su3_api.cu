@@ -239,7 +239,11 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
     const int64_t max_grid = (int64_t)di.sms * ctas;
     int stages = tn.stages;
     if (stages == 0) {
-      stages = 3;
+      // ring depth 3 at HBM-bound sizes (deeper rings open more DRAM pages at once and measured 1-3 % slower from 40^4
+      // fp32 / 36^4 fp64 on); up to 3 x L2 a good part of the loads hits L2, latency rather than DRAM limits a 20-70 us
+      // launch, and more bytes in flight pay: depth 4 measured +4..12 % at 20^4-28^4 fp64 and 24^4-36^4 fp32 (ncu at
+      // 24^4 with depth 3, warm: DRAM 44 % busy, profiles/r02_knee.md)
+      stages = footprint_bytes <= (size_t)di.l2 * 3 ? 4 : 3;
       while (stages > 2 && stages * stage_bytes + 256 > budget) stages--;
     }
     if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);

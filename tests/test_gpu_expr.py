@@ -128,6 +128,11 @@ def test_expr_random_programs_fuzz(prec, layout, W):
     fs = [upload(desc, h) for h in hosts]
     z = su3.alloc_field(desc)
     Wn = su3.su3_desc_normalize(desc).W
+    abs_hosts = []                                               # (|a|, 0) for every complex number a, in fp64
+    for h in hosts:
+        a = np.zeros(h.size, dtype=np.float64).reshape(-1, 2)
+        a[:, 0] = np.hypot(*h.astype(np.float64).reshape(-1, 2).T)
+        abs_hosts.append(a.reshape(-1))
     seen_temps = 0
     for _ in range(60):
         n_ops = int(rng.integers(1, 7))
@@ -138,9 +143,16 @@ def test_expr_random_programs_fuzz(prec, layout, W):
         z.tensor.fill_(0xFF)
         su3.su3_expr(z, prog, fs[:n_ops])
         got, ref = download(z), oracle.expr(g, prog, *hosts[:n_ops])
-        # relative to the largest entry of the result field: x - x style cancellations make per-matrix norms meaningless
-        scale = max(np.abs(ref).max(), 1.0)
-        assert np.isfinite(got).all() and np.abs(got - ref).max() / scale <= 50 * TOL[prec], prog
+        # x - x style cancellations make per-matrix relative norms meaningless, so the bar is the componentwise forward
+        # error bound of the expression (Higham, Accuracy and Stability, ch. 3): |fl(E) - E| <= gamma_k * E_abs, where E_abs
+        # is the SAME program evaluated on the moduli |a_ij| with '-' replaced by '+' (no cancellation left) and
+        # k counts the roundings on the longest path: <= 8 per complex product-and-sum of three terms (gamma_3 for the sum,
+        # gamma_2 * sqrt(2) for each complex product, FMA or not: about 4.8 u per '*') and 1 per '+'/'-'; K = 8 per operator.
+        u = 2.0 ** -53 if prec == F64 else 2.0 ** -24
+        K = 8 * (prog.count("*") + prog.count("+") + prog.count("-")) + 4     # + 4: the oracle's own fp64 roundings in fp32 runs
+        e_abs = oracle.expr(g, prog.replace("-", "+"), *abs_hosts[:n_ops]).reshape(-1, 2)[:, 0]
+        diff = np.hypot(*(got.astype(np.float64) - ref).reshape(-1, 2).T)
+        assert np.isfinite(got).all() and (diff <= K * u * e_abs).all(), (prog, float((diff / (u * e_abs)).max()), K)
         seen_temps += prog.count("*") > 2
     assert seen_temps > 10
 

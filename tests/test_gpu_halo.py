@@ -137,7 +137,7 @@ def test_sharded_shifts_equal_the_oracle_on_the_global_lattice(prec, world, gL, 
 @pytest.mark.parametrize("prec", [su3.SU3_F64, su3.SU3_F32])
 @pytest.mark.parametrize("world,gL,nl,W,simd", [(2, (8, 4, 4, 12), 1, 1, None), (3, (4, 4, 4, 12), 4, 1, None), (2, (8, 4, 4, 12), 1, 4, None),
                                                 (2, (8, 4, 4, 8), 1, 4, (2, 2, 1, 1)), (4, (4, 2, 4, 16), 1, 8, (2, 2, 2, 1)),
-                                                (2, (16, 8, 8, 16), 1, 1, None), (2, (6, 2, 2, 6), 1, 1, None)])
+                                                (2, (16, 8, 8, 16), 1, 1, None), (2, (6, 2, 2, 6), 1, 1, None), (2, (3, 3, 3, 4), 1, 1, None)])
 def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
     """su3_cshift_slab / halo.PeerShift: the neighbour's slab is read by the shift kernel itself (here: another field on the
     same device stands for peer memory).  Fused (scalar layout, simd[3] = 1) and two-launch (x3 split) variants."""
@@ -155,7 +155,7 @@ def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
     xs, ys = slabs(gx), slabs(gy)
     ps = halo.PeerShift()
     l3 = lL[3]
-    for disp in (1, -1, 2, -(l3 - 1), l3 - 1, 0):
+    for disp in sorted({v for v in (1, -1, 2, -(l3 - 1), l3 - 1, 0) if abs(v) < l3}):
         zc = [su3.alloc_field(d) for _ in range(world)]
         zm = [su3.alloc_field(d) for _ in range(world)]
         for r in range(world):
@@ -163,6 +163,8 @@ def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
             n0 = su3.su3_launch_count()
             ps.cshift(zc[r], ys[r], nxt, prv, disp)
             fused = W == 1 or su3.su3_desc_normalize(d).simd[3] == 1
+            if prec == su3.SU3_F32 and W == 1 and (lL[0] * lL[1] * lL[2] * nl) % 2:
+                fused = False          # 72-byte records with odd run boundaries: bulk copies cannot be 16-byte aligned
             if disp != 0:
                 assert su3.su3_launch_count() - n0 == (1 if fused else 2)
             ps.mul_shift(zm[r], xs[r], ys[r], nxt, prv, disp)
