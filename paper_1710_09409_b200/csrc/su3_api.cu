@@ -486,11 +486,11 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return SU3_OK;
   }
-  // The shifted product: the TMA pipeline with a shifted operand for fp64 whenever a tile has at most ~2 runs (a cycle of
-  // rd*P records is at least a tile long); measured at 48^4: 0.94-1.00 x copy against 0.89-0.97 for the register kernel.
-  // fp32 stays on the register kernel (0.97-0.99 x copy against 0.90-0.98).  path = 1 forces the pipeline.
-  const int64_t tile_recs = (9216 / (9 * 2 * d.prec)) / d.W;
-  const bool pipe_pays = d.prec == SU3_F64 && (int64_t)p.rd * P >= tile_recs;
+  // The shifted product: the TMA pipeline with a shifted operand for fp64 (the producer warp issues the runs of a tile in
+  // parallel, so even 5-6 runs per tile along the fastest dimension cost nothing: measured 0.92-1.00 x copy at 32^4-64^4
+  // against 0.88-0.95 for the register kernel); fp32 stays on the register kernel (0.95-0.99 against 0.85-0.96: its
+  // 4.6 KB operand slots make the pipeline's per-tile costs twice as visible).  path = 1 forces the pipeline, 2 the other.
+  const bool pipe_pays = d.prec == SU3_F64;
   if (op == su3::SH_MUL && (tn.path == 1 || (tn.path == 0 && pipe_pays)) && !odd72 && z->nmat < 0x7fffffffLL) {  // record indices fit 31 bits (P <= records)
     su3::ShiftInfo sh = {};
     sh.P = P; sh.rd = p.rd; sh.dmod = p.disp % p.rd; sh.qrot = p.disp / p.rd; sh.simd_d = p.simd_d; sh.lstride = p.lstride;

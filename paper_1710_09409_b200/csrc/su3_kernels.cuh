@@ -337,8 +337,13 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
   __syncthreads();
 
   if (tid >= NCW * 32) {
-    // ------------------------------------------------ producer: one elected lane issues the TMA bulk loads
-    if (tid == NCW * 32) {
+    // ------------------------------------------------ producer: one elected lane issues the TMA bulk loads; the runs of a
+    // shifted operand are issued by the whole producer warp, lane k taking the k-th run of the tile (closed form: run
+    // boundaries sit at blocks cyc + {0, rd - dmod} of every cycle of rd blocks) -- a shift along the fastest dimension
+    // has 5-6 runs per tile.  (Not with FIX8: there a run may need 8-byte head / tail copies tied to one thread's arrival.)
+    constexpr bool PAR = SHIFT && !FIX8;
+    const int plane = tid - NCW * 32;
+    if (plane == 0 || PAR) {
       const unsigned char *src[4] = {(const unsigned char *)p.x, (const unsigned char *)p.y,
                                      (const unsigned char *)p.u, (const unsigned char *)p.v};
       uint64_t pol = 0, pol_keep = 0;
@@ -357,7 +362,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
         const size_t goff = (size_t)m0 * 9u * CB;
         const uint64_t tpol = (p.hint == 2 && tile < p.pin_tiles) ? pol_keep : pol;
         constexpr int NPLAIN = SHIFT ? NIN - 1 : NIN;  // operands that are read at the site itself
-        if (bytes != b16) {  // fp32 with an odd matrix count: 8 trailing bytes per operand
+        if (plane == 0 && bytes != b16) {  // fp32 with an odd matrix count: 8 trailing bytes per operand
 #pragma unroll
           for (int o = 0; o < NPLAIN; o++)
             *reinterpret_cast<uint64_t *>(st + (FIRST + o) * slot_bytes + b16) =
@@ -374,45 +379,64 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
           constexpr uint32_t rb = 9u * W * CB;  // bytes per record
           int blk = R0 / P;
           int oc = blk % rd;
-          tinfo[s] = make_int2(oc, R0 - blk * P);
-          int Ra = R0;
-          while (Ra < R1) {
-            const bool carry = oc + dmod >= rd;
-            const int cyc = blk - oc;  // first block of this rd-cycle
-            const int eb = carry ? cyc + rd : cyc + rd - dmod;  // first block after this run
-            const long long Rbl = (long long)eb * P;
-            const int Rb = Rbl < R1 ? (int)Rbl : R1;
-            const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
-            const size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
-            unsigned char *d = sy + (size_t)(Ra - R0) * rb;
-            size_t gs16 = gs, ge16 = ge;
-            if (FIX8) {  // the first / last 8 bytes of a run that is not 16-byte aligned
-              gs16 = (gs + 15) & ~(size_t)15;
-              ge16 = ge & ~(size_t)15;
-              if (gs16 != gs) cp_async8(d, gy + gs);
-              if (ge16 != ge && ge16 >= gs16) cp_async8(d + (ge16 - gs), gy + ge16);
+          if (plane == 0) tinfo[s] = make_int2(oc, R0 - blk * P);
+          if (PAR) {
+            total += (uint32_t)(R1 - R0) * rb;
+            const int cyc0 = blk - oc;
+            for (int m = (oc >= rd - dmod ? 1 : 0) + plane;; m += 32) {
+              const long long ba = (long long)(cyc0 + (m >> 1) * rd + ((m & 1) ? rd - dmod : 0)) * P;
+              if (ba >= R1) break;
+              const long long bb = (long long)(cyc0 + ((m + 1) >> 1) * rd + (((m + 1) & 1) ? rd - dmod : 0)) * P;
+              const int Ra = ba > R0 ? (int)ba : R0, Rb = bb < R1 ? (int)bb : R1;
+              if (Rb <= Ra) continue;  // dmod = 0: the carry runs are empty
+              const long long Rs = (long long)Ra + (long long)((m & 1) ? dmod - rd : dmod) * P;
+              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
+              if (p.hint) bulk_g2s_hint(d, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s], tpol);
+              else bulk_g2s(d, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
             }
-            if (ge16 > gs16) {
-              total += (uint32_t)(ge16 - gs16);
-              if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
-              else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
+          } else {
+            int Ra = R0;
+            while (Ra < R1) {
+              const bool carry = oc + dmod >= rd;
+              const int cyc = blk - oc;  // first block of this rd-cycle
+              const int eb = carry ? cyc + rd : cyc + rd - dmod;  // first block after this run
+              const long long Rbl = (long long)eb * P;
+              const int Rb = Rbl < R1 ? (int)Rbl : R1;
+              const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
+              const size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
+              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
+              size_t gs16 = gs, ge16 = ge;
+              if (FIX8) {  // the first / last 8 bytes of a run that is not 16-byte aligned
+                gs16 = (gs + 15) & ~(size_t)15;
+                ge16 = ge & ~(size_t)15;
+                if (gs16 != gs) cp_async8(d, gy + gs);
+                if (ge16 != ge && ge16 >= gs16) cp_async8(d + (ge16 - gs), gy + ge16);
+              }
+              if (ge16 > gs16) {
+                total += (uint32_t)(ge16 - gs16);
+                if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
+                else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
+              }
+              Ra = Rb;
+              blk = eb;          // the next run starts at the block where the carry status flips
+              oc = eb % rd;
             }
-            Ra = Rb;
-            blk = eb;          // the next run starts at the block where the carry status flips
-            oc = eb % rd;
+            if (FIX8) cp_async_arrive_noinc(&full[s]);  // arrives once all cp.async copies above have landed (at once if none)
           }
-          if (FIX8) cp_async_arrive_noinc(&full[s]);  // arrives once all cp.async copies above have landed (at once if none)
         }
+        if (plane == 0) {
 #pragma unroll
-        for (int o = 0; o < NPLAIN; o++) {
-          if (p.hint)
-            bulk_g2s_hint(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s], tpol);
-          else
-            bulk_g2s(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s]);
+          for (int o = 0; o < NPLAIN; o++) {
+            if (p.hint)
+              bulk_g2s_hint(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s], tpol);
+            else
+              bulk_g2s(st + (FIRST + o) * slot_bytes, src[o] + goff, b16, &full[s]);
+          }
+          // expect-tx and the producer's arrival: the phase cannot complete before this arrival nor before every byte
+          // counted in `total` has landed, whichever lane issues its copy and whenever (the transaction count may be
+          // transiently negative until here)
+          mbar_arrive_expect_tx(&full[s], total);
         }
-        // expect-tx and the producer's arrival come LAST: the phase cannot complete before this arrival, and by now
-        // the byte count of the runs is known (the transaction count may be transiently negative until here)
-        mbar_arrive_expect_tx(&full[s], total);
         if (++s == S) {
           s = 0;
           ph ^= 1u;
@@ -521,24 +545,37 @@ __global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams 
       oc = eb % rd;
     }
   };
-  auto load = [&](int i) {  // lane 0 only
+  // The whole warp issues a tile's loads: run boundaries sit at blocks cyc + {0, rd - dmod} of every cycle of rd blocks,
+  // so lane k finds the k-th run of the tile in closed form and issues its bulk copy -- a shift along the fastest
+  // dimension has 5-6 runs per tile, and one lane walking them (two integer divisions per run) was what the kernel
+  // waited for there.
+  auto load = [&](int i) {  // all lanes
     const int s = i % S;
     const int R0 = ((int)blockIdx.x + i * (int)gridDim.x) * TR;
     const int R1 = R0 + TR < nrec ? R0 + TR : nrec;
     unsigned char *buf = smem + (size_t)s * tile_bytes;
-    mbar_arrive_expect_tx(&full[s], (uint32_t)(R1 - R0) * rb);
-    for_runs(R0, R1, [&](int Ra, int Rb, bool carry) {
+    if (lane == 0) mbar_arrive_expect_tx(&full[s], (uint32_t)(R1 - R0) * rb);
+    const int blk0 = R0 / P, oc0 = blk0 % rd, cyc0 = blk0 - oc0;
+    const int m0 = oc0 >= rd - dmod ? 1 : 0;  // boundary m: block cyc0 + (m / 2) * rd + (m odd ? rd - dmod : 0); runs m odd carry
+    for (int m = m0 + lane;; m += 32) {
+      const long long ba = (long long)(cyc0 + (m >> 1) * rd + ((m & 1) ? rd - dmod : 0)) * P;
+      if (ba >= R1) break;
+      const long long bb = (long long)(cyc0 + ((m + 1) >> 1) * rd + (((m + 1) & 1) ? rd - dmod : 0)) * P;
+      const int Ra = ba > R0 ? (int)ba : R0, Rb = bb < R1 ? (int)bb : R1;
+      if (Rb <= Ra) continue;  // dmod = 0: the carry runs are empty
+      const bool carry = m & 1;
       const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
       const unsigned char *base = (galt && (int)carry == p.sh.alt_carry) ? galt : gy;
       bulk_g2s(buf + (size_t)(Ra - R0) * rb, base + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
-    });
+    }
   };
   if (lane == 0) {
     for (int s = 0; s < S; s++) mbar_init(&full[s], 1);
     fence_mbar_init();
     fence_proxy_async();
-    for (int i = 0; i < mine && i < S; i++) load(i);
   }
+  __syncwarp();
+  for (int i = 0; i < mine && i < S; i++) load(i);
   __syncwarp();
   for (int i = 0; i < mine; i++) {
     const int s = i % S;
@@ -582,11 +619,10 @@ __global__ void __launch_bounds__(32) su3_cshift_bulk_kernel(const StreamParams 
       bulk_s2g(gz + (size_t)R0 * rb, buf, (uint32_t)(R1 - R0) * rb);
       bulk_commit();
       // the store before this one has finished reading its buffer: refill that buffer
-      if (i >= 1) {
-        bulk_wait_read<1>();
-        if (i - 1 + S < mine) load(i - 1 + S);
-      }
+      if (i >= 1) bulk_wait_read<1>();
     }
+    __syncwarp();
+    if (i >= 1 && i - 1 + S < mine) load(i - 1 + S);
   }
   if (lane == 0) bulk_wait_all<0>();
 }
