@@ -510,8 +510,8 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
 // ---------------------------------------------------------------- Cshift as a pure TMA copy (f3)
 // z[s] = y[s + disp*dim_hat] moves whole records, and in storage order a tile's sources are a few contiguous runs (see
 // ShiftInfo).  So Cshift is the ceiling kernel su3_bulk_copy_kernel with its one load per tile split into runs: one warp
-// per CTA, lane 0 moves tiles global -> shared -> global with bulk copies through a ring of `stages` buffers, and no
-// register ever holds data -- except for records that cross the sub-lattice boundary in a dimension that is split over
+// per CTA moves tiles global -> shared -> global with bulk copies through a ring of `stages` buffers (the loads of a
+// tile issued by all lanes, one run each; the store by lane 0), and no register ever holds data -- except for records that cross the sub-lattice boundary in a dimension that is split over
 // virtual nodes (simd_d > 1): their lanes rotate (S3), which the warp does in place in shared memory before the store.
 // p.x = the shifted field y, p.z = z; p.tile_mats = matrices per tile (a multiple of W).
 template <typename R, int W>
