@@ -759,7 +759,7 @@ def run_next_rows(args, r):
         c64 = c32 = r["ceil"].fresh(Ln, prec)
         dr = su3.make_desc(Ln, n_lorentz=4, prec=prec)
         nr = su3.su3_real_bytes(dr)
-        reps = max(1, (1 << 29) // nr)                       # batch enough copies of the field to stream >= 0.5 GB each
+        reps = max(1, min((1 << 29) // nr, f["zc"].nbytes // nr))   # batch copies of the field to stream up to 0.5 GB each (within the resident fields)
         dbig = su3.make_desc((Ln, Ln, Ln, Ln * reps), n_lorentz=4, prec=prec)
         nbig = su3.su3_real_bytes(dbig)
         v1, v2, v3 = (su3.su3_real_wrap(dbig, f[n_].tensor[:nbig]) for n_ in ("xs", "ys", "zc"))

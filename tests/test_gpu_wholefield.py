@@ -134,3 +134,44 @@ def test_64x4_fp64_mul_whole_field_then_soak():
         su3.su3_mul(zv, xv, yv)
         su3.su3_convert(outs[0], zv)
         assert torch.equal(outs[0].tensor, ref.tensor), "vector launch %d" % rnd
+
+
+@pytest.mark.parametrize("prec,layout,W", [(F64, SC, 1), (F64, VE, 4), (F32, VE, 8), (F32, SC, 1)])
+def test_32x4_round2_kernels_whole_field_then_soak(prec, layout, W):
+    """The kernels rebuilt in round 2 -- the row-split interpreter (incl. a product whose right factor is computed: the
+    three warps of a matrix exchange rows), the menu rows, Cshift and the shifted product with their runs issued by the
+    whole warp (dim 0: 5-6 runs per tile; dim 3: lane rotation in the vector layout) -- at 32^4 (1 M matrices, HBM-bound,
+    library defaults): every element against the oracle, then 30 repetitions bit-identical to the verified result."""
+    desc = su3.make_desc(32, prec=prec, layout=layout, W=W)
+    g, gs = geom_of(desc), geom_of(su3.make_desc(32, prec=prec))
+    hs = [oracle.convert(g, gs, logical(desc, 77, fid)) if layout == VE else logical(desc, 77, fid) for fid in range(4)]
+    fs = [up(desc, h) for h in hs]
+    z = su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    dt = NPDT[prec]
+
+    def down():
+        torch.cuda.synchronize()
+        return z.tensor.cpu().numpy().view(dt)
+
+    cases = [("expr 01*23**", lambda: su3.su3_expr(z, "01*23**", fs), lambda: oracle.expr(g, "01*23**", *hs), 4),
+             ("expr 012**", lambda: su3.su3_expr(z, "012**", fs[:3]), lambda: oracle.expr(g, "012**", *hs[:3]), 4),
+             ("expr 01*2*3* (interpreter)", lambda: su3.su3_expr(z, "01*2*3*", fs), lambda: oracle.expr(g, "01*2*3*", *hs), 4),
+             ("expr 01*23*+ (menu)", lambda: su3.su3_expr(z, "01*23*+", fs), lambda: oracle.expr(g, "01*23*+", *hs), 4),
+             ("mul_shift dim 0", lambda: su3.su3_mul_shift(z, fs[0], fs[1], 0, 1), lambda: oracle.mul_shift(g, hs[0], hs[1], 0, 1), 1),
+             ("mul_shift dim 3", lambda: su3.su3_mul_shift(z, fs[0], fs[1], 3, -1), lambda: oracle.mul_shift(g, hs[0], hs[1], 3, -1), 1)]
+    for name, run, ref, k in cases:
+        run()
+        first = down().copy()
+        err, _ = rel_err_chunked(first, ref(), Wn)
+        assert err <= k * TOL[prec], (name, err)
+        for _ in range(30):
+            run()
+        assert np.array_equal(down(), first), name
+    for dim, disp in ((0, 1), (0, -3), (3, 1), (2, -1)):
+        su3.su3_cshift(z, fs[1], dim, disp)
+        first = down().copy()
+        assert np.array_equal(first, oracle.cshift(g, hs[1], dim, disp)), (dim, disp)
+        for _ in range(30):
+            su3.su3_cshift(z, fs[1], dim, disp)
+        assert np.array_equal(down(), first), (dim, disp)
