@@ -58,6 +58,10 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true", help="skip the volume sweep (configs[4]) after the timed steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--halo", action="store_true",
+                    help="N > 1 with one GPU per rank (NCCL) only, opt-in: also time the one exchange step of the path, Cshift "
+                         "along x3 across the slabs (halo.SlabShift: face pack -> NCCL send/recv || local shift -> unpack), and "
+                         "report it beside the local su3_cshift under \"halo\"")
     ap.add_argument("--profile-pass", action="store_true",
                     help="launch every kernel variant of the library once at 48^4 (no timing): the command ncu wraps "
                          "for profiles/*_all_kernels.md")
@@ -450,6 +454,40 @@ def time_calls(torch, fn, target_ms=2.0, batches=10, warm=3, graph_below_us=0.0)
         b.record(); b.synchronize()
         per.append(a.elapsed_time(b) / nloop)
     return float(min(per)), float(np.median(per)), how
+
+
+def run_halo(args, r, world, rank):
+    """The exchange step of the multi-GPU path, timed on every rank with CUDA events, max over ranks.
+    A tripwire checks the data that crossed: the last x3 plane of rank r's result must be the first plane of rank r+1's input."""
+    torch, su3, f, dist = r["torch"], r["su3"], r["f"], r["dist"]
+    from paper_1710_09409_b200 import halo, shard
+    sh = halo.SlabShift(halo.DistComm(dist))
+    out = []
+    for name_y, name_z, lay in (("ys", "zc", "scalar"), ("yv", "zv", "vector W=%d" % W64)):
+        y, z = f[name_y], f[name_z]
+        res = {"layout": lay}
+        for label, fn in (("sharded", lambda: sh.cshift(z, y, 3, 1)), ("local_periodic", lambda: su3.su3_cshift(z, y, 3, 1))):
+            for _ in range(3):
+                fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            r["barrier"]()
+            a.record()
+            for _ in range(10):
+                fn()
+            b.record(); b.synchronize()
+            _, ms, _ = shard.job_throughput(1.0, a.elapsed_time(b) / 10, dist, r["dev"])
+            res[label + "_ms"] = ms
+            res[label + "_GBps_per_rank"] = 2 * y.nbytes / (ms * 1e-3) / 1e9
+        if lay == "scalar":
+            sh.cshift(z, y, 3, 1)
+            torch.cuda.synchronize()
+            plane = y.nbytes // y.desc.L[3]
+            mine = torch.stack([y.tensor[:plane].to(torch.int64).sum(), z.tensor[-plane:].to(torch.int64).sum()])
+            allv = [torch.zeros_like(mine) for _ in range(world)]
+            dist.all_gather(allv, mine)
+            res["face_checksum_ok"] = bool(all(int(allv[k][1]) == int(allv[(k + 1) % world][0]) for k in range(world)))
+        out.append(res)
+    return out
 
 
 def run_e2e(args, r, world):
@@ -909,6 +947,9 @@ def main():
     r = run_ours(args, rank, world, local_rank)
     torch = r["torch"]
     e2e = None if args.no_e2e else run_e2e(args, r, world)
+    halo_leg = None
+    if args.halo and world > 1 and r["dist"] is not None and r["dist"].get_backend() == "nccl":
+        halo_leg = run_halo(args, r, world, rank)
     ceilings, sweep = ({}, [])
     next_rows = None
     if rank == 0:
@@ -962,7 +1003,7 @@ def main():
         "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
         "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k not in ("wsweep", "by_size", "convert_f32")},
         "ceilings_by_size": ceilings.get("by_size"), "convert_f32": ceilings.get("convert_f32"),
-        "wsweep": ceilings.get("wsweep"), "next_rows": next_rows, "sweep": sweep, "checks": r["checks"],
+        "wsweep": ceilings.get("wsweep"), "next_rows": next_rows, "halo": halo_leg, "sweep": sweep, "checks": r["checks"],
         "wall_s_timed_region": r["t_wall"],
         # the paper's own numbers for z = x*y, as context only (other hardware, fp32, volumes unstated)
         "paper_context": {"hardware": "NVIDIA GTX 1080, 288 GB/s peak, ~240 GB/s sustainable (P:156)",

@@ -451,6 +451,13 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
   const int base = (t / W) * 9 * W + (t % W);
   uint64_t pol = 0;
   if (p.hint && t == 0) pol = policy_evict_first();
+  // SHIFT across virtual nodes: the lane that holds my neighbour, for records that do / do not wrap around the sub-lattice
+  int lsrc_plain = t % W, lsrc_carry = t % W;
+  if (SHIFT && W > 1 && p.sh.simd_d > 1) {
+    const int ic = (lsrc_plain / p.sh.lstride) % p.sh.simd_d;
+    lsrc_carry += ((ic + p.sh.qrot + 1) % p.sh.simd_d - ic) * p.sh.lstride;
+    lsrc_plain += ((ic + p.sh.qrot) % p.sh.simd_d - ic) * p.sh.lstride;
+  }
   int s = 0, prev_s = -1;
   uint32_t ph = 0;
   for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -467,12 +474,12 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
         int lsrc = t % W;
         if (W > 1 && p.sh.simd_d > 1) {  // which lane holds my neighbour: a step across the sub-lattice boundary rotates lanes
           const int2 ti = tinfo[s];
-          const int r = ti.y + t / W;
-          const int oc = (ti.x + r / (int)p.sh.P) % p.sh.rd;
-          const int carry = oc + p.sh.dmod >= p.sh.rd ? 1 : 0;
-          const int ic = (lsrc / p.sh.lstride) % p.sh.simd_d;
-          const int icn = (ic + p.sh.qrot + carry) % p.sh.simd_d;
-          lsrc += (icn - ic) * p.sh.lstride;
+          const int r = ti.y + t / W, P = (int)p.sh.P, rd = p.sh.rd;
+          // blocks of P records between the tile's first record and mine: 0 or 1 when a block is at least a tile long
+          const int k = P >= TM / W ? (r >= P ? 1 : 0) : r / P;
+          int oc = ti.x + k;
+          if (oc >= rd) oc = k <= 1 ? oc - rd : oc % rd;
+          lsrc = oc + p.sh.dmod >= rd ? lsrc_carry : lsrc_plain;
         }
         src[NIN - 1] = reinterpret_cast<const C2 *>(st + (NSLOT - 1) * slot_bytes + p.sh.phase) + (t / W) * 9 * W + lsrc;
       }
