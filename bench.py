@@ -736,7 +736,8 @@ def run_next_rows(args, r):
         # programs on the ahead-of-time menu (they run on the pipeline kernel), programs that are not (the interpreter),
         # and two menu programs forced through the interpreter (launch knob path = 3) for comparison
         for prog, force in (("01*", 0), ("01*2*", 0), ("01*2+", 0), ("01+01*+", 0), ("01*23*+", 0), ("01+2+3+", 0),
-                            ("01*2*3*", 0), ("01*23**", 0), ("012**", 0), ("01+01*+", 1), ("01*23*+", 1)):
+                            ("01*2*3*", 0), ("01*23**", 0), ("012**", 0), ("01*2*0*", 0), ("01*23*+0-", 0),
+                            ("01+01*+", 1), ("01*23*+", 1), ("01*23**", 1)):
             n = max(int(c) for c in prog if c.isdigit()) + 1
             st, fl = su3.su3_expr_cost(prog, n)
             plan = su3.su3_expr_plan(prog, n)

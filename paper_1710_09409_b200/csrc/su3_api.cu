@@ -402,7 +402,7 @@ int match_menu(const ExprProgram &pr, int nops, bool real, int map[4]) {
   return -1;
 }
 const char *const kMenuPostfix[su3::OP_COUNT] = {"01*", "01*2*", "01*2+", "01+", "01+01*+", "01*23*+", "01*23*-", "01*2-",
-                                                 "01+2+", "01+2+3+", "01-", "01*", "01+01*+", "0"};
+                                                 "01+2+", "01+2+3+", "01-", "01*", "01+01*+", "01*2*3*", "012**", "01*23**", "0"};
 
 // ---------------------------------------------------------------- Cshift / shifted product
 // alt != NULL (su3_cshift_slab, op = SH_COPY only): the runs that leave the slab are read from the neighbouring slab

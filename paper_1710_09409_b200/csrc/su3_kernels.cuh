@@ -176,8 +176,11 @@ enum { OP_MUL = 0, OP_MUL3 = 1, OP_MUL_ADD = 2, OP_ADD = 3,
        OP_SUB = 10,         // a - b              "01-"
        OP_EMUL = 11,        // reals: a*b         "01*" on real scalar fields
        OP_SUM_EPROD = 12,   // reals: a + b + a*b "01+01*+" on real scalar fields (Listing 2 itself)
-       OP_COPY = 13,        // z = a (only used with a shifted operand: Cshift)
-       OP_COUNT = 14 };
+       OP_MUL4 = 13,        // a*b*c*d            "01*2*3*"   products of three and four matrices in every association:
+       OP_MUL_R = 14,       // a*(b*c)            "012**"     the shapes of plaquette-like expressions
+       OP_MULMUL_MUL = 15,  // (a*b)*(c*d)        "01*23**"
+       OP_COPY = 16,        // z = a (only used with a shifted operand: Cshift)
+       OP_COUNT = 17 };
 struct MenuProg {
   int nin, nins, min_ctas;  // operands, instructions, resident CTAs per SM the registers must allow
   ExprIns ins[4];
@@ -198,6 +201,9 @@ __host__ __device__ constexpr MenuProg menu_prog(int op) {
     case OP_SUB: return {2, 1, 3, {{EX_SUB, 0, 1, N}}};
     case OP_EMUL: return {2, 1, 3, {{EX_EMUL, 0, 1, N}}};
     case OP_SUM_EPROD: return {2, 3, 3, {{EX_ADD, 0, 1, N}, {EX_EMUL, 0, 1, T}, {EX_ADD, T, A, N}}};
+    case OP_MUL4: return {4, 3, 2, {{EX_MUL, 0, 1, N}, {EX_MUL, A, 2, N}, {EX_MUL, A, 3, N}}};
+    case OP_MUL_R: return {3, 2, 3, {{EX_MUL, 1, 2, N}, {EX_MUL, 0, A, N}}};
+    case OP_MULMUL_MUL: return {4, 3, 2, {{EX_MUL, 0, 1, N}, {EX_MUL, 2, 3, T}, {EX_MUL, T, A, N}}};
     case OP_COPY: return {1, 1, 3, {{EX_COPY, 0, N, N}}};
   }
   return {0, 0, 1, {}};

@@ -27,6 +27,9 @@ template <typename R> stream_kernel_t menu_any(int op, int W) {
     case su3::OP_MUL_MUL_ADD: return pipe_for_w<R, su3::OP_MUL_MUL_ADD>(W);
     case su3::OP_MUL_MUL_SUB: return pipe_for_w<R, su3::OP_MUL_MUL_SUB>(W);
     case su3::OP_MUL_SUB: return pipe_for_w<R, su3::OP_MUL_SUB>(W);
+    case su3::OP_MUL4: return pipe_for_w<R, su3::OP_MUL4>(W);
+    case su3::OP_MUL_R: return pipe_for_w<R, su3::OP_MUL_R>(W);
+    case su3::OP_MULMUL_MUL: return pipe_for_w<R, su3::OP_MULMUL_MUL>(W);
     case su3::OP_ADD3: return su3::su3_pipe_kernel<R, 1, su3::OP_ADD3, NCW, 0>;
     case su3::OP_ADD4: return su3::su3_pipe_kernel<R, 1, su3::OP_ADD4, NCW, 0>;
     case su3::OP_SUB: return su3::su3_pipe_kernel<R, 1, su3::OP_SUB, NCW, 0>;

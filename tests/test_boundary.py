@@ -321,11 +321,11 @@ def test_ahead_of_time_menu_rows_and_matching():
     operands and by either order of the sources of '+'; everything else goes to the interpreter"""
     rows = {}
     for prog, n in [("01*", 2), ("01*2*", 3), ("01*2+", 3), ("01+", 2), ("01+01*+", 2), ("01*23*+", 4), ("01*23*-", 4),
-                    ("01*2-", 3), ("01+2+", 3), ("01+2+3+", 4), ("01-", 2)]:
+                    ("01*2-", 3), ("01+2+", 3), ("01+2+3+", 4), ("01-", 2), ("01*2*3*", 4), ("012**", 3), ("01*23**", 4)]:
         plan = su3.su3_expr_plan(prog, n)
         assert plan[0] == "menu" and plan[2] == prog and plan[3] == list(range(n)), (prog, plan)
         rows[prog] = plan[1]
-    assert sorted(rows.values()) == list(range(11))          # eleven distinct rows for matrix fields
+    assert sorted(rows.values()) == list(range(11)) + [13, 14, 15]   # fourteen distinct rows for matrix fields (11, 12: real fields)
     # renamed operands: slot k of the row holds the operand that plays its part
     assert su3.su3_expr_plan("10*", 2) == ("menu", rows["01*"], "01*", [1, 0])
     assert su3.su3_expr_plan("20*1+", 3) == ("menu", rows["01*2+"], "01*2+", [2, 0, 1])
@@ -333,7 +333,8 @@ def test_ahead_of_time_menu_rows_and_matching():
     assert su3.su3_expr_plan("10+01*+", 2)[:2] == ("menu", rows["01+01*+"])
     assert su3.su3_expr_plan("32*10*+", 4) == ("menu", rows["01*23*+"], "01*23*+", [3, 2, 1, 0])
     # not on the menu: repeated fields, other shapes, non-commutative swaps
-    for prog, n in [("00*", 1), ("012**", 3), ("201*-", 3), ("01*21*-", 3), ("01*23*45*++", 6), ("0", 1), ("01-2-", 3)]:
+    assert su3.su3_expr_plan("210**", 3) == ("menu", rows["012**"], "012**", [2, 1, 0])
+    for prog, n in [("00*", 1), ("01*2*3*4*", 5), ("0123***", 4), ("201*-", 3), ("01*21*-", 3), ("01*23*45*++", 6), ("0", 1), ("01-2-", 3)]:
         assert su3.su3_expr_plan(prog, n) == "interpreter", prog
     # real scalar fields: '*' is element-wise; Listing 2's two programs are on the menu
     assert su3.su3_expr_plan("01+", 2, real_fields=True)[:2] == ("menu", rows["01+"])

@@ -180,7 +180,8 @@ def test_lattice_front_end_assign():
 
 
 MENU = [("01+01*+", 2), ("10+01*+", 2), ("01*23*+", 4), ("32*10*+", 4), ("01*23*-", 4), ("01*2-", 3), ("01+2+", 3),
-        ("01+2+3+", 4), ("01-", 2), ("10-", 2), ("201*+", 3)]
+        ("01+2+3+", 4), ("01-", 2), ("10-", 2), ("201*+", 3), ("01*2*3*", 4), ("012**", 3), ("210**", 3), ("01*23**", 4),
+        ("32*10**", 4)]
 
 
 @pytest.mark.parametrize("prec", [F64, F32])
