@@ -1650,39 +1650,46 @@ __global__ void __launch_bounds__(NT, 8) su3_convert_tma_kernel(const ConvertPar
     bulk_g2s(tile, src + (size_t)rec0 * NC * W * CB, (uint32_t)n * CB, bar);
   }
   mbar_wait(bar, 0);
-  // Slot idx of the block handles element (lane l, row k).  Plain order (l fastest) is conflict-free on both sides for
-  // 16-byte complex numbers and for W <= 8; with 8-byte complex numbers and W >= 16 a half-warp would hit 16 rows whose
-  // bases are all even (rows are 16-byte aligned), i.e. 8 bank pairs: there lanes 0-7 of a 16-lane group take row 2j
-  // and lanes 8-15 row 2j+1 in one half-warp, the other way round in the next (pitch = 2 mod 16).
+  // Slot idx = i*NT + tid of the block handles element (lane l, row index k).  Plain order (l fastest) is conflict-free on
+  // both sides for 16-byte complex numbers and for W <= 8; with 8-byte complex numbers and W >= 16 a half-warp would hit
+  // 16 rows whose bases are all even (rows are 16-byte aligned), i.e. 8 bank pairs: there lanes 0-7 of a 16-lane group
+  // take row 2j and lanes 8-15 row 2j+1 in one half-warp, the other way round in the next (pitch = 2 mod 16).
+  // Either way (l, k) is LINEAR in i -- l fixed per thread, k = k0 + i*DK -- so both passes are a pointer walk with a
+  // constant stride: two instructions per element.  (Decoding idx per element cost ~50 instructions each and made the
+  // fp32 kernel issue-bound at W >= 16: ncu, math-pipe throttle and 0.95 eligible warps per cycle.)
   const int K = nr * NC;
-  auto decode = [&](int idx, int &l, int &k) {
-    if (CB == 8 && W >= 16) {
-      const int i = idx & 31, blk = idx >> 5;
-      constexpr int G = W >= 16 ? W / 16 : 1;  // 16-lane groups per record
-      const int g = blk % G, kp = blk / G;
-      l = 16 * g + (i & 15);
-      k = 2 * kp + (((i >> 4) + ((i & 15) >> 3)) & 1);
-    } else {
-      l = idx % W;
-      k = idx / W;
-    }
-  };
-  C2 v[PER];
-#pragma unroll
-  for (int i = 0; i < PER; i++) {
-    int l, k;
-    decode(i * NT + tid, l, k);
-    if (k < K) v[i] = p.to_vector ? tile[l * pitch + k] : tile[k * W + l];
+  int l, k0;
+  constexpr bool SWZ = CB == 8 && W >= 16;
+  constexpr int DK = SWZ ? 2 * (NT / 32) / (W / 16) : NT / W;  // rows advanced per i
+  static_assert(NT % 32 == 0 && NT % W == 0 && (!SWZ || (NT / 32) % (W / 16) == 0), "slot order must be linear in i");
+  if constexpr (SWZ) {
+    constexpr int G = W / 16;  // 16-lane groups per record
+    const int i5 = tid & 31, w = tid >> 5;
+    l = 16 * (w % G) + (i5 & 15);
+    k0 = 2 * (w / G) + (((i5 >> 4) + ((i5 & 15) >> 3)) & 1);
+  } else {
+    l = tid % W;
+    k0 = tid / W;
   }
-  __syncthreads();
+  const int row = l * pitch + k0, dense = k0 * W + l;     // element (l, k0) in the [lane][k] rows / in the dense [k][lane] tile
+  const C2 *rp = tile + (p.to_vector ? row : dense);
+  C2 *wp = tile + (p.to_vector ? dense : row);
+  const int rs = p.to_vector ? DK : DK * W, ws = p.to_vector ? DK * W : DK;
+  C2 v[PER];
+  if (nr == TR) {
 #pragma unroll
-  for (int i = 0; i < PER; i++) {
-    int l, k;
-    decode(i * NT + tid, l, k);
-    if (k < K) {
-      if (p.to_vector) tile[k * W + l] = v[i];
-      else tile[l * pitch + k] = v[i];
-    }
+    for (int i = 0; i < PER; i++) v[i] = rp[i * rs];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < PER; i++) wp[i * ws] = v[i];
+  } else {  // the last, ragged block
+#pragma unroll
+    for (int i = 0; i < PER; i++)
+      if (k0 + i * DK < K) v[i] = rp[i * rs];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < PER; i++)
+      if (k0 + i * DK < K) wp[i * ws] = v[i];
   }
   fence_proxy_async();
   __syncthreads();
