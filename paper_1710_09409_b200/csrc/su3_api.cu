@@ -220,7 +220,9 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
   } else {
     // defaults measured on B200: 9 KB operand slots (64 fp64 / 128 fp32 matrices),
     // a 3-deep ring, 2 persistent CTAs per SM
-    int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 2;
+    // 2 persistent CTAs per SM; 3 for the copy through a shifted slot (Cshift of 72-byte records with odd run boundaries:
+    // no arithmetic to hide behind, measured 0.81 -> 0.96 x copy)
+    int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (sh && nin == 1 ? 3 : 2);
     int tm = tn.tile_mats;
     if (tm == 0) {
       tm = 9216 / (9 * cb);
@@ -491,7 +493,11 @@ su3_status launch_shift(int op, su3_field *z, const su3_field *x, const su3_fiel
   // against 0.88-0.95 for the register kernel); fp32 stays on the register kernel (0.95-0.99 against 0.85-0.96: its
   // 4.6 KB operand slots make the pipeline's per-tile costs twice as visible).  path = 1 forces the pipeline, 2 the other.
   const bool pipe_pays = d.prec == SU3_F64;
-  if (op == su3::SH_MUL && (tn.path == 1 || (tn.path == 0 && pipe_pays)) && !odd72 && z->nmat < 0x7fffffffLL) {  // record indices fit 31 bits (P <= records)
+  // Cshift of 72-byte records whose run boundaries are odd (no 16-byte alignment for the pure copy kernel above): the
+  // pipeline with OP_COPY, whose consumers move the matrices out of the 8-byte-shifted slot (0.95-0.96 x copy against 0.88
+  // for the cp.async gather kernel, which path = 3 still selects, and 0.82 for the register kernel, path = 2)
+  const bool copy_pipe = op == su3::SH_COPY && !bulk_applies && (tn.path == 1 || tn.path == 0);
+  if (((op == su3::SH_MUL && (tn.path == 1 || (tn.path == 0 && pipe_pays))) || copy_pipe) && !odd72 && z->nmat < 0x7fffffffLL) {  // record indices fit 31 bits (P <= records)
     su3::ShiftInfo sh = {};
     sh.P = P; sh.rd = p.rd; sh.dmod = p.disp % p.rd; sh.qrot = p.disp / p.rd; sh.simd_d = p.simd_d; sh.lstride = p.lstride;
     sh.phase = (d.prec == SU3_F32 && d.W == 1 && ((int64_t)sh.dmod * P) % 2) ? 8 : 0;

@@ -334,7 +334,7 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
 
   if (tid == 0) {
     for (int s = 0; s < S; s++) {
-      mbar_init(&full[s], FIX8 ? 2 : 1);
+      mbar_init(&full[s], FIX8 ? 33 : 1);  // FIX8: + one cp.async arrival per producer lane
       mbar_init(&empty[s], 1);
     }
     fence_mbar_init();
@@ -346,8 +346,9 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
     // ------------------------------------------------ producer: one elected lane issues the TMA bulk loads; the runs of a
     // shifted operand are issued by the whole producer warp, lane k taking the k-th run of the tile (closed form: run
     // boundaries sit at blocks cyc + {0, rd - dmod} of every cycle of rd blocks) -- a shift along the fastest dimension
-    // has 5-6 runs per tile.  (Not with FIX8: there a run may need 8-byte head / tail copies tied to one thread's arrival.)
-    constexpr bool PAR = SHIFT && !FIX8;
+    // has 5-6 runs per tile.  With FIX8 a run may also need 8-byte head / tail copies (cp.async): every producer lane then
+    // arrives on the stage's mbarrier once its own cp.async copies have landed (33 arrivals per phase).
+    constexpr bool PAR = SHIFT;
     const int plane = tid - NCW * 32;
     if (plane == 0 || PAR) {
       const unsigned char *src[4] = {(const unsigned char *)p.x, (const unsigned char *)p.y,
@@ -386,48 +387,35 @@ __global__ void __launch_bounds__((NCW + 1) * 32, menu_prog(OP).min_ctas) su3_pi
           int blk = R0 / P;
           int oc = blk % rd;
           if (plane == 0) tinfo[s] = make_int2(oc, R0 - blk * P);
-          if (PAR) {
-            total += (uint32_t)(R1 - R0) * rb;
-            const int cyc0 = blk - oc;
-            for (int m = (oc >= rd - dmod ? 1 : 0) + plane;; m += 32) {
-              const long long ba = (long long)(cyc0 + (m >> 1) * rd + ((m & 1) ? rd - dmod : 0)) * P;
-              if (ba >= R1) break;
-              const long long bb = (long long)(cyc0 + ((m + 1) >> 1) * rd + (((m + 1) & 1) ? rd - dmod : 0)) * P;
-              const int Ra = ba > R0 ? (int)ba : R0, Rb = bb < R1 ? (int)bb : R1;
-              if (Rb <= Ra) continue;  // dmod = 0: the carry runs are empty
-              const long long Rs = (long long)Ra + (long long)((m & 1) ? dmod - rd : dmod) * P;
-              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
-              if (p.hint) bulk_g2s_hint(d, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s], tpol);
-              else bulk_g2s(d, gy + (size_t)Rs * rb, (uint32_t)(Rb - Ra) * rb, &full[s]);
+          uint32_t mine = 0;  // bytes of my bulk copies
+          const int cyc0 = blk - oc;
+          for (int m = (oc >= rd - dmod ? 1 : 0) + plane;; m += 32) {
+            const long long ba = (long long)(cyc0 + (m >> 1) * rd + ((m & 1) ? rd - dmod : 0)) * P;
+            if (ba >= R1) break;
+            const long long bb = (long long)(cyc0 + ((m + 1) >> 1) * rd + (((m + 1) & 1) ? rd - dmod : 0)) * P;
+            const int Ra = ba > R0 ? (int)ba : R0, Rb = bb < R1 ? (int)bb : R1;
+            if (Rb <= Ra) continue;  // dmod = 0: the carry runs are empty
+            const long long Rs = (long long)Ra + (long long)((m & 1) ? dmod - rd : dmod) * P;
+            const size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
+            unsigned char *d = sy + (size_t)(Ra - R0) * rb;
+            size_t gs16 = gs, ge16 = ge;
+            if (FIX8) {  // the first / last 8 bytes of a run that is not 16-byte aligned
+              gs16 = (gs + 15) & ~(size_t)15;
+              ge16 = ge & ~(size_t)15;
+              if (gs16 != gs) cp_async8(d, gy + gs);
+              if (ge16 != ge && ge16 >= gs16) cp_async8(d + (ge16 - gs), gy + ge16);
             }
+            if (ge16 > gs16) {
+              mine += (uint32_t)(ge16 - gs16);
+              if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
+              else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
+            }
+          }
+          if (FIX8) {
+            cp_async_arrive_noinc(&full[s]);  // arrives once this lane's cp.async copies have landed (at once if none)
+            total += __reduce_add_sync(0xffffffffu, mine);
           } else {
-            int Ra = R0;
-            while (Ra < R1) {
-              const bool carry = oc + dmod >= rd;
-              const int cyc = blk - oc;  // first block of this rd-cycle
-              const int eb = carry ? cyc + rd : cyc + rd - dmod;  // first block after this run
-              const long long Rbl = (long long)eb * P;
-              const int Rb = Rbl < R1 ? (int)Rbl : R1;
-              const long long Rs = (long long)Ra + (long long)(carry ? dmod - rd : dmod) * P;
-              const size_t gs = (size_t)Rs * rb, ge = gs + (size_t)(Rb - Ra) * rb;
-              unsigned char *d = sy + (size_t)(Ra - R0) * rb;
-              size_t gs16 = gs, ge16 = ge;
-              if (FIX8) {  // the first / last 8 bytes of a run that is not 16-byte aligned
-                gs16 = (gs + 15) & ~(size_t)15;
-                ge16 = ge & ~(size_t)15;
-                if (gs16 != gs) cp_async8(d, gy + gs);
-                if (ge16 != ge && ge16 >= gs16) cp_async8(d + (ge16 - gs), gy + ge16);
-              }
-              if (ge16 > gs16) {
-                total += (uint32_t)(ge16 - gs16);
-                if (p.hint) bulk_g2s_hint(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s], tpol);
-                else bulk_g2s(d + (gs16 - gs), gy + gs16, (uint32_t)(ge16 - gs16), &full[s]);
-              }
-              Ra = Rb;
-              blk = eb;          // the next run starts at the block where the carry status flips
-              oc = eb % rd;
-            }
-            if (FIX8) cp_async_arrive_noinc(&full[s]);  // arrives once all cp.async copies above have landed (at once if none)
+            total += (uint32_t)(R1 - R0) * rb;
           }
         }
         if (plane == 0) {
