@@ -114,3 +114,40 @@ def test_random_geometries_and_splits_fuzz():
         su3.su3_mul(fz, fx, fy)
         err, _ = rel_err(download(fz), oracle.mul(g, x, y), W)
         assert err <= TOL[prec], (L, W, simd, err)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,nl,layout,W", [((2, 8, 8, 12), 1, SC, 1), ((4, 2, 6, 16), 1, SC, 1), ((6, 6, 6, 6), 4, SC, 1),
+                                           ((3, 5, 2, 16), 1, SC, 1), ((8, 8, 4, 8), 1, VE, 4), ((4, 4, 8, 8), 1, VE, 8),
+                                           ((16, 4, 4, 4), 1, VE, 2)])
+def test_every_shift_kernel_agrees_bitwise(prec, L, nl, layout, W):
+    """the kernels behind the `path` knob -- pure TMA copy / pipeline with a shifted slot (runs issued by all lanes, incl.
+    tiles with MORE than 32 runs: cycles of 2-4 records along dim 0, and the 8-byte run ends of 72-byte records),
+    register kernel, cp.async gather -- give the same bits as the default, which is checked against the oracle"""
+    desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=layout, W=W)
+    g = geom_of(desc)
+    x, y = host_field(desc, 53, 0), host_field(desc, 53, 1)
+    fx, fy, fz, fr = upload(desc, x), upload(desc, y), su3.alloc_field(desc), su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    for dim in range(4):
+        for disp in (1, -1, 2):
+            su3.su3_tune_set()
+            su3.su3_cshift(fr, fy, dim, disp)
+            assert np.array_equal(download(fr), oracle.cshift(g, y, dim, disp)), (dim, disp)
+            for path in (1, 2, 3):
+                su3.su3_tune_set(path=path)
+                fz.tensor.fill_(0xEE)
+                su3.su3_cshift(fz, fy, dim, disp)
+                torch.cuda.synchronize()
+                assert torch.equal(fz.tensor, fr.tensor), ("cshift", path, dim, disp)
+            su3.su3_tune_set()
+            su3.su3_mul_shift(fr, fx, fy, dim, disp)
+            err, _ = rel_err(download(fr), oracle.mul_shift(g, x, y, dim, disp), Wn)
+            assert err <= TOL[prec], (dim, disp, err)
+            for path in (1, 2):
+                su3.su3_tune_set(path=path)
+                fz.tensor.fill_(0xEE)
+                su3.su3_mul_shift(fz, fx, fy, dim, disp)
+                torch.cuda.synchronize()
+                assert torch.equal(fz.tensor, fr.tensor), ("mul_shift", path, dim, disp)
+    su3.su3_tune_set()
