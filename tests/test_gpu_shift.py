@@ -119,7 +119,7 @@ def test_random_geometries_and_splits_fuzz():
 @pytest.mark.parametrize("prec", [F64, F32])
 @pytest.mark.parametrize("L,nl,layout,W", [((2, 8, 8, 12), 1, SC, 1), ((4, 2, 6, 16), 1, SC, 1), ((6, 6, 6, 6), 4, SC, 1),
                                            ((3, 5, 2, 16), 1, SC, 1), ((8, 8, 4, 8), 1, VE, 4), ((4, 4, 8, 8), 1, VE, 8),
-                                           ((16, 4, 4, 4), 1, VE, 2)])
+                                           ((16, 4, 4, 4), 1, VE, 2), ((2, 32, 32, 64), 1, SC, 1), ((4, 16, 16, 64), 1, VE, 2)])
 def test_every_shift_kernel_agrees_bitwise(prec, L, nl, layout, W):
     """the kernels behind the `path` knob -- pure TMA copy / pipeline with a shifted slot (runs issued by all lanes, incl.
     tiles with MORE than 32 runs: cycles of 2-4 records along dim 0, and the 8-byte run ends of 72-byte records),
