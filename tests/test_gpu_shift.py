@@ -151,3 +151,43 @@ def test_every_shift_kernel_agrees_bitwise(prec, L, nl, layout, W):
                 torch.cuda.synchronize()
                 assert torch.equal(fz.tensor, fr.tensor), ("mul_shift", path, dim, disp)
     su3.su3_tune_set()
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("L,layout,W,simd", [((1, 1, 1, 1), SC, 1, None), ((1, 1, 1, 5), SC, 1, None), ((2, 1, 1, 1), VE, 2, (2, 1, 1, 1)),
+                                             ((1, 2, 1, 2), VE, 4, (1, 2, 1, 2)), ((1, 1, 3, 1), SC, 1, None)])
+def test_degenerate_lattices(prec, L, layout, W, simd):
+    """a single site, a single record, extents of 1: every shift is (partly) the identity, every tile is ragged; shifts,
+    the shifted product, the interpreter and the face calls (incl. zero planes) against the oracle"""
+    desc = su3.make_desc(L, prec=prec, layout=layout, W=W, simd=simd)
+    g = geom_of(desc)
+    x, y = host_field(desc, 59, 0), host_field(desc, 59, 1)
+    fx, fy, fz = upload(desc, x), upload(desc, y), su3.alloc_field(desc)
+    Wn = su3.su3_desc_normalize(desc).W
+    for path in (0, 1, 2, 3):
+        su3.su3_tune_set(path=path)
+        for dim in range(4):
+            for disp in (0, 1, -1, 7):
+                fz.tensor.fill_(0xEE)
+                su3.su3_cshift(fz, fy, dim, disp)
+                assert np.array_equal(download(fz), oracle.cshift(g, y, dim, disp)), (path, dim, disp)
+                if path < 3:
+                    su3.su3_mul_shift(fz, fx, fy, dim, disp)
+                    err, _ = rel_err(download(fz), oracle.mul_shift(g, x, y, dim, disp), Wn)
+                    assert err <= TOL[prec], (path, dim, disp, err)
+    su3.su3_tune_set(path=3)
+    for prog in ("01*", "01*01*+", "010**"):
+        su3.su3_expr(fz, prog, [fx, fy])
+        err, _ = rel_err(download(fz), oracle.expr(g, prog, x, y), Wn)
+        assert err <= 4 * TOL[prec], (prog, err)
+    su3.su3_tune_set()
+    for dim in range(4):
+        nb = su3.su3_face_bytes(fx, dim, L[dim])
+        assert nb == fx.nbytes and su3.su3_face_bytes(fx, dim, 0) == 0
+        buf = torch.empty(max(nb, 16), dtype=torch.uint8, device="cuda")
+        n0 = su3.su3_launch_count()
+        su3.su3_face_pack(buf, fx, dim, 0, 0)                      # zero planes: nothing is launched
+        assert su3.su3_launch_count() == n0
+        su3.su3_face_pack(buf, fx, dim, 0, L[dim])                 # all planes: the packed face is the scalar-layout field
+        gs = oracle.Geom(L)
+        assert np.array_equal(buf[:nb].cpu().numpy().view(x.dtype), oracle.convert(gs, g, x))
