@@ -860,7 +860,10 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   p.z = z->ptr;
   for (int i = 0; i < n_operands; i++) p.ops[i] = operands[i]->ptr;
   p.nmat = nrec; p.tile_mats = mps; p.stages = sw; p.nops = n_operands; p.nins = pr.nins; p.ntemp = pr.ntemp; p.xchg = xchg;
-  for (int i = 0; i < pr.nins; i++) p.ins[i] = pr.ins[i];
+  for (int i = 0; i < pr.nins; i++) {
+    p.ins[i] = pr.ins[i];
+    p.insx[i] = make_int4(pr.ins[i].op, pr.ins[i].a, pr.ins[i].b, pr.ins[i].spill);
+  }
   const int64_t ntiles = (nrec + mps - 1) / mps, max_grid = (int64_t)di.sms * ctas;
   k<<<(unsigned)(ntiles < max_grid ? ntiles : max_grid), 96, smem, (cudaStream_t)cuda_stream>>>(p);
   e = cudaGetLastError();

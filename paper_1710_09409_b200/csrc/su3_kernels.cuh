@@ -692,6 +692,7 @@ struct ExprParams {
   int tile_mats, stages, nops, nins, ntemp, hint;  // stages = ring depth of the CTA's private ring
   int xchg;                                          // 1: the program multiplies by a computed value on the RIGHT (one more slot)
   ExprIns ins[16];
+  int4 insx[16];  // the same instructions, one int per field (op, a, b, spill): what the interpreter reads
 };
 
 // row `c` = row `a` of the left factor times the full right factor: the rows of mat33_mul, operation for operation
@@ -782,71 +783,73 @@ __global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
     for (int t = lane; t < MPS; t += 32) {
       const int base = (t / W) * 9 * W + (t % W);   // element 0 of matrix t
       const int rbase = base + 3 * row * W;         // element (row, 0)
-      C2 acc[3], a[3], b[9];
+      // The dispatch is written so that NO copy of the accumulator is needed outside the one case that really needs it
+      // (a product whose LEFT factor is the accumulator): with a generic "load a, load b, combine" body the compiler
+      // copied the 12 accumulator registers at the top of every interpreted instruction (16 % of all executed
+      // instructions, ncu), and unpacking the four bytes of an ExprIns cost six more: insx holds them as four ints.
+      C2 acc[3];
 #pragma unroll 1
       for (int i = 0; i < p.nins; i++) {
-        const ExprIns in = p.ins[i];
-        if (in.spill != EX_NONE) {
-          C2 *sp = reinterpret_cast<C2 *>(temps + (size_t)(in.spill - EX_TEMP0) * slot_bytes) + rbase;
+        const int4 in = p.insx[i];   // x = op, y = a, z = b, w = spill
+        if (in.w != EX_NONE) {
+          C2 *sp = reinterpret_cast<C2 *>(temps + (size_t)(in.w - EX_TEMP0) * slot_bytes) + rbase;
 #pragma unroll
           for (int e = 0; e < 3; e++) sp[e * W] = acc[e];
         }
-        if (in.a == EX_SRC_ACC) {
-#pragma unroll
-          for (int e = 0; e < 3; e++) a[e] = acc[e];
-        } else {
-          const C2 *sa = reinterpret_cast<const C2 *>(in.a < EX_TEMP0 ? st + in.a * slot_bytes
-                                                                     : temps + (size_t)(in.a - EX_TEMP0) * slot_bytes) + rbase;
-#pragma unroll
-          for (int e = 0; e < 3; e++) a[e] = sa[e * W];
-        }
-        if (in.op == EX_MUL) {
-          if (in.b < EX_TEMP0) {
-            const C2 *sb = reinterpret_cast<const C2 *>(st + in.b * slot_bytes) + base;
+        const C2 *pa = reinterpret_cast<const C2 *>(in.y < EX_TEMP0 ? st + in.y * slot_bytes
+                                                                   : temps + (size_t)(in.y - EX_TEMP0) * slot_bytes) + rbase;
+        if (in.x == EX_MUL) {
+          C2 b[9];
+          if (in.z < EX_TEMP0) {
+            const C2 *sb = reinterpret_cast<const C2 *>(st + in.z * slot_bytes) + base;
 #pragma unroll
             for (int e = 0; e < 9; e++) b[e] = sb[e * W];
           } else {
             // the right factor is a computed value: its rows live in three different warps
             const C2 *whole;
-            if (in.b == EX_SRC_ACC) {
+            if (in.z == EX_SRC_ACC) {
               C2 *xs = reinterpret_cast<C2 *>(xchg) + rbase;
 #pragma unroll
               for (int e = 0; e < 3; e++) xs[e * W] = acc[e];
               whole = reinterpret_cast<const C2 *>(xchg) + base;
             } else {
-              whole = reinterpret_cast<const C2 *>(temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + base;
+              whole = reinterpret_cast<const C2 *>(temps + (size_t)(in.z - EX_TEMP0) * slot_bytes) + base;
             }
             __syncthreads();  // all three rows written
 #pragma unroll
             for (int e = 0; e < 9; e++) b[e] = whole[e * W];
             __syncthreads();  // all three warps have read: the slot may be written again
           }
-          mat33_mul_row(a, b, acc);
-        } else if (in.op == EX_COPY) {
+          if (in.y == EX_SRC_ACC) {
+            C2 r[3];
+            mat33_mul_row(acc, b, r);
 #pragma unroll
-          for (int e = 0; e < 3; e++) acc[e] = a[e];
-        } else {
-          C2 bb[3];
-          if (in.b == EX_SRC_ACC) {
-#pragma unroll
-            for (int e = 0; e < 3; e++) bb[e] = acc[e];
+            for (int e = 0; e < 3; e++) acc[e] = r[e];
           } else {
-            const C2 *sb = reinterpret_cast<const C2 *>(in.b < EX_TEMP0 ? st + in.b * slot_bytes
-                                                                       : temps + (size_t)(in.b - EX_TEMP0) * slot_bytes) + rbase;
+            C2 a[3];
 #pragma unroll
-            for (int e = 0; e < 3; e++) bb[e] = sb[e * W];
+            for (int e = 0; e < 3; e++) a[e] = pa[e * W];
+            mat33_mul_row(a, b, acc);
           }
+        } else if (in.x == EX_COPY) {
+#pragma unroll
+          for (int e = 0; e < 3; e++) acc[e] = pa[e * W];
+        } else {
+          // element-wise: acc = a (op) b with a, b each an operand / temporary in shared memory or the accumulator itself
+          const C2 *pb = reinterpret_cast<const C2 *>(in.z < EX_TEMP0 ? st + in.z * slot_bytes
+                                                                     : temps + (size_t)(in.z - EX_TEMP0) * slot_bytes) + rbase;
+          const R sgn = in.x == EX_SUB ? R(-1) : R(1);
 #pragma unroll
           for (int e = 0; e < 3; e++) {
-            if (in.op == EX_ADD) {
-              acc[e].x = add_rn(a[e].x, bb[e].x);
-              acc[e].y = add_rn(a[e].y, bb[e].y);
-            } else if (in.op == EX_SUB) {
-              acc[e].x = add_rn(a[e].x, -bb[e].x);
-              acc[e].y = add_rn(a[e].y, -bb[e].y);
-            } else {  // EX_EMUL
-              acc[e].x = mul_rn(a[e].x, bb[e].x);
-              acc[e].y = mul_rn(a[e].y, bb[e].y);
+            C2 av = acc[e], bv = acc[e];
+            if (in.y != EX_SRC_ACC) av = pa[e * W];
+            if (in.z != EX_SRC_ACC) bv = pb[e * W];
+            if (in.x == EX_EMUL) {
+              acc[e].x = mul_rn(av.x, bv.x);
+              acc[e].y = mul_rn(av.y, bv.y);
+            } else {  // a + b, a - b = a + (-1)*b exactly
+              acc[e].x = add_rn(av.x, sgn * bv.x);
+              acc[e].y = add_rn(av.y, sgn * bv.y);
             }
           }
         }
