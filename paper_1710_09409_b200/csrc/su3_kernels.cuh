@@ -745,9 +745,8 @@ __global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
   const long long ntiles = (p.nmat + MPS - 1) / MPS;
   const long long gw = blockIdx.x, GW = gridDim.x;
   const long long mine = ntiles > gw ? (ntiles - gw + GW - 1) / GW : 0;  // my tiles: gw, gw + GW, ...
-  auto load = [&](long long j) {  // tid 0 only
-    const int s = (int)(j % SW);
-    const long long m0 = (gw + j * GW) * MPS;
+  auto load = [&](int s, long long tile) {  // tid 0 only: tile `tile` into stage s
+    const long long m0 = tile * MPS;
     const long long left = p.nmat - m0;
     const int nm = left < MPS ? (int)left : MPS;
     const uint32_t bytes = (uint32_t)nm * 9u * CB;
@@ -766,17 +765,19 @@ __global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
     for (int q = 0; q < SW; q++) mbar_init(&full[q], 1);
     fence_mbar_init();
     fence_proxy_async();
-    for (long long j = 0; j < mine && j < SW; j++) load(j);
+    for (long long j = 0; j < mine && j < SW; j++) load((int)j, gw + j * GW);
   }
   __syncthreads();
-  for (long long j = 0; j < mine; j++) {
-    const int s = (int)(j % SW);
-    const long long m0 = (gw + j * GW) * MPS;
+  int s = 0;          // stage of tile j = j % SW, kept as a counter (no division per tile)
+  uint32_t ph = 0;    // its phase bit = (j / SW) & 1
+  long long tile = gw;
+  for (long long j = 0; j < mine; j++, tile += GW) {
+    const long long m0 = tile * MPS;
     const long long left = p.nmat - m0;
     const int nm = left < MPS ? (int)left : MPS;
     unsigned char *st = smem + (size_t)s * stage_bytes;
     unsigned char *myout = outs + (size_t)(j & 1) * slot_bytes;
-    mbar_wait(&full[s], (uint32_t)((j / SW) & 1));
+    mbar_wait(&full[s], ph);
     // every lane runs every iteration (the barriers below are CTA-wide); lanes past the ragged end compute on stale
     // shared memory inside the slot and their rows are never stored
 #pragma unroll 1
@@ -838,19 +839,37 @@ __global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
           // element-wise: acc = a (op) b with a, b each an operand / temporary in shared memory or the accumulator itself
           const C2 *pb = reinterpret_cast<const C2 *>(in.z < EX_TEMP0 ? st + in.z * slot_bytes
                                                                      : temps + (size_t)(in.z - EX_TEMP0) * slot_bytes) + rbase;
-          const R sgn = in.x == EX_SUB ? R(-1) : R(1);
+          // four source combinations, each a straight-line body (no selects, no copies)
+          auto ew = [&](const C2 (&av)[3], const C2 (&bv)[3]) {
 #pragma unroll
-          for (int e = 0; e < 3; e++) {
-            C2 av = acc[e], bv = acc[e];
-            if (in.y != EX_SRC_ACC) av = pa[e * W];
-            if (in.z != EX_SRC_ACC) bv = pb[e * W];
-            if (in.x == EX_EMUL) {
-              acc[e].x = mul_rn(av.x, bv.x);
-              acc[e].y = mul_rn(av.y, bv.y);
-            } else {  // a + b, a - b = a + (-1)*b exactly
-              acc[e].x = add_rn(av.x, sgn * bv.x);
-              acc[e].y = add_rn(av.y, sgn * bv.y);
+            for (int e = 0; e < 3; e++) {
+              if (in.x == EX_EMUL) {
+                acc[e].x = mul_rn(av[e].x, bv[e].x);
+                acc[e].y = mul_rn(av[e].y, bv[e].y);
+              } else if (in.x == EX_ADD) {
+                acc[e].x = add_rn(av[e].x, bv[e].x);
+                acc[e].y = add_rn(av[e].y, bv[e].y);
+              } else {
+                acc[e].x = add_rn(av[e].x, -bv[e].x);
+                acc[e].y = add_rn(av[e].y, -bv[e].y);
+              }
             }
+          };
+          C2 a[3], bb[3];
+          if (in.y != EX_SRC_ACC) {
+#pragma unroll
+            for (int e = 0; e < 3; e++) a[e] = pa[e * W];
+          }
+          if (in.z != EX_SRC_ACC) {
+#pragma unroll
+            for (int e = 0; e < 3; e++) bb[e] = pb[e * W];
+          }
+          if (in.y == EX_SRC_ACC) {
+            if (in.z == EX_SRC_ACC) ew(acc, acc);
+            else ew(acc, bb);
+          } else {
+            if (in.z == EX_SRC_ACC) ew(a, acc);
+            else ew(a, bb);
           }
         }
       }
@@ -865,13 +884,17 @@ __global__ void __launch_bounds__(96) su3_expr_kernel(const ExprParams p) {
     // every thread has read what it needs from stage s and written its rows of the result: re-arm the stage with my
     // tile j + SW at once -- the refill never waits for the store -- and send the result on its way
     if (tid == 0) {
-      if (j + SW < mine) load(j + SW);
+      if (j + SW < mine) load(s, tile + (long long)SW * GW);
       const uint32_t bytes = (uint32_t)nm * 9u * CB;
       const uint32_t b16 = bytes & ~15u;
       unsigned char *zdst = (unsigned char *)p.z + (size_t)m0 * 9u * CB;
       bulk_s2g(zdst, myout, b16);
       bulk_commit();
       if (bytes != b16) *reinterpret_cast<uint64_t *>(zdst + b16) = *reinterpret_cast<const uint64_t *>(myout + b16);
+    }
+    if (++s == SW) {
+      s = 0;
+      ph ^= 1u;
     }
   }
   if (tid == 0) bulk_wait_all<0>();
