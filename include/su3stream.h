@@ -168,7 +168,7 @@ su3_status su3_expr_disasm(const char *program, int n_operands, char *buf, size_
  * order of the sources of '+'), else "interpreter".  The rows, as postfix programs over distinct fields: 01* 01*2* 01*2+
  * 01+ 01+01*+ 01*23*+ 01*23*- 01*2- 01+2+ 01+2+3+ 01- 01*2*3* 012** 01*23** (and, for real scalar fields, 01+ 01* 01+01*+).
  * real_fields != 0: the operands are real scalar fields ('*' is element-wise).  Both routes give bit-identical
- * results; the menu rows run at the copy ceiling, the interpreter at 0.6-1.06 x of it.  Host-only. */
+ * results; the menu rows run at the copy ceiling, the interpreter at 0.8-1.09 x of it for typical programs.  Host-only. */
 su3_status su3_expr_plan(const char *program, int n_operands, int real_fields, char *buf, size_t buf_len);
 
 /* Accounting of a program by reading S9: field streams (n_operands + 1) and flops per matrix (198 per '*',
