@@ -846,7 +846,8 @@ su3_status su3_expr(su3_field *z, const char *program, const su3_field *const *o
   // (`01+01*+` fp64: 4 CTAs x 3 stages 0.79, 6 x 3 0.92, 8 x 2 0.99 x copy)
   int sw = tn.stages > 0 ? tn.stages : 2;
   int ctas = ctas_for(sw);
-  const int reg_cap = z->d.prec == SU3_F64 ? 10 : 16;  // CTAs of 96 threads per SM that 56-62 (fp64) / 40 (fp32) registers per thread allow
+  const int reg_cap = z->d.prec == SU3_F64 ? 7 : 12;  // resident CTAs of 96 threads per SM that 88-90 (fp64) / 48-56 (fp32) registers per thread allow;
+                                                      // asking for more would leave CTAs of the persistent grid waiting for a slot
   if (ctas > reg_cap) ctas = reg_cap;
   if (tn.ctas_per_sm > 0 && tn.ctas_per_sm < ctas) ctas = tn.ctas_per_sm;
   if (ctas < 1 || sw < 2) return fail(SU3_ERR_INVALID, "expression needs more shared memory than the device has (%d operands, %d temporaries)",
