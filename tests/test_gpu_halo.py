@@ -175,3 +175,55 @@ def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
         su3.su3_cshift_slab(zc[0], ys[0], ys[1], l3)
     with pytest.raises(su3.Su3Error):
         su3.su3_cshift_slab(ys[0], ys[0], ys[1], 1)
+
+
+def test_slab_shift_fuzz():
+    """random slab counts, extents, virtual-node splits, precisions and displacements (up to two turns around the global
+    lattice): both executors -- packed faces through a communicator, and neighbour slabs read directly -- against the
+    oracle's Cshift / shifted product on the global lattice"""
+    rng = np.random.default_rng(2026)
+    for it in range(40):
+        world = int(rng.integers(2, 5))
+        W = int(2 ** rng.integers(0, 5))
+        simd, w = [1, 1, 1, 1], W
+        while w > 1:
+            simd[int(rng.integers(0, 4))] *= 2
+            w //= 2
+        lL = [int(s * rng.integers(1, 5)) for s in simd]
+        gL = (lL[0], lL[1], lL[2], lL[3] * world)
+        nl, prec = int(rng.choice([1, 4])), int(rng.choice([su3.SU3_F64, su3.SU3_F32]))
+        d = su3.make_desc(tuple(lL), n_lorentz=nl, prec=prec, layout=VEC if W > 1 else su3.SU3_SCALAR, W=W,
+                          simd=simd if W > 1 else None)
+        g, gx = _global(gL, nl, prec, su3gen.FIELD_X)
+        _, gy = _global(gL, nl, prec, su3gen.FIELD_Y)
+
+        def slabs(gf):
+            out = []
+            for r in range(world):
+                m0, m1 = shard.matrix_range(gL, nl, r, world)
+                out.append(upload(d, oracle.convert(geom_of(d), geom_of(scalar_desc(d)), gf[m0 * 18:m1 * 18].copy())))
+            return out
+        xs, ys = slabs(gx), slabs(gy)
+        hub = halo.LoopbackComm(world)
+        sh = [halo.SlabShift(hub.for_rank(r)) for r in range(world)]
+        ps = halo.PeerShift()
+        zc = [su3.alloc_field(d) for _ in range(world)]
+        zm = [su3.alloc_field(d) for _ in range(world)]
+        disp = int(rng.integers(-2 * gL[3], 2 * gL[3] + 1))
+        st = [sh[r].start(ys[r], 3, disp) for r in range(world)]
+        for r in range(world):
+            sh[r].finish_cshift(zc[r], st[r])
+        st = [sh[r].start(ys[r], 3, disp) for r in range(world)]
+        for r in range(world):
+            sh[r].finish_mul_shift(zm[r], xs[r], st[r])
+        assert np.array_equal(_gather(d, zc), oracle.cshift(g, gy, 3, disp)), (it, gL, world, W, simd, disp)
+        e, _ = rel_err(_gather(d, zm), oracle.mul_shift(g, gx, gy, 3, disp), 1)
+        assert e <= TOL[prec], (it, gL, world, W, simd, disp, e)
+        if lL[3] > 1:
+            dp = int(rng.integers(-(lL[3] - 1), lL[3]))
+            for r in range(world):
+                ps.cshift(zc[r], ys[r], ys[(r + 1) % world], ys[(r - 1) % world], dp)
+                ps.mul_shift(zm[r], xs[r], ys[r], ys[(r + 1) % world], ys[(r - 1) % world], dp)
+            assert np.array_equal(_gather(d, zc), oracle.cshift(g, gy, 3, dp)), (it, gL, world, W, simd, dp)
+            e, _ = rel_err(_gather(d, zm), oracle.mul_shift(g, gx, gy, 3, dp), 1)
+            assert e <= TOL[prec], (it, gL, world, W, simd, dp, e)

@@ -86,13 +86,13 @@ def test_random_geometries_and_splits_fuzz():
     and Cshift bit-exact against the oracle, products within tolerance"""
     from gpu_util import scalar_desc
     rng = np.random.default_rng(77)
-    for it in range(40):
+    for it in range(80):
         W = int(2 ** rng.integers(0, 6))
         simd, w = [1, 1, 1, 1], W
         while w > 1:
             simd[int(rng.integers(0, 4))] *= 2
             w //= 2
-        L = tuple(int(s * rng.integers(1, 4)) for s in simd)
+        L = tuple(int(s * rng.integers(1, 4 if it < 40 else 9)) for s in simd)
         nl = int(rng.choice([1, 4]))
         prec = int(rng.choice([F64, F32]))
         desc = su3.make_desc(L, n_lorentz=nl, prec=prec, layout=VE, W=W, simd=simd)
@@ -106,9 +106,12 @@ def test_random_geometries_and_splits_fuzz():
         su3.su3_convert(back, fx)
         assert np.array_equal(download(back), xs), (L, W, simd)
         dim, disp = int(rng.integers(0, 4)), int(rng.integers(-5, 6))
+        su3.su3_tune_set(path=int(rng.choice([0, 0, 1, 2, 3])))          # any of the shift kernels
         su3.su3_cshift(fz, fx, dim, disp)
         assert np.array_equal(download(fz), oracle.cshift(g, x, dim, disp)), (L, W, simd, dim, disp)
+        su3.su3_tune_set(path=int(rng.choice([0, 0, 1, 2])))
         su3.su3_mul_shift(fz, fx, fy, dim, disp)
+        su3.su3_tune_set()
         err, _ = rel_err(download(fz), oracle.mul_shift(g, x, y, dim, disp), W)
         assert err <= TOL[prec], (L, W, simd, dim, disp, err)
         su3.su3_mul(fz, fx, fy)
