@@ -239,6 +239,43 @@ su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, in
 su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, int dim, int plane0, int nplanes, void *cuda_stream);
 su3_status su3_face_copy(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes, void *cuda_stream);
 
+/* Moving a face WITHOUT any device allocation by anybody.  su3_face_pack + su3_face_unpack need a packed buffer that
+ * somebody has to allocate; some users of this library cannot do that at the point where they need a face moved:
+ *   - a job whose framework has handed all of HBM to its own pool (a 64^4 run sized for the card, a torch process with
+ *     a fixed memory fraction): a cudaMalloc from a plug-in library fails there, or succeeds and fragments the pool;
+ *   - a communication thread that overlaps the face exchange with the bulk kernels of other streams: cudaMalloc and
+ *     cudaFree serialise against work in flight on the whole device, which is exactly the stall it exists to hide;
+ *   - an embedding (another language runtime, a sandboxed driver of this C ABI) that receives raw field pointers from
+ *     its host and owns no allocator handle at all.
+ * For them the library carries ONE fixed staging area of SU3_STATIC_SCRATCH_BYTES (16 MiB) inside its own device image
+ * -- a file-scope device array, so every GPU that loads libsu3stream holds these 16 MiB from the moment the module is
+ * loaded until the process exits, whether or not this call is ever used.
+ *
+ * su3_face_move_static: planes [z_plane0, +nplanes) of z along dim <- planes [x_plane0, +nplanes) of x, staged through
+ * that area in the packed plane order described above: two launches of the face kernel (field -> area, area -> field)
+ * on cuda_stream.  The result is bit-identical to su3_face_pack followed by su3_face_unpack through a buffer of the
+ * caller's.  z and x must agree in L, n_lorentz, precision and kind (SU3_ERR_MISMATCH) but, unlike su3_face_copy, NOT
+ * in layout: the packed order is the same for every layout, so a face may go from a vector-layout slab into a
+ * scalar-layout one.  z may be x itself (planes are copied inside one field; overlapping source and destination plane
+ * ranges are fine, the first launch has read everything before the second writes).  Both fields must live on the
+ * current device.  The caller passes only its input and output fields.
+ *   Limit   : a face of more than SU3_STATIC_SCRATCH_BYTES (su3_face_bytes tells) is refused with SU3_ERR_SIZE and
+ *             nothing is launched -- one x3 plane of a 48^4 fp64 colour-matrix field (15.9 MB) fits, one of 64^4
+ *             (37.7 MB) does not; move larger faces in several calls, or use su3_face_pack with your own buffer.
+ *   Set-up  : the first call on each device looks up the device address of the area (cudaGetSymbolAddress with that
+ *             device current; a failure is returned as SU3_ERR_CUDA).  That look-up may make the runtime load the
+ *             module, so make this first call -- any valid call, nplanes = 0 included -- during initialisation, before
+ *             any stream capture is begun in the process.  Later calls only launch kernels.
+ *   No alloc: no cudaMalloc, cudaFree, stream/event creation or other allocating routine is called, ever.
+ *   Sharing : all calls on one device use the same area and it keeps whatever the last call left in it.  Nothing in it
+ *             has to start at zero: every byte the second launch reads was written by the first launch of the same
+ *             call, so there is nothing to clear.  Calls that can overlap on the GPU -- on different streams, from
+ *             different threads or from different handles of the library in one process -- race on the area and may
+ *             deliver each other's faces: keep all calls of a device on one stream, or order them with events. */
+#define SU3_STATIC_SCRATCH_BYTES (16u << 20)
+su3_status su3_face_move_static(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes,
+                                void *cuda_stream);
+
 /* Cshift along x3 on one slab of an x3-split lattice with the neighbouring slab mapped into this process (peer memory
  * over NVLink, or simply another field on the same device): z[s] = X[s + disp*e3], X = the slab x continued by x_nbr --
  * the NEXT rank's slab for disp > 0, the PREVIOUS rank's for disp < 0; 0 < |disp| < L[3] of the slab (disp = 0 copies x;

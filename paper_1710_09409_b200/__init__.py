@@ -18,7 +18,8 @@ EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normali
            "su3_field_free", "su3_field_desc", "su3_field_ptr", "su3_index", "su3_mul", "su3_mul3",
            "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_expr_plan", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release",
-           "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy", "su3_cshift_slab"]
+           "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy", "su3_cshift_slab",
+           "su3_face_move_static"]
 
 
 class su3_desc(ctypes.Structure):
@@ -84,6 +85,7 @@ def _load():
         "su3_face_unpack": (i32, [vp, vp, sz, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_face_copy": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_cshift_slab": (i32, [vp, vp, vp, ctypes.c_int, vp]),
+        "su3_face_move_static": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -365,6 +367,22 @@ def su3_face_unpack(z, buf, dim, plane0, nplanes, stream=None):
 
 def su3_face_copy(z, z_plane0, x, x_plane0, dim, nplanes, stream=None):
     _ck(lib.su3_face_copy(z.handle, int(z_plane0), x.handle, int(x_plane0), int(dim), int(nplanes), _stream(stream)))
+
+
+SU3_STATIC_SCRATCH_BYTES = 16 << 20
+
+
+def su3_face_move_static(z, z_plane0, x, x_plane0, dim, nplanes, stream=None):
+    """planes [z_plane0, +nplanes) of z <- planes [x_plane0, +nplanes) of x along dim, staged through the 16 MiB area
+    that lives inside the library's device image -- for callers that cannot allocate device memory where they need a
+    face moved (all of HBM already belongs to a framework's pool, a communication thread that must not stall the device
+    in cudaMalloc/cudaFree, an embedding that owns no allocator).  Nothing is allocated here either: no tensor is
+    created, the arguments are passed through.  Same result as su3_face_pack + su3_face_unpack; z and x may differ in
+    layout and may be the same field.  Faces above SU3_STATIC_SCRATCH_BYTES raise Su3Error(SU3_ERR_SIZE).  Make the
+    first call per device during start-up, before any stream capture; calls that overlap on the GPU race on the shared
+    area (include/su3stream.h has the full contract)."""
+    _ck(lib.su3_face_move_static(z.handle, int(z_plane0), x.handle, int(x_plane0), int(dim), int(nplanes),
+                                 _stream(stream)))
 
 
 def su3_cshift_slab(z, x, x_nbr, disp, stream=None):

@@ -1183,6 +1183,53 @@ su3_status su3_face_copy(su3_field *z, int z_plane0, const su3_field *x, int x_p
   return launch_face_copy(z, z->ptr, false, z_plane0, x->ptr, false, x_plane0, dim, nplanes, stream);
 }
 
+// ---------------------------------------------------------------- face move for callers that cannot allocate
+// The packed staging buffer of the pack -> unpack route, owned by the library's device image instead of the caller
+// (su3stream.h says who needs that and why).  File scope, so each device that loads this module holds its own 16 MiB
+// copy until the process exits; uninitialised (.nv.global is NOBITS: the .so does not grow).
+static __device__ __align__(256) unsigned char g_static_scratch[SU3_STATIC_SCRATCH_BYTES];
+
+// Device address of g_static_scratch on the device that is current on the calling thread.  In host code the array's
+// name is only the runtime's handle for the symbol -- not an address a kernel may be given -- so the address is asked
+// for once per device ordinal, with that device current, and cached.  A failed look-up is not cached.
+static su3_status static_scratch_ptr(void **out) {
+  static void *table[MAX_DEVICES];  // zero-initialised: NULL = not looked up yet
+  static std::mutex mu;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail("cudaGetDevice", e);
+  if (dev < 0 || dev >= MAX_DEVICES) return fail(SU3_ERR_CUDA, "device ordinal %d outside 0..%d", dev, MAX_DEVICES - 1);
+  std::lock_guard<std::mutex> lk(mu);
+  if (!table[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess) return cuda_fail("cudaGetSymbolAddress(static face scratch)", e);
+    if (!p || (uintptr_t)p % 256) return fail(SU3_ERR_CUDA, "static face scratch resolved to an unusable address %p", p);
+    table[dev] = p;
+  }
+  *out = table[dev];
+  return SU3_OK;
+}
+
+su3_status su3_face_move_static(su3_field *z, int z_plane0, const su3_field *x, int x_plane0, int dim, int nplanes,
+                                void *stream) {
+  size_t need = 0, need_x = 0;
+  if (su3_status st = face_args(z, dim, z_plane0, nplanes, &need)) return st;
+  if (su3_status st = face_args(x, dim, x_plane0, nplanes, &need_x)) return st;
+  if (!same_lattice(z->d, x->d) || z->ncomp != x->ncomp)
+    return fail(SU3_ERR_MISMATCH, "su3_face_move_static needs fields of one lattice, precision and kind (layouts may differ)");
+  if (need > (size_t)SU3_STATIC_SCRATCH_BYTES)
+    return fail(SU3_ERR_SIZE, "the face has %zu bytes, the library's static staging area holds %zu: move fewer planes per call, "
+                "or use su3_face_pack / su3_face_unpack with a buffer of your own", need, (size_t)SU3_STATIC_SCRATCH_BYTES);
+  if (su3_status sd = on_current_device({z, x})) return sd;
+  void *area = nullptr;
+  if (su3_status st = static_scratch_ptr(&area)) return st;  // first call on this device: the one-time address look-up
+  // field -> area (plane order), then area -> field.  Stream order makes the second launch see the first one's bytes;
+  // every byte it reads is one the first launch wrote, so what an earlier call left in the area never matters.
+  if (su3_status st = launch_face_copy(x, area, true, 0, x->ptr, false, x_plane0, dim, nplanes, stream)) return st;
+  return launch_face_copy(z, z->ptr, false, z_plane0, area, true, 0, dim, nplanes, stream);
+}
+
 su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
                          su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream) {
   if (op != SU3_OP_MUL && op != SU3_OP_MUL3 && op != SU3_OP_MUL_ADD) return fail(SU3_ERR_INVALID, "op = %d not in {0,1,2}", op);
