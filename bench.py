@@ -827,19 +827,22 @@ def run_next_rows(args, r):
     return out
 
 
-def ncu_traffic(L):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel: NOT measured in this run (no
-    number is ever taken under a profiler here) but read from the committed ncu --set full summary, whose own header
-    names the command, the lattice and the commit it was captured at.  None if there is no capture for this L."""
+def ncu_traffic(L, row="A1"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of one kernel of the step (row A1, the dominant family, or
+    A5, the largest single kernel): NOT measured in this run (no number is ever taken under a profiler here) but read
+    from the committed ncu --set full summaries, whose headers name the command, the lattice and the commit they were
+    captured at.  A line `traffic_bytes_per_launch = N (L = ..)` is row A1's, `traffic_bytes_per_launch[A5] = N (..)` row
+    A5's; the newest round's file wins.  None if there is no capture for this L."""
     import glob
     import re
-    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_pipe_kernel_full.md")), reverse=True):
+    tag = r"" if row == "A1" else r"\[%s\]" % re.escape(row)
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_full.md")), reverse=True):
         text = open(path).read()
-        m = re.search(r"traffic_bytes_per_launch\s*=\s*(\d+)\s*\(L\s*=\s*(\d+),\s*captured at commit ([0-9a-f]+), ([^)]*)\)", text)
-        if m and int(m.group(2)) == L:
-            return int(m.group(1)), "%s: ncu --set full capture at commit %s (%s); not re-measured in this run" % (
-                os.path.relpath(path, ROOT), m.group(3), m.group(4))
-    return None, "no committed ncu --set full capture for L = %d" % L
+        for m in re.finditer(r"traffic_bytes_per_launch" + tag + r"\s*=\s*(\d+)\s*\(L\s*=\s*(\d+),\s*captured at commit ([0-9a-f]+), ([^)]*)\)", text):
+            if int(m.group(2)) == L:
+                return int(m.group(1)), "%s: ncu --set full capture at commit %s (%s); not re-measured in this run" % (
+                    os.path.relpath(path, ROOT), m.group(3), m.group(4))
+    return None, "no committed ncu --set full capture of row %s for L = %d" % (row, L)
 
 
 def profile_pass(args):
@@ -982,7 +985,9 @@ def main():
                                         else "cudaDevAttrMemoryClockRate x 2 x bus / 8",
                 "pin_rate_peak_cuda_attr": pin_attr,
                 "pin_rate_peak_cuda_attr_source": "cudaDevAttrMemoryClockRate %.0f MHz x 2 x %d bit / 8" % (r["info"]["mem_clock_khz"] / 1e3, bus),
-                "traffic": traffic, "traffic_source": traffic_src}
+                "traffic": traffic, "traffic_source": traffic_src,
+                "traffic_by_kernel": {row: dict(zip(("traffic", "source"), ncu_traffic(args.L, row)), algorithmic_bytes=nb)
+                                      for row, nb in (("A1", 3 * B), ("A5", 2 * B))}}
     cpu = None
     if rank == 0 and not args.no_cpu:
         cpu = run_cpu_baseline(args, r["host"])
@@ -1012,7 +1017,91 @@ def main():
                           "z=x*y with coalesced_ptr (AoS -> AoSoAoS)": "saturates the memory bandwidth (~240 GB/s)",
                           "vector layout on GP100/V100": "follows the STREAM triad; plateau only at 16 threads per block (P:199-203)"},
     }
-    print(json.dumps(line), flush=True)
+    emit(line)
+
+
+def _compact(v, digits=6):
+    """floats to `digits` significant digits, NaN/inf to None (strict JSON), containers recursively"""
+    if isinstance(v, float):
+        if v != v or v in (float("inf"), float("-inf")):
+            return None
+        return float("%.*g" % (digits, v))
+    if isinstance(v, dict):
+        return {k: _compact(x, digits) for k, x in v.items()}
+    if isinstance(v, (list, tuple)):
+        return [_compact(x, digits) for x in v]
+    return v
+
+
+HEADLINE_KEYS = ("metric", "value", "unit", "n_gpus", "gpu", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                 "vs_baseline", "dtype", "data", "gpu_launches", "config", "clocks", "checks", "roofline", "cpu_baseline",
+                 "e2e", "bar", "GFLOPps", "detail")
+HEADLINE_MAX_BYTES = 4096
+
+
+def headline(line):
+    """The record the driver parses: the contract keys, `roofline` (A1, the dominant kernel family, at top level as the
+    contract asks; A1 and the largest single kernel A5 side by side under `kernels`), `cpu_baseline`, `e2e` and a digest
+    of the north_star bar (z = x*y at 48^4 and 64^4, GB/s and fraction of the same-size copy) -- under 4 KB.  Everything
+    else (sweep, ceilings, W sweep, next rows, per-config CPU points, paper context) is the detail record."""
+    pick = lambda d, keys: {k: d[k] for k in keys if d is not None and k in d}
+    ops = {o["row"]: o for o in line.get("ops") or []}
+    roof = line.get("roofline") or {}
+    kernels = []
+    for row, name, nbytes_key in (("A1", "su3_pipe_kernel<double,1,OP_MUL> z=x*y", "A1"), ("A5", "su3_convert_tma_kernel<double2,4> scalar->vector", "A5")):
+        o = next((v for k, v in ops.items() if k.startswith(row)), None)
+        if o is None:
+            continue
+        t = (roof.get("traffic_by_kernel") or {}).get(row) or {}
+        kernels.append({"row": row, "kernel": name, "achieved": o["GBps"], "peak": roof.get("peak"),
+                        "frac": o["frac_of_measured_peak"], "frac_of_same_run_copy": o["frac_of_copy"],
+                        "avg_launch_ms": o["ms"], "algorithmic_bytes_per_launch": t.get("algorithmic_bytes"),
+                        "traffic": t.get("traffic"), "traffic_source": t.get("source")})
+    roofline = pick(roof, ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "traffic_source", "peak_source",
+                           "algorithmic_bytes_per_launch", "avg_launch_ms", "frac_of_same_run_copy", "pin_rate_peak"))
+    roofline["kernels"] = kernels
+    cpu = line.get("cpu_baseline")
+    if cpu is not None:
+        cpu = dict(pick(cpu, ("value", "unit", "cores", "kind", "sample", "ms_per_step", "stream_triad_GBps")),
+                   one_thread_GBps=(cpu.get("one_thread") or {}).get("GBps"))
+    e2e = line.get("e2e")
+    if e2e is not None:
+        e2e = dict(pick(e2e, ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "steps", "api",
+                              "host_result_matches_device")),
+                   host_result_vs_oracle_sampled_ok=(e2e.get("host_result_vs_oracle_sampled") or {}).get("ok"))
+    bar = {"%d^4 %s %s" % (p["L"], p["prec"], p["layout"]): [p["GBps"], p.get("frac_of_copy")]
+           for p in line.get("sweep") or [] if p.get("L") in (48, 64)}
+    head = {k: line.get(k) for k in HEADLINE_KEYS if k in line}
+    head.update({"roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                 "bar": {"what": "z=x*y: [GB/s, fraction of the same-run same-size copy]; north_star bar 0.85", "points": bar},
+                 "detail": "stderr line 'DETAIL {json}' and gpurun_out/bench_detail.json"})
+    head = _compact(head)
+    for k in head["roofline"]["kernels"] + [head["roofline"]]:     # provenance strings: the profile file says the rest
+        if isinstance(k.get("traffic_source"), str) and len(k["traffic_source"]) > 160:
+            k["traffic_source"] = k["traffic_source"][:157] + "..."
+    if len(json.dumps(head, allow_nan=False)) > HEADLINE_MAX_BYTES:  # never let prose push the record over the limit
+        for obj, key in ((head["roofline"], "traffic_source"), (head["roofline"], "peak_source"), (head.get("e2e") or {}, "api"),
+                         (head.get("cpu_baseline") or {}, "sample"), (head["config"], "workload")):
+            if isinstance(obj.get(key), str) and len(obj[key]) > 120:
+                obj[key] = obj[key][:117] + "..."
+        for k in head["roofline"]["kernels"]:
+            if isinstance(k.get("traffic_source"), str):
+                k["traffic_source"] = k["traffic_source"][:80]
+    return head
+
+
+def emit(line):
+    """stdout: ONE compact line (the headline record, strict JSON, < 4 KB).  stderr and gpurun_out/: the full record."""
+    detail = json.dumps(_compact(line, 9), allow_nan=False)
+    print("DETAIL " + detail, file=sys.stderr, flush=True)
+    try:
+        out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "gpurun_out")
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, "bench_detail.json"), "w") as f:
+            f.write(detail + "\n")
+    except OSError as e:
+        log("note: could not write gpurun_out/bench_detail.json: %s" % e)
+    print(json.dumps(headline(line), allow_nan=False), flush=True)
 
 
 if __name__ == "__main__":
