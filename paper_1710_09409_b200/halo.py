@@ -116,12 +116,19 @@ class CudaOps:
 
 class SlabShift:
     """Cshift / shifted product along any dimension for one rank's slab.  Buffers for the faces (and, for shifts by a
-    whole slab or more, one scratch slab) are allocated once per size and reused."""
+    whole slab or more, one scratch slab) are allocated once per size and reused.
+
+    Because the buffers are shared by every shift of same-shaped fields, only ONE exchanging shift per field shape may
+    be between start() and its finish_*(): a second start() would overwrite the send buffer while the first send may
+    still be running, and the receive buffer before the first unpack.  start() raises RuntimeError in that case instead
+    of corrupting the first shift; finish the first one (or use a second SlabShift object, which has its own buffers).
+    Shifts that need no exchange (another dimension, or one rank) are not restricted."""
 
     def __init__(self, comm, ops=None):
         self.comm = comm
         self.ops = ops if ops is not None else CudaOps()
         self._buf = {}
+        self._in_flight = set()
 
     def _cached(self, key, make):
         if key not in self._buf:
@@ -134,7 +141,11 @@ class SlabShift:
         if dim != shard.SLAB_DIM or c.world == 1:
             return {"local": True, "dim": dim, "disp": disp, "y": y}
         plan = shard.cshift_plan(o.l3(y), c.rank, c.world, disp)
-        st = {"local": False, "plan": plan, "src": y, "works": [], "bulk_works": []}
+        if o.key(y) in self._in_flight:
+            raise RuntimeError("SlabShift: a shift of a field of this shape is still between start() and finish_*(); "
+                               "its face buffers are shared -- finish it first, or use another SlabShift object")
+        self._in_flight.add(o.key(y))
+        st = {"local": False, "plan": plan, "src": y, "works": [], "bulk_works": [], "key": o.key(y)}
         n = plan["nface"]
         if n:
             sbuf = self._cached(("send", n, o.key(y)), lambda: o.face_buffer(y, n))
@@ -165,15 +176,22 @@ class SlabShift:
             w.wait()
         if plan["nface"]:
             o.face_unpack(z, st["halo"], plan["dst_plane0"], plan["nface"])
+        self._in_flight.discard(st["key"])
 
     def finish_mul_shift(self, z, x, st):
         """Phase 2: z[s] = x[s] . y[s + disp*dim_hat] on the GLOBAL lattice.  The bulk is one su3_mul_shift (or su3_mul)
-        on the slab; the face is x's planes times the received planes, by su3_mul on the packed (scalar-layout) faces."""
+        on the slab; the face is x's planes times the received planes, by su3_mul on the packed (scalar-layout) faces.
+        z may be x (su3stream.h allows it for the product): x's face planes are packed BEFORE the bulk kernel runs,
+        because with z = x that kernel overwrites them with products of the wrongly wrapped planes."""
         o = self.ops
         if st["local"]:
             o.mul_shift(z, x, st["y"], st["dim"], st["disp"])
             return
         plan = st["plan"]
+        n = plan["nface"]
+        if n:
+            xb = self._cached(("xface", n, o.key(x)), lambda: o.face_buffer(x, n))
+            o.face_pack(xb, x, plan["dst_plane0"], n)
         for w in st["bulk_works"]:
             w.wait()
         if plan["shift"]:
@@ -182,13 +200,11 @@ class SlabShift:
             o.mul(z, x, st["src"])
         for w in st["works"]:
             w.wait()
-        n = plan["nface"]
         if n:
-            xb = self._cached(("xface", n, o.key(x)), lambda: o.face_buffer(x, n))
             zb = self._cached(("zface", n, o.key(x)), lambda: o.face_buffer(x, n))
-            o.face_pack(xb, x, plan["dst_plane0"], n)
             o.face_mul(zb, xb, st["halo"], x, n)
             o.face_unpack(z, zb, plan["dst_plane0"], n)
+        self._in_flight.discard(st["key"])
 
     def cshift(self, z, y, dim, disp):
         self.finish_cshift(z, self.start(y, dim, disp))
@@ -216,15 +232,16 @@ class PeerShift:
 
     def mul_shift(self, z, x, y, y_next, y_prev, disp):
         """z[s] = x[s] . Y[s + disp*e3]: the periodic product on the slab, then the |disp| wrapped planes again as
-        su3_mul on packed faces -- x's planes times the neighbour's planes, packed straight out of its memory."""
+        su3_mul on packed faces -- x's planes times the neighbour's planes, packed straight out of its memory.
+        z may be x: x's face is packed before the bulk kernel overwrites those planes."""
         su3 = self.su3
-        su3.su3_mul_shift(z, x, y, shard.SLAB_DIM, disp)
         n = abs(disp)
-        if n == 0:
-            return
         l3 = x.desc.L[shard.SLAB_DIM]
-        if n >= l3:
+        if n >= l3:                                                # checked before anything is launched
             raise ValueError("|disp| = %d must be below the slab's %d planes" % (n, l3))
+        if n == 0:
+            su3.su3_mul_shift(z, x, y, shard.SLAB_DIM, 0)
+            return
         nbr = y_next if disp > 0 else y_prev
         dst0, src0 = (l3 - n, 0) if disp > 0 else (0, l3 - n)
         nb = su3.su3_face_bytes(x, shard.SLAB_DIM, n)
@@ -233,6 +250,7 @@ class PeerShift:
             self._buf[key] = [self.torch.empty(nb, dtype=self.torch.uint8, device=x.tensor.device) for _ in range(3)]
         xb, hb, zb = self._buf[key]
         su3.su3_face_pack(xb, x, shard.SLAB_DIM, dst0, n)
+        su3.su3_mul_shift(z, x, y, shard.SLAB_DIM, disp)
         su3.su3_face_pack(hb, nbr, shard.SLAB_DIM, src0, n)
         L = tuple(x.desc.L)
         d = su3.make_desc((L[0], L[1], L[2], n), n_lorentz=x.desc.n_lorentz, prec=x.desc.prec)

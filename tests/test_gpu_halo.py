@@ -132,6 +132,16 @@ def test_sharded_shifts_equal_the_oracle_on_the_global_lattice(prec, world, gL, 
             su3.su3_mul(t, xs[r], zc[r])
             torch.cuda.synchronize()
             assert torch.equal(t.tensor, zm[r].tensor), (dim, disp, r)
+        # in place (z is x, which su3stream.h allows for the product): x's face is packed before the bulk kernel
+        xi = [su3.alloc_field(d) for _ in range(world)]
+        for r in range(world):
+            xi[r].tensor.copy_(xs[r].tensor)
+        st = [sh[r].start(ys[r], dim, disp) for r in range(world)]
+        for r in range(world):
+            sh[r].finish_mul_shift(xi[r], xi[r], st[r])
+        torch.cuda.synchronize()
+        for r in range(world):
+            assert torch.equal(xi[r].tensor, zm[r].tensor), ("z is x", dim, disp, r)
 
 
 @pytest.mark.parametrize("prec", [su3.SU3_F64, su3.SU3_F32])
@@ -168,6 +178,13 @@ def test_peer_mapped_slabs_one_kernel_exchange(prec, world, gL, nl, W, simd):
             if disp != 0:
                 assert su3.su3_launch_count() - n0 == (1 if fused else 2)
             ps.mul_shift(zm[r], xs[r], ys[r], nxt, prv, disp)
+            xi = su3.alloc_field(d)
+            xi.tensor.copy_(xs[r].tensor)
+            ps.mul_shift(xi, xi, ys[r], nxt, prv, disp)            # in place: z is x
+            torch.cuda.synchronize()
+            assert torch.equal(xi.tensor, zm[r].tensor), ("z is x", disp, r)
+        with pytest.raises(ValueError):
+            ps.mul_shift(zm[0], xs[0], ys[0], ys[1 % world], ys[-1 % world], l3)   # refused before any launch
         assert np.array_equal(_gather(d, zc), oracle.cshift(g, gy, 3, disp)), disp
         e, _ = rel_err(_gather(d, zm), oracle.mul_shift(g, gx, gy, 3, disp), 1)
         assert e <= TOL[prec], (disp, e)

@@ -130,6 +130,9 @@ def _worker(rank, world, port, gL, nl, W, disps, out_dir):
             zc, zm = _F(g, np.zeros_like(x.a)), _F(g, np.zeros_like(x.a))
             sh.cshift(zc, y, dim, disp)
             sh.mul_shift(zm, x, y, dim, disp)
+            xi = _F(g, x.a.copy())
+            sh.mul_shift(xi, xi, y, dim, disp)                     # in place: z is x (allowed for the product)
+            np.save(os.path.join(out_dir, "i%d_%d.npy" % (k, rank)), oracle.convert(gs, g, xi.a))
             np.save(os.path.join(out_dir, "c%d_%d.npy" % (k, rank)), oracle.convert(gs, g, zc.a))
             np.save(os.path.join(out_dir, "m%d_%d.npy" % (k, rank)), oracle.convert(gs, g, zm.a))
         dist.barrier()
@@ -153,3 +156,29 @@ def test_sharded_shift_equals_global_shift(tmp_path, world, gL, nl, W):
         got_m = np.concatenate([np.load(tmp_path / ("m%d_%d.npy" % (k, r))) for r in range(world)])
         assert np.array_equal(got_c, want_c), (dim, disp)
         assert np.array_equal(got_m, want_m), (dim, disp)
+        got_i = np.concatenate([np.load(tmp_path / ("i%d_%d.npy" % (k, r))) for r in range(world)])
+        assert np.array_equal(got_i, want_m), ("z is x", dim, disp)
+
+
+def test_second_start_before_finish_is_refused():
+    """the face buffers are cached per field shape: two shifts of same-shaped fields in flight would share them, so the
+    second start() raises instead of corrupting the first; after the matching finish a new shift may start"""
+    gL, world = (2, 2, 2, 8), 2
+    g, gx, gy = _fields(gL, 1)
+    hub = halo.LoopbackComm(world)
+    sh = [halo.SlabShift(hub.for_rank(r), ops=OracleOps()) for r in range(world)]
+    ys, zs = [], []
+    for r in range(world):
+        m0, m1 = shard.matrix_range(gL, 1, r, world)
+        gl = oracle.Geom(shard.local_extents(gL, r, world)[0], nl=1)
+        ys.append(_F(gl, gy[m0 * 18:m1 * 18].copy()))
+        zs.append(_F(gl, np.zeros(ys[-1].a.shape)))
+    for _ in range(2):                                             # the guard is released by finish_*: a second round works
+        st = [sh[r].start(ys[r], 3, 1) for r in range(world)]
+        with pytest.raises(RuntimeError, match="finish"):
+            sh[0].start(ys[0], 3, -1)
+        local = sh[0].start(ys[0], 1, 1)                           # no exchange: never restricted
+        sh[0].finish_cshift(_F(ys[0].g, np.zeros(ys[0].a.shape)), local)
+        for r in range(world):
+            sh[r].finish_cshift(zs[r], st[r])
+        assert np.array_equal(np.concatenate([z.a for z in zs]), oracle.cshift(g, gy, 3, 1))
