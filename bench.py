@@ -707,13 +707,26 @@ def run_ceilings_and_sweep(args, r):
                             su3.su3_mul(z_, x_, y_)
                         cmn, _, _ = time_calls(torch, rot, target_ms=4.0, warm=ntrip, graph_below_us=60.0)
                         cold = 3 * nb / (cmn * 1e-3) / 1e9
+                pl = su3.su3_launch_plan(d, 0)                      # the library's automatic choice at this point
+                plan = pl["family"] if pl["family"] != "pipe" else "pipe tile %d depth %d l2 %s" % (
+                    pl["tile"], pl["depth"], "pin %.1f MB/operand" % (pl["pin_bytes"] / 1e6) if pl["l2"] == "pin" else pl["l2"])
                 sweep.append({"L": Ls, "prec": "f64" if prec == 8 else "f32", "layout": "scalar" if layout == 0 else "vector",
-                              "W": W, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3, "issued": how,
+                              "W": W, "plan": plan, "footprint_MB": 3 * nb / 1e6, "us_min": mn * 1e3, "us_median": md * 1e3, "issued": how,
                               "GBps": gbs, "GFLOPps": FLOPS["mul"] * Ls ** 4 / (mn * 1e-3) / 1e9, "regime": regime, "cold_GBps": cold,
                               # against the SAME-SIZE ceilings of this run (warm: best of su3_copy / D2D; and the 2r1w add)
                               "frac_of_copy": gbs / c["best_copy"], "frac_of_add_2r1w": gbs / c["su3_add_2r1w"],
                               "cold_frac_of_copy": cold / c["su3_copy_cold"] if cold and c.get("su3_copy_cold") else None})
     out["by_size"] = by_size
+    # The denominator of the latency-bound ramp (Fig. 3's left end): the library's smallest launch -- z = x*y on
+    # a 2^4 lattice, 16 matrices, one block -- issued from the stream and replayed from a CUDA graph.  What an 8^4-16^4
+    # call costs beyond this is the kernel's own time; the floor itself is launch latency, not the library's.
+    d0 = su3.make_desc(2)
+    nb0 = su3.su3_field_bytes(d0)
+    f0 = [su3.su3_field_wrap(d0, t.tensor[:nb0]) for t in (f["zc"], f["xs"], f["ys"])]
+    fl_stream, _, _ = time_calls(torch, lambda: su3.su3_mul(*f0))
+    fl_graph, _, how = time_calls(torch, lambda: su3.su3_mul(*f0), graph_below_us=1e9)
+    out["launch_floor_us"] = {"what": "su3_mul on a 2^4 lattice (16 matrices): the cost of one launch of this library",
+                              "stream": fl_stream * 1e3, "graph_replay": fl_graph * 1e3, "graph": how}
     return out, sweep
 
 
@@ -1007,7 +1020,8 @@ def main():
                    "parallelism": "independent x3 slabs, no collective" if world > 1 else "single GPU"},
         "GFLOPps": world * r["step_flops"] / (r["ms_per_step"] * 1e-3) / 1e9,
         "gpu_launches": r["launches"], "clocks": r["clk"], "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
-        "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k not in ("wsweep", "by_size", "convert_f32")},
+        "ops": ops, "ceilings_GBps": {k: v for k, v in ceilings.items() if k not in ("wsweep", "by_size", "convert_f32", "launch_floor_us")},
+        "launch_floor_us": ceilings.get("launch_floor_us"),
         "ceilings_by_size": ceilings.get("by_size"), "convert_f32": ceilings.get("convert_f32"),
         "wsweep": ceilings.get("wsweep"), "next_rows": next_rows, "halo": halo_leg, "sweep": sweep, "checks": r["checks"],
         "wall_s_timed_region": r["t_wall"],

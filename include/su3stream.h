@@ -305,6 +305,18 @@ typedef enum { SU3_OP_MUL = 0, SU3_OP_MUL3 = 1, SU3_OP_MUL_ADD = 2 } su3_op;
 su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y_host, const void *u_host,
                          su3_field *zd, su3_field *xd, su3_field *yd, su3_field *ud, int chunks, void *cuda_stream);
 
+/* Which launch su3_mul / su3_mul3 / su3_mul_add (op = su3_op) would make on fields of this descriptor, with the calling
+ * thread's knobs (su3_tune_set) on the current device -- the library picks kernel family, tile, ring depth and L2 policy
+ * from the footprint (3 or 4 fields) against the L2 size, and this call reports that choice without launching anything:
+ *   "<family> tile=<matrices> depth=<ring depth> ctas=<per SM> grid=<blocks> block=<threads> smem=<bytes> l2=<policy> pin_bytes=<n>"
+ * family: "direct" (per-lane loads, L2-resident vector layouts), "warp" (warp-staged, L2-resident), "pipe" (the TMA
+ * pipeline); l2: "none", "evict_first", or "pin" = the first pin_bytes of every operand are kept in L2 from call to call
+ * (evict_last) and the rest is streamed -- chosen automatically between 0.6 and 2 x L2 for repeated calls on the same
+ * fields (the loop of Listing 3), never for the chunk launches of su3_eval_host nor for shifted operands.
+ * Written NUL-terminated into buf (SU3_ERR_SIZE if it does not fit).  Host arithmetic only, but it needs the current
+ * device's facts: SU3_ERR_CUDA without a device.  For bench.py's sweep rows and for the tests. */
+su3_status su3_launch_plan(const su3_desc *desc, int op, char *buf, size_t buf_len);
+
 /* Destroys the copy streams and events that su3_mul_host / su3_eval_host created (after waiting for their own
  * copies).  Optional teardown; must not run concurrently with those two calls.  At most 64 distinct
  * (device, stream) pairs may hold such resources at a time (SU3_ERR_SIZE beyond that). */

@@ -19,7 +19,7 @@ EXPORTS = ["su3_last_error", "su3_version", "su3_field_bytes", "su3_desc_normali
            "su3_mul_add", "su3_add", "su3_expr", "su3_expr_cost", "su3_expr_disasm", "su3_expr_plan", "su3_cshift", "su3_mul_shift", "su3_real_bytes", "su3_real_wrap", "su3_fill", "su3_vec_bytes", "su3_vec_wrap", "su3_vec_index", "su3_matvec", "su3_convert", "su3_copy", "su3_mul_host", "su3_eval_host", "su3_tune_set",
            "su3_tune_get", "su3_launch_count", "su3_device_info", "su3_device_name", "su3_host_release",
            "su3_face_bytes", "su3_face_pack", "su3_face_unpack", "su3_face_copy", "su3_cshift_slab",
-           "su3_face_move_static"]
+           "su3_face_move_static", "su3_launch_plan"]
 
 
 class su3_desc(ctypes.Structure):
@@ -85,6 +85,7 @@ def _load():
         "su3_face_unpack": (i32, [vp, vp, sz, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_face_copy": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
         "su3_cshift_slab": (i32, [vp, vp, vp, ctypes.c_int, vp]),
+        "su3_launch_plan": (i32, [D, ctypes.c_int, ctypes.c_char_p, sz]),
         "su3_face_move_static": (i32, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp]),
     }
     for name, (res, args) in sig.items():
@@ -367,6 +368,19 @@ def su3_face_unpack(z, buf, dim, plane0, nplanes, stream=None):
 
 def su3_face_copy(z, z_plane0, x, x_plane0, dim, nplanes, stream=None):
     _ck(lib.su3_face_copy(z.handle, int(z_plane0), x.handle, int(x_plane0), int(dim), int(nplanes), _stream(stream)))
+
+
+def su3_launch_plan(desc, op=0):
+    """the launch su3_mul (op 0) / su3_mul3 (1) / su3_mul_add (2) would make for this descriptor, as a dict:
+    family ("direct" | "warp" | "pipe"), tile, depth, ctas, grid, block, smem, l2 ("none" | "evict_first" | "pin"), pin_bytes"""
+    buf = ctypes.create_string_buffer(256)
+    _ck(lib.su3_launch_plan(ctypes.byref(desc), int(op), buf, len(buf)))
+    words = buf.value.decode().split()
+    out = {"family": words[0]}
+    for w in words[1:]:
+        k, v = w.split("=")
+        out[k] = v if k == "l2" else int(v)
+    return out
 
 
 SU3_STATIC_SCRATCH_BYTES = 16 << 20

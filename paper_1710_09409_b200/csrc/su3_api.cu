@@ -164,18 +164,31 @@ su3_status on_current_device(std::initializer_list<const su3_field *> fs) {
   return SU3_OK;
 }
 
-// Launch one ahead-of-time program (su3_kernels.cuh: menu_prog(op)) over `nmat` matrices starting at the given
-// pointers; `sh` != NULL: the last operand is read at the shifted site (pipeline only).
-su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in, int64_t nmat,
-                         size_t footprint_bytes, cudaStream_t stream, const su3::ShiftInfo *sh = nullptr) {
-  const DevInfo &di = devinfo();
-  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
-  if (nmat == 0) return SU3_OK;
-  const su3_tune tn = g_tune;
+// What launch_stream will launch for (op, prec, W, nmat, footprint) with the knobs `tn` on the device `di`: kernel
+// family, geometry, ring depth and L2 policy.  Host arithmetic only, so that su3_launch_plan can report exactly the
+// choice the arithmetic calls make.
+struct StreamPlan {
+  int family = 0;         // su3tab::FAM_PIPE / FAM_DIRECT / FAM_WARP
+  unsigned grid = 0;
+  int block = 0;
+  size_t smem = 0;
+  int tile_mats = 0, stages = 0, ctas = 0;
+  int hint = 0;           // StreamParams::hint: 0 none, 1 evict_first, 2 pinned prefix (evict_last) + streamed rest
+  int64_t pin_tiles = 0;
+  size_t pin_bytes = 0;   // per operand
+};
+
+// shifted: the last operand is read at the shifted site (pipeline only).  one_shot: the operands were just written
+// and no repeat of this call on the same pointers is expected (the chunk launches of su3_eval_host, whose data has
+// just arrived from the host and is never re-read): the automatic pinned-prefix L2 policy, which pays only when the
+// same call is repeated back to back (Listing 3's loop), is then not applied.  Shifted launches do not get it
+// automatically either.  l2_hint = 3 still asks for it explicitly in every case.
+su3_status plan_stream(int op, int prec, int W, int64_t nmat, size_t footprint_bytes, bool shifted, bool one_shot,
+                       const su3_tune &tn, const DevInfo &di, StreamPlan *pl) {
   const int nin = su3::menu_prog(op).nin;
-  const int nslot = (sh && nin == 1) ? 2 : nin;
+  const int nslot = (shifted && nin == 1) ? 2 : nin;
   const int cb = 2 * prec;
-  const bool base_op = op <= su3::OP_ADD && !sh;  // the direct and warp-staged kernels exist for su3_mul/mul3/mul_add(/add) only
+  const bool base_op = op <= su3::OP_ADD && !shifted;  // the direct and warp-staged kernels exist for su3_mul/mul3/mul_add(/add) only
   // auto path: the TMA pipeline everywhere, except L2-resident problems in a vector layout whose element
   // vectors fill whole sectors (W*c >= 32 B): there the per-lane loads are already sector-perfect and the
   // pipeline's fixed latency (barrier set-up, two smem hops) is what one measures
@@ -185,10 +198,96 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
   const bool direct = base_op && op != su3::OP_ADD &&  // OP_ADD has no direct kernel (su3_add's path = 2 is its own plain kernel)
                       (tn.path == 2 || (tn.path == 0 && W * cb >= 32 && footprint_bytes <= (size_t)di.l2 * 6 / 10));
   const bool warp = base_op && !direct && (tn.path == 3 || (tn.path == 0 && footprint_bytes <= (size_t)di.l2 / 2));
-  const int family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
+  pl->family = warp ? su3tab::FAM_WARP : (direct ? su3tab::FAM_DIRECT : su3tab::FAM_PIPE);
+  if (warp) {
+    pl->tile_mats = 32;
+    const int64_t nwt = (nmat + 31) / 32;
+    int wpb = 4;  // warps per block; fewer on small lattices so that every SM gets a block
+    while (wpb > 1 && (nwt + wpb - 1) / wpb < 2 * (int64_t)di.sms) wpb >>= 1;
+    pl->smem = (size_t)wpb * nin * 288 * cb;
+    const int64_t blocks_needed = (nwt + wpb - 1) / wpb;
+    const int64_t cap = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 8) * (4 / wpb);
+    pl->grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
+    pl->block = wpb * 32;
+    return SU3_OK;
+  }
+  if (direct) {
+    int bs = 256;  // small lattices: smaller blocks so that every SM gets one
+    while (bs > 32 && (nmat + bs - 1) / bs < 2 * (int64_t)di.sms) bs >>= 1;
+    const int64_t blocks_needed = (nmat + bs - 1) / bs;
+    const int64_t cap = (int64_t)di.sms * 8 * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 1) * (256 / bs);
+    pl->grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
+    pl->block = bs;
+    return SU3_OK;
+  }
+  // defaults measured on B200: 9 KB operand slots (64 fp64 / 128 fp32 matrices),
+  // a 3-deep ring, 2 persistent CTAs per SM
+  // 2 persistent CTAs per SM; 3 for the copy through a shifted slot (Cshift of 72-byte records with odd run boundaries:
+  // no arithmetic to hide behind, measured 0.81 -> 0.96 x copy)
+  int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (shifted && nin == 1 ? 3 : 2);
+  int tm = tn.tile_mats;
+  if (tm == 0) {
+    tm = 9216 / (9 * cb);
+    // small lattices: shrink the tile until every persistent CTA has at least two tiles
+    while (tm > 32 && (nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
+  }
+  if (tm != 32 && tm != 64 && tm != 128) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128}", tm);
+  const size_t stage_bytes = (size_t)nslot * tm * 9 * cb + (shifted ? 16 : 0);
+  // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
+  size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+  // auto CTAs/SM: a big tile may leave room for fewer resident CTAs than the default
+  while (tn.ctas_per_sm == 0 && ctas > 1 && (budget - 256) / stage_bytes < 2) {
+    ctas--;
+    budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
+  }
+  const int64_t max_grid = (int64_t)di.sms * ctas;
+  int stages = tn.stages;
+  if (stages == 0) {
+    // ring depth 3 at HBM-bound sizes (deeper rings open more DRAM pages at once and measured 1-3 % slower from 40^4
+    // fp32 / 36^4 fp64 on); up to 3 x L2 a good part of the loads hits L2, latency rather than DRAM limits a 20-70 us
+    // launch, and more bytes in flight pay: depth 4 measured +4..12 % at 20^4-28^4 fp64 and 24^4-36^4 fp32 (ncu at
+    // 24^4 with depth 3, warm: DRAM 44 % busy, profiles/r02_knee.md)
+    stages = footprint_bytes <= (size_t)di.l2 * 3 ? 4 : 3;
+    while (stages > 2 && stages * stage_bytes + 256 > budget) stages--;
+  }
+  if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);
+  pl->smem = stages * stage_bytes + 3 * stages * sizeof(uint64_t);
+  if (pl->smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "pipeline needs %zu B of shared memory, device allows %d", pl->smem, di.smem_optin);
+  pl->tile_mats = tm; pl->stages = stages; pl->ctas = ctas;
+  // L2 policy (l2_hint): 0/1 none (evict_first measured neutral at every HBM-bound size), 2 evict_first
+  // everywhere, 3 keep the first l2_pin_mb MB of every operand in L2 (evict_last) and stream the rest (evict_first)
+  pl->hint = tn.l2_hint == 2 ? 1 : (tn.l2_hint == 3 ? 2 : 0);
+  pl->pin_bytes = (size_t)tn.l2_pin_mb * 1000000;   // per operand
+  if (tn.l2_hint == 0 && !one_shot && !shifted && footprint_bytes > (size_t)di.l2 * 6 / 10 && footprint_bytes <= (size_t)di.l2 * 2) {
+    // auto, footprint between 0.6 and 2 x L2 ("straddling"): a plain LRU keeps NOTHING of a cyclic sweep that is a
+    // little larger than the cache; keeping ~36 % of L2 worth of operand prefixes resident from one call to the next
+    // (Listing 3 repeats z = x*y on the same fields) and streaming the rest measured +32 % at 24^4 fp64, +7 % at
+    // 32^4 fp32; beyond 2 x L2 the same policy costs 2-4 %, so it is not applied there.  It helps only a call that is
+    // repeated on the same pointers: not applied to one-shot chunk launches and to shifted launches (see above)
+    pl->hint = 2;
+    pl->pin_bytes = (size_t)di.l2 * 36 / 100 / nin;
+  }
+  if (pl->hint == 2) pl->pin_tiles = (int64_t)(pl->pin_bytes / ((size_t)tm * 9 * cb));
+  else pl->pin_bytes = 0;
+  const int64_t ntiles = (nmat + tm - 1) / tm;
+  pl->grid = (unsigned)(ntiles < max_grid ? ntiles : max_grid);
+  pl->block = (NCW + 1) * 32;
+  return SU3_OK;
+}
+
+// Launch one ahead-of-time program (su3_kernels.cuh: menu_prog(op)) over `nmat` matrices starting at the given
+// pointers; `sh` != NULL: the last operand is read at the shifted site (pipeline only).
+su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in, int64_t nmat,
+                         size_t footprint_bytes, cudaStream_t stream, const su3::ShiftInfo *sh = nullptr, bool one_shot = false) {
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  if (nmat == 0) return SU3_OK;
+  StreamPlan pl;
+  if (su3_status st = plan_stream(op, prec, W, nmat, footprint_bytes, sh != nullptr, one_shot, g_tune, di, &pl)) return st;
+  const int nin = su3::menu_prog(op).nin;
   stream_kernel_t k = nullptr;
   if (sh) k = su3tab::shift_pipe_kernel(prec, op, W);
-  else if (op <= su3::OP_ADD) k = prec == SU3_F64 ? su3tab::stream_f64(family, op, W) : su3tab::stream_f32(family, op, W);
+  else if (op <= su3::OP_ADD) k = prec == SU3_F64 ? su3tab::stream_f64(pl.family, op, W) : su3tab::stream_f32(pl.family, op, W);
   else k = prec == SU3_F64 ? su3tab::menu_f64(op, W) : su3tab::menu_f32(op, W);
   if (!k) return fail(SU3_ERR_INVALID, "no kernel for op %d prec %d W %d", op, prec, W);
 
@@ -197,80 +296,12 @@ su3_status launch_stream(int op, int prec, int W, void *z, const void *const *in
   p.z = z; p.x = in[0]; p.y = nin > 1 ? in[1] : nullptr; p.u = nin > 2 ? in[2] : nullptr; p.v = nin > 3 ? in[3] : nullptr;
   p.nmat = nmat;
   if (sh) p.sh = *sh;
-
-  if (warp) {
-    p.tile_mats = 32; p.stages = 0;
-    const int64_t nwt = (nmat + 31) / 32;
-    int wpb = 4;  // warps per block; fewer on small lattices so that every SM gets a block
-    while (wpb > 1 && (nwt + wpb - 1) / wpb < 2 * (int64_t)di.sms) wpb >>= 1;
-    const size_t smem = (size_t)wpb * nin * 288 * cb;
+  p.tile_mats = pl.tile_mats; p.stages = pl.stages; p.hint = pl.hint; p.pin_tiles = pl.pin_tiles;
+  if (pl.family != su3tab::FAM_DIRECT) {
     cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
     if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
-    const int64_t blocks_needed = (nwt + wpb - 1) / wpb;
-    const int64_t cap = (int64_t)di.sms * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 8) * (4 / wpb);
-    k<<<(unsigned)(blocks_needed < cap ? blocks_needed : cap), wpb * 32, smem, stream>>>(p);
-  } else if (direct) {
-    p.tile_mats = 0; p.stages = 0;
-    int bs = 256;  // small lattices: smaller blocks so that every SM gets one
-    while (bs > 32 && (nmat + bs - 1) / bs < 2 * (int64_t)di.sms) bs >>= 1;
-    const int64_t blocks_needed = (nmat + bs - 1) / bs;
-    const int64_t cap = (int64_t)di.sms * 8 * (tn.ctas_per_sm > 0 ? tn.ctas_per_sm : 1) * (256 / bs);
-    const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    k<<<grid, bs, 0, stream>>>(p);
-  } else {
-    // defaults measured on B200: 9 KB operand slots (64 fp64 / 128 fp32 matrices),
-    // a 3-deep ring, 2 persistent CTAs per SM
-    // 2 persistent CTAs per SM; 3 for the copy through a shifted slot (Cshift of 72-byte records with odd run boundaries:
-    // no arithmetic to hide behind, measured 0.81 -> 0.96 x copy)
-    int ctas = tn.ctas_per_sm > 0 ? tn.ctas_per_sm : (sh && nin == 1 ? 3 : 2);
-    int tm = tn.tile_mats;
-    if (tm == 0) {
-      tm = 9216 / (9 * cb);
-      // small lattices: shrink the tile until every persistent CTA has at least two tiles
-      while (tm > 32 && (nmat + tm - 1) / tm < 2 * (int64_t)di.sms * ctas) tm >>= 1;
-    }
-    if (tm != 32 && tm != 64 && tm != 128) return fail(SU3_ERR_INVALID, "tile_mats = %d not in {32,64,128}", tm);
-    const size_t stage_bytes = (size_t)nslot * tm * 9 * cb + (sh ? 16 : 0);
-    // 1 KB of every CTA's shared memory is reserved by the system; keep 256 B for the barriers
-    size_t budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
-    // auto CTAs/SM: a big tile may leave room for fewer resident CTAs than the default
-    while (tn.ctas_per_sm == 0 && ctas > 1 && (budget - 256) / stage_bytes < 2) {
-      ctas--;
-      budget = ((size_t)di.smem_optin + 1024) / ctas - 1024;
-    }
-    const int64_t max_grid = (int64_t)di.sms * ctas;
-    int stages = tn.stages;
-    if (stages == 0) {
-      // ring depth 3 at HBM-bound sizes (deeper rings open more DRAM pages at once and measured 1-3 % slower from 40^4
-      // fp32 / 36^4 fp64 on); up to 3 x L2 a good part of the loads hits L2, latency rather than DRAM limits a 20-70 us
-      // launch, and more bytes in flight pay: depth 4 measured +4..12 % at 20^4-28^4 fp64 and 24^4-36^4 fp32 (ncu at
-      // 24^4 with depth 3, warm: DRAM 44 % busy, profiles/r02_knee.md)
-      stages = footprint_bytes <= (size_t)di.l2 * 3 ? 4 : 3;
-      while (stages > 2 && stages * stage_bytes + 256 > budget) stages--;
-    }
-    if (stages < 2 || stages > 16) return fail(SU3_ERR_INVALID, "stages = %d outside 2..16 (tile %d, %d CTAs/SM)", stages, tm, ctas);
-    const size_t smem = stages * stage_bytes + 3 * stages * sizeof(uint64_t);
-    if (smem > (size_t)di.smem_optin) return fail(SU3_ERR_INVALID, "pipeline needs %zu B of shared memory, device allows %d", smem, di.smem_optin);
-    cudaError_t e = allow_max_smem((const void *)k, di.smem_optin);
-    if (e != cudaSuccess) return cuda_fail("cudaFuncSetAttribute", e);
-    p.tile_mats = tm; p.stages = stages;
-    // L2 policy (l2_hint): 0/1 none (evict_first measured neutral at every HBM-bound size), 2 evict_first
-    // everywhere, 3 keep the first l2_pin_mb MB of every operand in L2 (evict_last) and stream the rest (evict_first)
-    p.hint = tn.l2_hint == 2 ? 1 : (tn.l2_hint == 3 ? 2 : 0);
-    size_t pin_bytes = (size_t)tn.l2_pin_mb * 1000000;   // per operand
-    if (tn.l2_hint == 0 && footprint_bytes > (size_t)di.l2 * 6 / 10 && footprint_bytes <= (size_t)di.l2 * 2) {
-      // auto, footprint between 0.6 and 2 x L2 ("straddling"): a plain LRU keeps NOTHING of a cyclic sweep that is a
-      // little larger than the cache; keeping ~36 % of L2 worth of operand prefixes resident from one call to the next
-      // (Listing 3 repeats z = x*y on the same fields) and streaming the rest measured +32 % at 24^4 fp64, +7 % at
-      // 32^4 fp32; beyond 2 x L2 the same policy costs 2-4 %, so it is not applied there
-      p.hint = 2;
-      pin_bytes = (size_t)di.l2 * 36 / 100 / nin;
-    }
-    if (p.hint == 2) p.pin_tiles = (int64_t)(pin_bytes / ((size_t)tm * 9 * cb));
-    const int64_t ntiles = (nmat + tm - 1) / tm;
-    const unsigned grid = (unsigned)(ntiles < max_grid ? ntiles : max_grid);
-    k<<<grid, (NCW + 1) * 32, smem, stream>>>(p);
   }
+  k<<<pl.grid, pl.block, pl.smem, stream>>>(p);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail("kernel launch", e);
   g_launches.fetch_add(1, std::memory_order_relaxed);
@@ -1277,7 +1308,7 @@ su3_status su3_eval_host(int op, void *z_host, const void *x_host, const void *y
     SU3_CK(cudaEventRecord(ev_in, g_hp.h2d));
     SU3_CK(cudaStreamWaitEvent(user, ev_in, 0));
     const void *in[4] = {(const char *)xd->ptr + off, (const char *)yd->ptr + off, has_u ? (const char *)ud->ptr + off : nullptr, nullptr};
-    st = launch_stream(op, prec, W, (char *)zd->ptr + off, in, nm, (has_u ? 4 : 3) * zd->nbytes, user);
+    st = launch_stream(op, prec, W, (char *)zd->ptr + off, in, nm, (has_u ? 4 : 3) * zd->nbytes, user, nullptr, /*one_shot=*/true);
     if (st != SU3_OK) return st;
     SU3_CK(cudaEventRecord(ev_k, user));
     SU3_CK(cudaStreamWaitEvent(g_hp.d2h, ev_k, 0));
@@ -1310,6 +1341,26 @@ su3_status su3_host_release(void) {
   }
   if (have) cudaSetDevice(cur);
   (void)cudaGetLastError();
+  return SU3_OK;
+}
+
+su3_status su3_launch_plan(const su3_desc *desc, int op, char *buf, size_t buf_len) {
+  if (!buf || buf_len == 0) return fail(SU3_ERR_NULL, "buf is NULL or empty");
+  if (op != SU3_OP_MUL && op != SU3_OP_MUL3 && op != SU3_OP_MUL_ADD) return fail(SU3_ERR_INVALID, "op = %d not in {0,1,2}", op);
+  su3_desc d;
+  if (su3_status st = normalize(desc, &d)) return st;
+  const DevInfo &di = devinfo();
+  if (!di.ok) return fail(SU3_ERR_CUDA, "%s", di.err);
+  const int64_t nmat = volume_of(d) * d.n_lorentz;
+  const size_t field = (size_t)nmat * 18 * d.prec;
+  const int kop = op == SU3_OP_MUL ? su3::OP_MUL : (op == SU3_OP_MUL3 ? su3::OP_MUL3 : su3::OP_MUL_ADD);
+  StreamPlan pl;
+  if (su3_status st = plan_stream(kop, d.prec, d.W, nmat, field * (op == SU3_OP_MUL ? 3 : 4), false, false, g_tune, di, &pl)) return st;
+  const char *fam = pl.family == su3tab::FAM_WARP ? "warp" : (pl.family == su3tab::FAM_DIRECT ? "direct" : "pipe");
+  const char *l2 = pl.hint == 2 ? "pin" : (pl.hint == 1 ? "evict_first" : "none");
+  const int n = snprintf(buf, buf_len, "%s tile=%d depth=%d ctas=%d grid=%u block=%d smem=%zu l2=%s pin_bytes=%zu", fam, pl.tile_mats,
+                         pl.stages, pl.ctas, pl.grid, pl.block, pl.smem, l2, pl.pin_bytes);
+  if (n < 0 || (size_t)n >= buf_len) return fail(SU3_ERR_SIZE, "plan needs %d bytes, buf has %zu", n + 1, buf_len);
   return SU3_OK;
 }
 
