@@ -100,6 +100,16 @@ def test_48x4_fp32_scalar_and_W8_mul_whole_field():
     whole_field(48, 1, F32, [(SC, 1), (VE, 8)], su3gen.config_seed(5), ["mul"])
 
 
+def test_64x4_fp32_scalar_and_W8_mul_whole_field():
+    """config 5's largest fp32 points, every element (the sampled comparison of test_gpu_fullsize.py covers 1 524 sites)"""
+    whole_field(64, 1, F32, [(SC, 1), (VE, 8)], su3gen.config_seed(5), ["mul"], check_convert=False)
+
+
+def test_64x4_fp64_W4_mul_whole_field():
+    """config 5's top point in the vector layout, every element, inputs permuted on the host by the oracle"""
+    whole_field(64, 1, F64, [(VE, 4)], su3gen.config_seed(5), ["mul"], check_convert=False)
+
+
 def test_64x4_fp64_mul_whole_field_then_soak():
     """the bench workload's A1 launch: every element against the oracle once, then 50 launches back to back
     (5 at a time into 5 different outputs, so that consecutive launches overlap their drain and fill) must all
