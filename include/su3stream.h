@@ -233,7 +233,10 @@ su3_status su3_copy(su3_field *dst, const su3_field *src, void *cuda_stream);
  *   su3_face_pack  : buffer <- planes of x          su3_face_unpack: planes of z <- buffer
  *   su3_face_copy  : planes [z_plane0, +n) of z <- planes [x_plane0, +n) of x, same descriptor; x may be memory of a PEER
  *                    device mapped into this process (NVLink P2P): the exchange is then this single launch.
- * plane range outside 0..L[dim] -> SU3_ERR_INVALID; buffer too small -> SU3_ERR_SIZE, misaligned -> SU3_ERR_ALIGN. */
+ * plane range outside 0..L[dim] -> SU3_ERR_INVALID; buffer too small -> SU3_ERR_SIZE, misaligned -> SU3_ERR_ALIGN; a buffer
+ * that is plain device memory of another GPU which the current one cannot reach as a peer -> SU3_ERR_MISMATCH (the runtime
+ * is asked where the pointer lives; whether peer access has been ENABLED stays the caller's responsibility, as does the
+ * residency of pinned or managed buffers). */
 su3_status su3_face_bytes(const su3_field *f, int dim, int nplanes, size_t *nbytes);
 su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, int dim, int plane0, int nplanes, void *cuda_stream);
 su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, int dim, int plane0, int nplanes, void *cuda_stream);

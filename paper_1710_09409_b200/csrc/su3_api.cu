@@ -1179,6 +1179,25 @@ static su3_status launch_face_copy(const su3_field *geo, void *dst, bool dpacked
   return SU3_OK;
 }
 
+// The packed buffer is a raw pointer, not a handle: ask the runtime where it lives (as su3_field_wrap does for fields).
+// Plain device memory of ANOTHER device that the current one cannot reach as a peer would fault asynchronously inside
+// the kernel; it is refused here instead.  Anything the runtime cannot classify (no device, unregistered host memory)
+// and pinned / managed memory pass: their residency is the caller's business.
+static su3_status face_buffer_reachable(const void *buf) {
+  cudaPointerAttributes at;
+  int cur = 0;
+  if (cudaPointerGetAttributes(&at, buf) == cudaSuccess && at.type == cudaMemoryTypeDevice && cudaGetDevice(&cur) == cudaSuccess &&
+      at.device != cur) {
+    int can = 0;
+    if (cudaDeviceCanAccessPeer(&can, cur, at.device) != cudaSuccess || !can) {
+      (void)cudaGetLastError();
+      return fail(SU3_ERR_MISMATCH, "the face buffer is memory of device %d, which device %d (current) cannot access as a peer", at.device, cur);
+    }
+  }
+  (void)cudaGetLastError();
+  return SU3_OK;
+}
+
 su3_status su3_face_bytes(const su3_field *f, int dim, int nplanes, size_t *nbytes) {
   if (!nbytes) return fail(SU3_ERR_NULL, "nbytes is NULL");
   return face_args(f, dim, 0, nplanes, nbytes);
@@ -1191,6 +1210,7 @@ su3_status su3_face_pack(void *buf_dev, size_t buf_bytes, const su3_field *x, in
   if ((uintptr_t)buf_dev % 16) return fail(SU3_ERR_ALIGN, "face buffer is not 16-byte aligned");
   if (buf_bytes < need) return fail(SU3_ERR_SIZE, "face buffer has %zu bytes, the face needs %zu", buf_bytes, need);
   if (su3_status sd = on_current_device({x})) return sd;
+  if (su3_status sb = face_buffer_reachable(buf_dev)) return sb;
   return launch_face_copy(x, buf_dev, true, 0, x->ptr, false, plane0, dim, nplanes, stream);
 }
 
@@ -1201,6 +1221,7 @@ su3_status su3_face_unpack(su3_field *z, const void *buf_dev, size_t buf_bytes, 
   if ((uintptr_t)buf_dev % 16) return fail(SU3_ERR_ALIGN, "face buffer is not 16-byte aligned");
   if (buf_bytes < need) return fail(SU3_ERR_SIZE, "face buffer has %zu bytes, the face needs %zu", buf_bytes, need);
   if (su3_status sd = on_current_device({z})) return sd;
+  if (su3_status sb = face_buffer_reachable(buf_dev)) return sb;
   return launch_face_copy(z, z->ptr, false, plane0, buf_dev, true, 0, dim, nplanes, stream);
 }
 
