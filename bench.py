@@ -458,7 +458,8 @@ def time_calls(torch, fn, target_ms=2.0, batches=10, warm=3, graph_below_us=0.0)
 
 def run_halo(args, r, world, rank):
     """The exchange step of the multi-GPU path, timed on every rank with CUDA events, max over ranks.
-    A tripwire checks the data that crossed: the last x3 plane of rank r's result must be the first plane of rank r+1's input."""
+    A tripwire checks the data that crossed: the last x3 plane of rank r's result must equal, bit for bit and in both
+    layouts, the first plane of rank r+1's input."""
     torch, su3, f, dist = r["torch"], r["su3"], r["f"], r["dist"]
     from paper_1710_09409_b200 import halo, shard
     sh = halo.SlabShift(halo.DistComm(dist))
@@ -478,14 +479,27 @@ def run_halo(args, r, world, rank):
             _, ms, _ = shard.job_throughput(1.0, a.elapsed_time(b) / 10, dist, r["dev"])
             res[label + "_ms"] = ms
             res[label + "_GBps_per_rank"] = 2 * y.nbytes / (ms * 1e-3) / 1e9
-        if lay == "scalar":
+        # tripwire on the data that crossed, in BOTH layouts and over the whole plane: the last x3 plane of my result must be,
+        # bit for bit, the first x3 plane of the next rank's input.  Planes are compared in the packed plane order
+        # (su3_face_pack), which is the same for every layout; the next rank's plane arrives over a ring send/recv.
+        try:
             sh.cshift(z, y, 3, 1)
+            nb = su3.su3_face_bytes(y, 3, 1)
+            first_in, last_out, nxt_in = (torch.empty(nb, dtype=torch.uint8, device=y.tensor.device) for _ in range(3))
+            su3.su3_face_pack(first_in, y, 3, 0, 1)
+            su3.su3_face_pack(last_out, z, 3, y.desc.L[3] - 1, 1)
             torch.cuda.synchronize()
-            plane = y.nbytes // y.desc.L[3]
-            mine = torch.stack([y.tensor[:plane].to(torch.int64).sum(), z.tensor[-plane:].to(torch.int64).sum()])
-            allv = [torch.zeros_like(mine) for _ in range(world)]
-            dist.all_gather(allv, mine)
-            res["face_checksum_ok"] = bool(all(int(allv[k][1]) == int(allv[(k + 1) % world][0]) for k in range(world)))
+            works = dist.batch_isend_irecv([dist.P2POp(dist.isend, first_in, (rank - 1) % world),
+                                            dist.P2POp(dist.irecv, nxt_in, (rank + 1) % world)])
+            for w in works:
+                w.wait()
+            torch.cuda.synchronize()
+            ok = torch.tensor([1 if torch.equal(nxt_in, last_out) else 0], device=y.tensor.device)
+            dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+            res["face_plane_bit_equal"] = bool(int(ok.item()) == 1)
+        except Exception as e:  # the opt-in leg must not take the bench line down with it
+            res["face_plane_bit_equal"] = None
+            res["face_check_error"] = "%s: %s" % (type(e).__name__, e)
         out.append(res)
     return out
 
